@@ -1,0 +1,102 @@
+/* lgo.h — ORACLE (test infrastructure, not product code).
+ *
+ * Plain, slow, single-threaded CPU implementation of the paper's plan evaluation
+ * (arxiv 1909.10286, /root/reference/PAPER.md) with the readings listed in DESIGN.md.
+ * It shares no code with the CUDA path under paper_1909_10286_b200/csrc/: only tests/,
+ * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may load it.
+ *
+ * Every function below cites the passage of PAPER.md it follows.
+ * Pins (tests/test_oracle_*.py): Philox known answers + cuRAND header; hand toy A (P1);
+ * Alg. 2 traces B and C (P2, P3); decoder / score invariants (P4, P5); brute force (P8).
+ */
+#ifndef LGO_H
+#define LGO_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LGO_OK       0
+#define LGO_EINVAL  (-1)
+#define LGO_ETOOBIG (-2)
+#define LGO_ENOMEM  (-4)
+
+#define LGO_Q 1024   /* quanta per unit (t, ha, ha/h); R18 */
+
+/* Same field order as the product's lgx_instance_desc (restated, not shared). */
+typedef struct {
+  double   hq_x, hq_y;
+  int32_t  n_fields;   const double *field_x, *field_y, *field_supply_t, *field_area_ha;
+  int32_t  n_bps;      const double *bp_x, *bp_y, *bp_demand_t;
+  int32_t  n_hu_total; const double *hu_rate_ha_per_h;
+  int32_t  n_su_total; const double *su_capacity_t;
+  int32_t  n_tours;
+  double   v_hu_road_kmh, v_su_road_kmh, v_infield_kmh;
+  double   su_fill_h_per_t;
+  double   w_path, w_time;
+  uint32_t extra_field_thresh;
+  uint32_t flags;
+} lgo_instance_desc;
+
+typedef struct lgo_instance lgo_instance;
+
+int  lgo_instance_create (const lgo_instance_desc *desc, lgo_instance **out);
+int  lgo_instance_destroy(lgo_instance *inst);
+
+/* S1: one Philox4x32-10 block. key=(seed_lo,seed_hi), counter=(id_lo,id_hi,stream,block). */
+void lgo_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+/* S1: draw d of stream s for (seed,id) = word d%4 of block d/4. */
+uint32_t lgo_draw(uint64_t seed, uint64_t id, uint32_t stream, uint32_t d);
+
+/* S0: distance between vertices (0=HQ, 1..N_B=BPs, then fields), quantised inputs. */
+double  lgo_distance(const lgo_instance *inst, int32_t u, int32_t v);
+int64_t lgo_quantum(const lgo_instance *inst, int what, int32_t i); /* 0 s_q,1 h_q,2 d_q,3 r_q,4 c_q */
+
+/* S2+S3: decode (seed,id) into an explicit plan.  Arrays are caller-allocated:
+ * bp_tour[N_B], bp_pos[N_B]  : tour of each BP and its position on that tour
+ * field_bp[N_F], field_pos[N_F]: BP of each field and its position in that BP's list
+ * hu_tour[N_HU], su_tour[N_SU]: tour of each unit (S2)                                */
+int lgo_decode(const lgo_instance *inst, uint64_t seed, uint64_t id,
+               uint8_t *bp_tour, uint8_t *bp_pos, uint16_t *field_bp, uint16_t *field_pos,
+               uint8_t *hu_tour, uint8_t *su_tour);
+
+/* S4-S7: score an explicit plan.  Any of the array outputs may be NULL.
+ * scalars[8] = {feasible(0/1), L_HU, L_eSU, L_lSU, path_km, makespan_h, cost, n_alg2_moves}
+ * infeasible: scalars[1..6] = +inf.                                                     */
+int lgo_score(const lgo_instance *inst,
+              const uint8_t *bp_tour, const uint8_t *bp_pos,
+              const uint16_t *field_bp, const uint16_t *field_pos,
+              const uint8_t *hu_tour, const uint8_t *su_tour_init,
+              double *scalars,
+              double *tour_route_km,      /* [N_T] L_tour(g)                 */
+              double *tour_time_h,        /* [N_T] T(g)                      */
+              double *tour_E_h,           /* [N_T] E(g)                      */
+              double *tour_wait_h,        /* [N_T] T_wait(g) after Alg. 2    */
+              double *tour_len_km,        /* [N_T] L(g)                      */
+              int64_t *bp_supply_q,       /* [N_B] S_q(b)                    */
+              int64_t *field_shuttles,    /* [N_F] eq. (4) count             */
+              uint8_t *su_tour_final);    /* [N_SU]                          */
+
+/* S6 alone (Algorithm 2) on explicit numbers, for traces B and C.
+ * cap_q: capacities in quanta; su_tour in/out; wait_h out; returns accepted moves.    */
+int lgo_su_local_min(int32_t n_tours, const double *E_h, const int32_t *n_hu,
+                     int32_t n_su, const int64_t *cap_q, uint8_t *su_tour,
+                     double kappa_h_per_t, double *wait_h);
+
+/* eval = score o decode on host arrays; ids==NULL => ids = first_id + i. */
+int lgo_eval_batch(const lgo_instance *inst, uint64_t seed, const uint64_t *ids,
+                   uint64_t first_id, uint64_t n,
+                   double *cost, double *path_km, double *makespan_h, uint8_t *feasible);
+int lgo_decode_batch(const lgo_instance *inst, uint64_t seed, const uint64_t *ids,
+                     uint64_t first_id, uint64_t n,
+                     uint8_t *bp_tour, uint8_t *bp_pos, uint16_t *field_bp, uint16_t *field_pos,
+                     uint8_t *hu_tour, uint8_t *su_tour_init, uint8_t *su_tour_final);
+/* S8: ordered min over ids [first_id, first_id+budget) of (cost bits, id). */
+int lgo_search(const lgo_instance *inst, uint64_t seed, uint64_t first_id, uint64_t budget,
+               double *best_cost, uint64_t *best_id);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
