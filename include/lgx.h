@@ -1,0 +1,117 @@
+/* lgx.h — C ABI of lgx: B200-native mass evaluation of biomass-logistics plans.
+ *
+ * Hot path of arxiv 1909.10286 (M. Graf Plessen, "GPU-accelerated Logistics Optimisation
+ * for Biomass Production with Multiple Simultaneous Harvesters Tours, Fields and Plants";
+ * citations are lines of /root/reference/PAPER.md): every candidate plan is decoded from
+ * (seed, id), checked against the BP demand constraints (eq. (2)), scored by the
+ * path-length criterion of §2.2 (L100-106) plus the maximum completion time (L190, L205)
+ * after the embedded SU assignment of Algorithm 2 (L209-227), and reduced to a global
+ * argmin (L167).  DESIGN.md states every reading (R1..R30) the paper leaves open.
+ *
+ * Conventions
+ *  - extern "C", no exceptions, no global state.  Return 0 (LGX_OK) or a negative code.
+ *  - "d_" pointers are DEVICE pointers (caller-allocated, e.g. torch tensors' data_ptr());
+ *    "h_" pointers and everything inside lgx_instance_desc are HOST pointers.
+ *  - cuda_stream is a cudaStream_t passed as void* (NULL = default stream).
+ *  - No CPU fallback: without a CUDA device every compute call returns LGX_ECUDA.
+ */
+#ifndef LGX_H
+#define LGX_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LGX_OK        0
+#define LGX_EINVAL   (-1)   /* bad argument / instance violates the documented ranges        */
+#define LGX_ETOOBIG  (-2)   /* instance image or per-candidate state does not fit on an SM   */
+#define LGX_ECUDA    (-3)   /* CUDA runtime error; text via lgx_strerror(LGX_ECUDA)          */
+#define LGX_ENOMEM   (-4)
+
+typedef struct lgx_instance lgx_instance;   /* opaque; owns host + device copies */
+
+/* Problem statement (Table 1 L51-65 and the list under it, L65; §2.1).
+ * All arrays are copied by lgx_instance_create; the caller may free them afterwards.   */
+typedef struct {
+  double   hq_x, hq_y;                       /* km; HQ, "at the origin" in §3.1 (L267)          */
+  int32_t  n_fields;                         /* N_F, 1..65535                                    */
+  const double *field_x, *field_y;           /* km, field centroids (Fig. 1, L21)                */
+  const double *field_supply_t;              /* s_f, expected supply (t), eq. (2)/(3) L79-85     */
+  const double *field_area_ha;               /* h_f (ha), L83                                    */
+  int32_t  n_bps;                            /* N_B, 1..255                                      */
+  const double *bp_x, *bp_y;                 /* km                                               */
+  const double *bp_demand_t;                 /* d_b^min (t), eq. (2)                         */
+  int32_t  n_hu_total;                       /* N_HU^total, eq. (1)                          */
+  const double *hu_rate_ha_per_h;            /* v_HU^area per unit (ha/h), L96 (ii), classes L75 */
+  int32_t  n_su_total;                       /* N_SU^total, eq. (1)                          */
+  const double *su_capacity_t;               /* l_SU^load per unit (t), L87                      */
+  int32_t  n_tours;                          /* N_T <= min(N_B, N_HU^total, N_SU^total) (L69)    */
+  double   v_hu_road_kmh, v_su_road_kmh;     /* v_HU^edge, v_SU^edge (Table 1: 40, 40)           */
+  double   v_infield_kmh;                    /* configs only; stored, not used by the cost (R24) */
+  double   su_fill_h_per_t;                  /* kappa: t_SU^load = kappa * capacity (L96 (iii))  */
+  double   w_path, w_time;                   /* cost = w_path*path_km + w_time*makespan_h (R1)   */
+  uint32_t extra_field_thresh;               /* decoder knob: P(extra field) = thresh / 2^32     */
+  uint32_t flags;                            /* reserved, must be 0                              */
+} lgx_instance_desc;
+
+/* Instance encoder.  Quantises supply/area/demand/rate/capacity to Q=1024
+ * quanta, builds the shared-memory image (distance tables or coordinates, unit tables) and
+ * uploads it.  Errors: LGX_EINVAL (null pointer, n_tours out of range, non-finite or
+ * negative input, zero rate/capacity/velocity, counts beyond the ranges above),
+ * LGX_ETOOBIG (integer ranges: max s_q*N_SU + sum c_q, sum s_q, sum h_q, sum r_q, d_q must
+ * stay below 2^32; or the per-candidate state does not fit in 227 KB of shared memory),
+ * LGX_ECUDA, LGX_ENOMEM.                                                                    */
+int lgx_instance_create (const lgx_instance_desc *desc, lgx_instance **out);
+int lgx_instance_destroy(lgx_instance *inst);
+
+/* Candidate decoder + tour simulator + demand check + Algorithm 2 + cost (a2..a6), one
+ * candidate per thread.  ids: d_ids[i] if d_ids != NULL, else first_id + i.  Row i of every
+ * output belongs to candidate i; any output pointer may be NULL.  Infeasible candidates
+ * (eq. (2) violated) get feasible=0 and +inf in the three doubles.
+ * Asynchronous on cuda_stream.                                                              */
+int lgx_eval_batch(const lgx_instance *inst, uint64_t seed,
+                   const uint64_t *d_ids, uint64_t first_id, uint64_t n,
+                   double *d_cost, double *d_path_km, double *d_makespan_h, uint8_t *d_feasible,
+                   void *cuda_stream);
+
+/* Same, with HOST buffers: copies ids in (if given) and results out inside the call
+ * (chunked, synchronous).  Used for the end-to-end number in bench.py.                     */
+int lgx_eval_batch_host(const lgx_instance *inst, uint64_t seed,
+                        const uint64_t *h_ids, uint64_t first_id, uint64_t n,
+                        double *h_cost, double *h_path_km, double *h_makespan_h, uint8_t *h_feasible);
+
+/* a2..a7: evaluate ids [first_id, first_id + n) and return the ordered minimum of
+ * (cost bit pattern, id): lowest cost, lowest id on ties (R29).  No feasible
+ * candidate => *h_best_cost = +inf and *h_best_id = first_id.  n == 0 => LGX_EINVAL.
+ * Synchronises cuda_stream before returning; results go to host pointers.                  */
+int lgx_search_range(const lgx_instance *inst, uint64_t seed, uint64_t first_id, uint64_t n,
+                     double *h_best_cost, uint64_t *h_best_id, void *cuda_stream);
+/* lgx_search(budget) == lgx_search_range(0, budget). */
+int lgx_search(const lgx_instance *inst, uint64_t seed, uint64_t budget,
+               double *h_best_cost, uint64_t *h_best_id, void *cuda_stream);
+
+/* Diagnostic export of decoded plans (needed for the "plans bit-exact" parity clause).
+ * Layouts: d_bp_tour/d_bp_pos [n][N_B] (tour of BP b, its position on that tour);
+ * d_field_bp/d_field_pos [n][N_F] (BP of field f, its position in that BP's list);
+ * d_hu_tour [n][N_HU]; d_su_tour_init / d_su_tour_final [n][N_SU] (before / after Alg. 2;
+ * equal for infeasible candidates).  Any pointer may be NULL.  Asynchronous.               */
+int lgx_decode_batch(const lgx_instance *inst, uint64_t seed,
+                     const uint64_t *d_ids, uint64_t first_id, uint64_t n,
+                     uint8_t *d_bp_tour, uint8_t *d_bp_pos,
+                     uint16_t *d_field_bp, uint16_t *d_field_pos,
+                     uint8_t *d_hu_tour, uint8_t *d_su_tour_init, uint8_t *d_su_tour_final,
+                     void *cuda_stream);
+
+/* Introspection for bench.py / tests: what = 0 image bytes, 1 threads per block,
+ * 2 blocks in the persistent grid, 3 dynamic shared memory bytes per block,
+ * 4 distance mode (0 = packed table in smem, 1 = coordinates), 5 per-candidate state bytes,
+ * 6 SM count, 7 kernel launches issued so far through this instance.                       */
+int lgx_instance_query(const lgx_instance *inst, int what, int64_t *out);
+
+const char *lgx_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

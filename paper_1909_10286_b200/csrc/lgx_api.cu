@@ -1,0 +1,363 @@
+// lgx_api.cu — C ABI of lgx (include/lgx.h): instance encoder (host side) and launchers.
+// Product code (CUDA path); shares nothing with oracle/.  No CPU fallback: every compute
+// entry point fails with LGX_ECUDA when there is no usable CUDA device.
+#include "../../include/lgx.h"
+#include "lgx_image.h"
+#include "lgx_kernels.cuh"
+
+#include <algorithm>
+#include <atomic>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <numeric>
+#include <string>
+#include <vector>
+
+using namespace lgx;
+
+struct lgx_instance {
+  ImgHdr hdr{};
+  std::vector<uint8_t> image;      // host copy of the image
+  uint8_t *d_image = nullptr;      // device copy
+  int device = 0, sm_count = 0;
+  int threads = 0, grid = 0;       // launch configuration of the persistent kernels
+  size_t smem_bytes = 0;
+  mutable std::atomic<long long> launches{0};
+};
+
+namespace {
+
+thread_local std::string g_cuda_msg = "no CUDA error recorded";
+
+int cuda_fail(cudaError_t e, const char *where)
+{
+  g_cuda_msg = std::string(where) + ": " + cudaGetErrorString(e);
+  cudaGetLastError();
+  return LGX_ECUDA;
+}
+#define CU(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return cuda_fail(e__, #call); } while (0)
+
+inline bool fin_nonneg(double v) { return std::isfinite(v) && v >= 0.0; }
+inline int64_t quantise(double v) { return (int64_t)std::llrint(v * (double)kQ); }   // round-half-even (R18)
+
+inline uint32_t align16(uint32_t v) { return (v + 15u) & ~15u; }
+
+// Straight-line edge, one rounding per operation (compiled with -ffp-contract=off).
+inline double edge(double ax, double ay, double bx, double by)
+{
+  const double dx = ax - bx, dy = ay - by;
+  const double xx = dx * dx, yy = dy * dy;
+  const double ss = xx + yy;
+  return std::sqrt(ss);
+}
+
+using KernelFn = void (*)(const KParams);
+
+template <int MODE> KernelFn pick_kernel(const ImgHdr &h)
+{
+  const bool p16 = h.perm16 != 0, co = h.coords != 0; const int mw = (int)h.mask_words;
+#define LGX_PICK(P, C, M) if (p16 == P && co == C && mw == M) return lgx_candidates<P, C, M, MODE>;
+  LGX_PICK(false, false, 1) LGX_PICK(false, false, 2) LGX_PICK(false, true, 1) LGX_PICK(false, true, 2)
+  LGX_PICK(true,  false, 1) LGX_PICK(true,  false, 2) LGX_PICK(true,  true, 1) LGX_PICK(true,  true, 2)
+#undef LGX_PICK
+  return nullptr;
+}
+
+void fill_round_keys(KParams &P, uint64_t seed)
+{
+  uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+  for (int r = 0; r < 10; ++r) { P.rk[2 * r] = k0; P.rk[2 * r + 1] = k1; k0 += kPhiloxW0; k1 += kPhiloxW1; }
+}
+
+int launch(const lgx_instance *I, KernelFn fn, KParams &P, cudaStream_t st)
+{
+  if (!fn) return LGX_EINVAL;
+  CU(cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)I->smem_bytes));
+  P.image = I->d_image; P.image_bytes = I->hdr.image_bytes;
+  const uint64_t blocks_needed = (P.n + (uint64_t)I->threads - 1) / (uint64_t)I->threads;
+  const unsigned grid = (unsigned)std::min<uint64_t>((uint64_t)I->grid, std::max<uint64_t>(blocks_needed, 1));
+  void *args[] = { (void *)&P };
+  CU(cudaLaunchKernel((const void *)fn, dim3(grid), dim3((unsigned)I->threads), args, I->smem_bytes, st));
+  I->launches.fetch_add(1);
+  return LGX_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *lgx_strerror(int code)
+{
+  switch (code) {
+    case LGX_OK:      return "ok";
+    case LGX_EINVAL:  return "invalid argument or instance outside the documented ranges";
+    case LGX_ETOOBIG: return "instance image or per-candidate state does not fit (shared memory / 32-bit quanta)";
+    case LGX_ECUDA:   return g_cuda_msg.c_str();
+    case LGX_ENOMEM:  return "out of memory";
+    default:          return "unknown lgx error code";
+  }
+}
+
+int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
+{
+  if (!d || !out) return LGX_EINVAL;
+  *out = nullptr;
+  // ---- validation (same documented rules as the header; PAPER.md:L69 N_T <= N_HU^total)
+  if (d->n_fields < 1 || d->n_bps < 1 || d->n_hu_total < 1 || d->n_su_total < 1) return LGX_EINVAL;
+  if (d->n_tours < 1 || d->n_tours > d->n_bps || d->n_tours > d->n_hu_total || d->n_tours > d->n_su_total) return LGX_EINVAL;
+  if (d->n_fields > 65535 || d->n_bps > 255 || d->n_tours > 255 || d->n_hu_total > 255 || d->n_su_total > 255) return LGX_EINVAL;
+  if (!d->field_x || !d->field_y || !d->field_supply_t || !d->field_area_ha || !d->bp_x || !d->bp_y ||
+      !d->bp_demand_t || !d->hu_rate_ha_per_h || !d->su_capacity_t) return LGX_EINVAL;
+  if (!std::isfinite(d->hq_x) || !std::isfinite(d->hq_y)) return LGX_EINVAL;
+  if (!(std::isfinite(d->v_hu_road_kmh) && d->v_hu_road_kmh > 0.0)) return LGX_EINVAL;
+  if (!(std::isfinite(d->v_su_road_kmh) && d->v_su_road_kmh > 0.0)) return LGX_EINVAL;
+  if (!fin_nonneg(d->su_fill_h_per_t) || !fin_nonneg(d->w_path) || !fin_nonneg(d->w_time)) return LGX_EINVAL;
+  if (d->flags != 0u) return LGX_EINVAL;
+  const int nf = d->n_fields, nb = d->n_bps, nhu = d->n_hu_total, nsu = d->n_su_total, nt = d->n_tours;
+  for (int f = 0; f < nf; ++f)
+    if (!std::isfinite(d->field_x[f]) || !std::isfinite(d->field_y[f]) || !fin_nonneg(d->field_supply_t[f]) ||
+        !fin_nonneg(d->field_area_ha[f])) return LGX_EINVAL;
+  for (int b = 0; b < nb; ++b)
+    if (!std::isfinite(d->bp_x[b]) || !std::isfinite(d->bp_y[b]) || !fin_nonneg(d->bp_demand_t[b])) return LGX_EINVAL;
+  for (int u = 0; u < nhu; ++u) if (!fin_nonneg(d->hu_rate_ha_per_h[u])) return LGX_EINVAL;
+  for (int u = 0; u < nsu; ++u) if (!fin_nonneg(d->su_capacity_t[u])) return LGX_EINVAL;
+
+  // ---- quantisation (Q = 1024) and the documented 32-bit ranges
+  std::vector<int64_t> s_q(nf), h_q(nf), d_q(nb), r_q(nhu), c_q(nsu);
+  int64_t s_max = 0, s_sum = 0, h_sum = 0, r_sum = 0, c_sum = 0;
+  for (int f = 0; f < nf; ++f) {
+    s_q[f] = quantise(d->field_supply_t[f]); h_q[f] = quantise(d->field_area_ha[f]);
+    s_max = std::max(s_max, s_q[f]); s_sum += s_q[f]; h_sum += h_q[f];
+  }
+  for (int b = 0; b < nb; ++b) d_q[b] = quantise(d->bp_demand_t[b]);
+  for (int u = 0; u < nhu; ++u) { r_q[u] = quantise(d->hu_rate_ha_per_h[u]); if (r_q[u] <= 0) return LGX_EINVAL; r_sum += r_q[u]; }
+  for (int u = 0; u < nsu; ++u) { c_q[u] = quantise(d->su_capacity_t[u]); if (c_q[u] <= 0) return LGX_EINVAL; c_sum += c_q[u]; }
+  const int64_t lim = (int64_t)1 << 32;
+  if (s_max * (int64_t)nsu + c_sum >= lim || s_sum >= lim || h_sum >= lim || r_sum >= lim) return LGX_ETOOBIG;
+  for (int b = 0; b < nb; ++b) if (d_q[b] >= lim) return LGX_ETOOBIG;
+  // kernel limits of this build
+  if (nb > 127 || nsu > 128) return LGX_ETOOBIG;
+
+  lgx_instance *I = new (std::nothrow) lgx_instance();
+  if (!I) return LGX_ENOMEM;
+  ImgHdr &H = I->hdr;
+  H.n_f = nf; H.n_b = nb; H.n_hu = nhu; H.n_su = nsu; H.n_t = nt;
+  H.thresh = d->extra_field_thresh;
+  H.v_hu = d->v_hu_road_kmh; H.v_su = d->v_su_road_kmh; H.kappa = d->su_fill_h_per_t;
+  H.w_path = d->w_path; H.w_time = d->w_time;
+  H.perm16 = nf > 255 ? 1 : 0;
+  H.mask_words = nsu > 64 ? 2u : 1u;
+
+  // ---- per-candidate state rows (32-bit words per thread)
+  const uint32_t per_word = H.perm16 ? 2u : 4u;
+  const uint32_t n_small = (uint32_t)std::max(nb, std::max(nhu, nsu));
+  uint32_t row = 0;
+  H.row_perm   = row; row += ((uint32_t)nf + per_word - 1) / per_word;
+  H.row_bpseq  = row; row += ((uint32_t)nb + 3) / 4;
+  H.row_segend = row; row += ((uint32_t)nb + per_word - 1) / per_word;
+  H.row_scra   = row; row += (n_small + 3) / 4;
+  H.row_scrb   = row; row += ((uint32_t)nb + 3) / 4;
+  H.tour_words = TR_MASK + 2u * H.mask_words;
+  H.row_tour   = row; row += (uint32_t)nt * H.tour_words;
+  H.words_per_thread = row;
+
+  // ---- image: packed distance tables when they leave room for >= 256 candidates per SM,
+  //      else vertex coordinates
+  const uint64_t tri_bytes = (uint64_t)(nf + 1) * (uint64_t)nf / 2 * 8, dfb_bytes = (uint64_t)nf * nb * 8;
+  const uint64_t small_bytes = sizeof(ImgHdr) + 8ull * nf + 4ull * (nb + nhu + nsu) + 2ull * nsu + 256;
+  const uint64_t state_256 = 256ull * 4ull * H.words_per_thread;
+  H.coords = (small_bytes + tri_bytes + dfb_bytes + state_256 > (uint64_t)kMaxSmem - 1024) ? 1 : 0;
+
+  uint32_t off = (uint32_t)sizeof(ImgHdr);
+  if (!H.coords) {
+    H.off_dtri = off; off = align16(off + (uint32_t)tri_bytes);
+    H.off_dfb  = off; off = align16(off + (uint32_t)dfb_bytes);
+    H.off_xy = 0;
+  } else {
+    H.off_dtri = H.off_dfb = 0;
+    H.off_xy = off; off = align16(off + 16u * (uint32_t)(1 + nb + nf));
+  }
+  H.off_sh   = off; off = align16(off + 8u * (uint32_t)nf);
+  H.off_dq   = off; off = align16(off + 4u * (uint32_t)nb);
+  H.off_rq   = off; off = align16(off + 4u * (uint32_t)nhu);
+  H.off_cs   = off; off = align16(off + 4u * (uint32_t)nsu);
+  H.off_rank = off; off = align16(off + (uint32_t)nsu);
+  H.off_unit = off; off = align16(off + (uint32_t)nsu);
+  H.image_bytes = off;
+
+  I->image.assign(off, 0);
+  uint8_t *img = I->image.data();
+  if (!H.coords) {
+    // strict lower triangle over {HQ = 0, field f = f + 1}: entry (hi, lo) at hi(hi-1)/2 + lo
+    double *tri = reinterpret_cast<double *>(img + H.off_dtri);
+    for (int hi = 1; hi <= nf; ++hi)
+      for (int lo = 0; lo < hi; ++lo) {
+        const double ax = d->field_x[hi - 1], ay = d->field_y[hi - 1];
+        const double bx = lo ? d->field_x[lo - 1] : d->hq_x, by = lo ? d->field_y[lo - 1] : d->hq_y;
+        tri[(size_t)hi * (hi - 1) / 2 + lo] = edge(ax, ay, bx, by);
+      }
+    double *dfb = reinterpret_cast<double *>(img + H.off_dfb);
+    for (int f = 0; f < nf; ++f)
+      for (int b = 0; b < nb; ++b) dfb[(size_t)f * nb + b] = edge(d->field_x[f], d->field_y[f], d->bp_x[b], d->bp_y[b]);
+  } else {
+    double *xy = reinterpret_cast<double *>(img + H.off_xy);
+    xy[0] = d->hq_x; xy[1] = d->hq_y;
+    for (int b = 0; b < nb; ++b) { xy[2 * (1 + b)] = d->bp_x[b]; xy[2 * (1 + b) + 1] = d->bp_y[b]; }
+    for (int f = 0; f < nf; ++f) { xy[2 * (1 + nb + f)] = d->field_x[f]; xy[2 * (1 + nb + f) + 1] = d->field_y[f]; }
+  }
+  uint32_t *sh = reinterpret_cast<uint32_t *>(img + H.off_sh);
+  for (int f = 0; f < nf; ++f) { sh[2 * f] = (uint32_t)s_q[f]; sh[2 * f + 1] = (uint32_t)h_q[f]; }
+  uint32_t *dq = reinterpret_cast<uint32_t *>(img + H.off_dq);
+  for (int b = 0; b < nb; ++b) dq[b] = (uint32_t)d_q[b];
+  uint32_t *rq = reinterpret_cast<uint32_t *>(img + H.off_rq);
+  for (int u = 0; u < nhu; ++u) rq[u] = (uint32_t)r_q[u];
+  // SUs ascending by (capacity quanta, unit index): "rising fill times" (R16, R17)
+  std::vector<int> order(nsu);
+  std::iota(order.begin(), order.end(), 0);
+  std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return c_q[a] < c_q[b]; });
+  uint32_t *cs = reinterpret_cast<uint32_t *>(img + H.off_cs);
+  for (int r = 0; r < nsu; ++r) { cs[r] = (uint32_t)c_q[order[r]]; img[H.off_unit + r] = (uint8_t)order[r]; img[H.off_rank + order[r]] = (uint8_t)r; }
+  std::memcpy(img, &H, sizeof(ImgHdr));
+
+  // ---- device: launch configuration and upload
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess || ndev < 1) { delete I; return cuda_fail(e != cudaSuccess ? e : cudaErrorNoDevice, "cudaGetDeviceCount"); }
+  if ((e = cudaGetDevice(&I->device)) != cudaSuccess) { delete I; return cuda_fail(e, "cudaGetDevice"); }
+  int smem_optin = 0;
+  cudaDeviceGetAttribute(&I->sm_count, cudaDevAttrMultiProcessorCount, I->device);
+  cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, I->device);
+  const int64_t budget = std::min<int64_t>(smem_optin, kMaxSmem) - 1024;   // static smem of the reduction
+  int64_t t = (budget - (int64_t)H.image_bytes) / (4ll * H.words_per_thread);
+  t = std::min<int64_t>(t, kMaxThreads) / 32 * 32;
+  if (t < 32) { delete I; return LGX_ETOOBIG; }
+  I->threads = (int)t;
+  I->grid = I->sm_count;                       // one persistent block per SM
+  I->smem_bytes = (size_t)H.image_bytes + 4ull * H.words_per_thread * (size_t)I->threads;
+  if ((e = cudaMalloc((void **)&I->d_image, H.image_bytes)) != cudaSuccess) { delete I; return cuda_fail(e, "cudaMalloc(image)"); }
+  if ((e = cudaMemcpy(I->d_image, img, H.image_bytes, cudaMemcpyHostToDevice)) != cudaSuccess) {
+    cudaFree(I->d_image); delete I; return cuda_fail(e, "cudaMemcpy(image)");
+  }
+  *out = I;
+  return LGX_OK;
+}
+
+int lgx_instance_destroy(lgx_instance *I)
+{
+  if (!I) return LGX_EINVAL;
+  if (I->d_image) cudaFree(I->d_image);
+  delete I;
+  return LGX_OK;
+}
+
+int lgx_instance_query(const lgx_instance *I, int what, int64_t *out)
+{
+  if (!I || !out) return LGX_EINVAL;
+  switch (what) {
+    case 0: *out = I->hdr.image_bytes; break;
+    case 1: *out = I->threads; break;
+    case 2: *out = I->grid; break;
+    case 3: *out = (int64_t)I->smem_bytes; break;
+    case 4: *out = I->hdr.coords; break;
+    case 5: *out = 4ll * I->hdr.words_per_thread; break;
+    case 6: *out = I->sm_count; break;
+    case 7: *out = I->launches.load(); break;
+    default: return LGX_EINVAL;
+  }
+  return LGX_OK;
+}
+
+int lgx_eval_batch(const lgx_instance *I, uint64_t seed, const uint64_t *d_ids, uint64_t first_id, uint64_t n,
+                   double *d_cost, double *d_path_km, double *d_makespan_h, uint8_t *d_feasible, void *stream)
+{
+  if (!I) return LGX_EINVAL;
+  if (n == 0) return LGX_OK;
+  KParams P{};
+  fill_round_keys(P, seed);
+  P.ids = d_ids; P.first_id = first_id; P.n = n;
+  P.cost = d_cost; P.path_km = d_path_km; P.makespan_h = d_makespan_h; P.feasible = d_feasible;
+  return launch(I, pick_kernel<MODE_EVAL>(I->hdr), P, (cudaStream_t)stream);
+}
+
+int lgx_decode_batch(const lgx_instance *I, uint64_t seed, const uint64_t *d_ids, uint64_t first_id, uint64_t n,
+                     uint8_t *d_bp_tour, uint8_t *d_bp_pos, uint16_t *d_field_bp, uint16_t *d_field_pos,
+                     uint8_t *d_hu_tour, uint8_t *d_su_tour_init, uint8_t *d_su_tour_final, void *stream)
+{
+  if (!I) return LGX_EINVAL;
+  if (n == 0) return LGX_OK;
+  KParams P{};
+  fill_round_keys(P, seed);
+  P.ids = d_ids; P.first_id = first_id; P.n = n;
+  P.bp_tour = d_bp_tour; P.bp_pos = d_bp_pos; P.field_bp = d_field_bp; P.field_pos = d_field_pos;
+  P.hu_tour = d_hu_tour; P.su_init = d_su_tour_init; P.su_final = d_su_tour_final;
+  return launch(I, pick_kernel<MODE_DECODE>(I->hdr), P, (cudaStream_t)stream);
+}
+
+int lgx_search_range(const lgx_instance *I, uint64_t seed, uint64_t first_id, uint64_t n,
+                     double *h_best_cost, uint64_t *h_best_id, void *stream)
+{
+  if (!I || !h_best_cost || !h_best_id || n == 0) return LGX_EINVAL;
+  cudaStream_t st = (cudaStream_t)stream;
+  // scratch: [grid][2] block minima, [2] result, done counter
+  const size_t words = 2ull * (size_t)I->grid + 2 + 1;
+  unsigned long long *d_scratch = nullptr;
+  CU(cudaMallocAsync((void **)&d_scratch, words * sizeof(unsigned long long), st));
+  cudaError_t e = cudaMemsetAsync(d_scratch, 0, words * sizeof(unsigned long long), st);
+  if (e != cudaSuccess) { cudaFreeAsync(d_scratch, st); return cuda_fail(e, "cudaMemsetAsync"); }
+  KParams P{};
+  fill_round_keys(P, seed);
+  P.ids = nullptr; P.first_id = first_id; P.n = n;
+  P.block_best = d_scratch; P.result = d_scratch + 2ull * I->grid;
+  P.done_counter = reinterpret_cast<unsigned int *>(d_scratch + 2ull * I->grid + 2);
+  int rc = launch(I, pick_kernel<MODE_SEARCH>(I->hdr), P, st);
+  unsigned long long res[2] = {0, 0};
+  if (rc == LGX_OK) {
+    e = cudaMemcpyAsync(res, P.result, sizeof res, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) rc = cuda_fail(e, "lgx_search: copy/synchronize");
+  }
+  cudaFreeAsync(d_scratch, st);
+  if (rc != LGX_OK) return rc;
+  std::memcpy(h_best_cost, &res[0], 8);
+  *h_best_id = res[1];
+  return LGX_OK;
+}
+
+int lgx_search(const lgx_instance *I, uint64_t seed, uint64_t budget, double *h_best_cost, uint64_t *h_best_id, void *stream)
+{
+  return lgx_search_range(I, seed, 0, budget, h_best_cost, h_best_id, stream);
+}
+
+int lgx_eval_batch_host(const lgx_instance *I, uint64_t seed, const uint64_t *h_ids, uint64_t first_id, uint64_t n,
+                        double *h_cost, double *h_path_km, double *h_makespan_h, uint8_t *h_feasible)
+{
+  if (!I) return LGX_EINVAL;
+  if (n == 0) return LGX_OK;
+  const uint64_t chunk = std::min<uint64_t>(n, 1ull << 22);
+  uint64_t *d_ids = nullptr; double *d_c = nullptr, *d_p = nullptr, *d_m = nullptr; uint8_t *d_f = nullptr;
+  int rc = LGX_OK;
+  cudaError_t e = cudaSuccess;
+  auto cleanup = [&]() { cudaFree(d_ids); cudaFree(d_c); cudaFree(d_p); cudaFree(d_m); cudaFree(d_f); };
+  if (h_ids && (e = cudaMalloc((void **)&d_ids, chunk * 8)) != cudaSuccess) { cleanup(); return cuda_fail(e, "cudaMalloc"); }
+  if (h_cost && (e = cudaMalloc((void **)&d_c, chunk * 8)) != cudaSuccess) { cleanup(); return cuda_fail(e, "cudaMalloc"); }
+  if (h_path_km && (e = cudaMalloc((void **)&d_p, chunk * 8)) != cudaSuccess) { cleanup(); return cuda_fail(e, "cudaMalloc"); }
+  if (h_makespan_h && (e = cudaMalloc((void **)&d_m, chunk * 8)) != cudaSuccess) { cleanup(); return cuda_fail(e, "cudaMalloc"); }
+  if (h_feasible && (e = cudaMalloc((void **)&d_f, chunk)) != cudaSuccess) { cleanup(); return cuda_fail(e, "cudaMalloc"); }
+  for (uint64_t o = 0; o < n && rc == LGX_OK; o += chunk) {
+    const uint64_t m = std::min<uint64_t>(chunk, n - o);
+    if (h_ids && (e = cudaMemcpyAsync(d_ids, h_ids + o, m * 8, cudaMemcpyHostToDevice, 0)) != cudaSuccess) { rc = cuda_fail(e, "H2D ids"); break; }
+    rc = lgx_eval_batch(I, seed, h_ids ? d_ids : nullptr, first_id + o, m, d_c, d_p, d_m, d_f, nullptr);
+    if (rc != LGX_OK) break;
+    if (h_cost && (e = cudaMemcpyAsync(h_cost + o, d_c, m * 8, cudaMemcpyDeviceToHost, 0)) != cudaSuccess) { rc = cuda_fail(e, "D2H"); break; }
+    if (h_path_km && (e = cudaMemcpyAsync(h_path_km + o, d_p, m * 8, cudaMemcpyDeviceToHost, 0)) != cudaSuccess) { rc = cuda_fail(e, "D2H"); break; }
+    if (h_makespan_h && (e = cudaMemcpyAsync(h_makespan_h + o, d_m, m * 8, cudaMemcpyDeviceToHost, 0)) != cudaSuccess) { rc = cuda_fail(e, "D2H"); break; }
+    if (h_feasible && (e = cudaMemcpyAsync(h_feasible + o, d_f, m, cudaMemcpyDeviceToHost, 0)) != cudaSuccess) { rc = cuda_fail(e, "D2H"); break; }
+    if ((e = cudaStreamSynchronize(0)) != cudaSuccess) { rc = cuda_fail(e, "cudaStreamSynchronize"); break; }
+  }
+  cleanup();
+  return rc;
+}
+
+}  // extern "C"

@@ -1,0 +1,190 @@
+"""GPU parity (-m gpu): the CUDA path through the C ABI against the oracle, element by
+element on the same seeded inputs.  Bar (BASELINE.json north_star): decoded plans and
+feasibility flags bit-exact, FP64 costs within 1e-9 relative (the kernels reproduce the
+oracle's operation order, so the tests first assert bit equality and report the relative
+error if that ever fails), identical argmin id."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from oracle import lgo
+from paper_1909_10286_b200 import binding, workloads as wl
+from helpers import mk_instance
+
+RTOL = 1e-9
+N_ORACLE = {"toy": 1 << 16, "small": 1 << 15, "medium": 1 << 14, "large": 1 << 12, "sweep": 3 << 10, "paper_scale": 1 << 9}
+
+
+@pytest.fixture(scope="module")
+def ctxs():
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the product path must fail loudly, not fall back")
+    cache = {}
+    def get(name):
+        if name not in cache:
+            inst = wl.make(name)
+            cache[name] = (inst, lgo.Oracle(inst), binding.Instance(inst))
+        return cache[name]
+    return get
+
+
+def id_sets(inst, n):
+    """first n ids, n ids sampled over the whole budget (incl. >= 2^31 for the big configs),
+    and the last n ids of the budget."""
+    yield "first", None, 0
+    yield "sampled", wl.sample_ids(inst.budget, n), 0
+    yield "last", None, inst.budget - n
+
+
+def assert_costs(got, want, what):
+    got = np.asarray(got); want = np.asarray(want)
+    fin = np.isfinite(want)
+    assert np.array_equal(np.isfinite(got), fin), what
+    if not np.array_equal(got[fin], want[fin]):
+        rel = np.abs(got[fin] - want[fin]) / np.abs(want[fin])
+        assert rel.max() <= RTOL, f"{what}: max rel err {rel.max():.3e}"
+        pytest.fail(f"{what}: within {RTOL} (max rel {rel.max():.3e}) but not bit-equal — operation order drifted")
+
+
+@pytest.mark.parametrize("name", ["toy", "small", "medium", "large", "sweep"])
+def test_eval_batch_matches_oracle(ctxs, name):
+    inst, o, g = ctxs(name)
+    n = N_ORACLE[name]
+    for label, ids, first in id_sets(inst, n):
+        want = o.eval_batch(inst.seed, ids=ids, first_id=first, n=n)
+        d_ids = torch.from_numpy(ids.astype(np.int64)).cuda() if ids is not None else None
+        got = [t.cpu().numpy() for t in g.eval_batch(inst.seed, ids=d_ids, first_id=first, n=n)]
+        assert np.array_equal(got[3], want[3]), f"{name}/{label}: feasibility flags differ"
+        for k, nm in enumerate(("cost", "path_km", "makespan_h")):
+            assert_costs(got[k], want[k], f"{name}/{label}/{nm}")
+        assert 0 < want[3].mean() <= 1.0
+
+
+@pytest.mark.parametrize("name", ["toy", "small", "medium", "large", "sweep"])
+def test_decode_batch_matches_oracle(ctxs, name):
+    inst, o, g = ctxs(name)
+    n = max(256, N_ORACLE[name] // 8)
+    for label, ids, first in id_sets(inst, n):
+        want = o.decode_batch(inst.seed, ids=ids, first_id=first, n=n)
+        d_ids = torch.from_numpy(ids.astype(np.int64)).cuda() if ids is not None else None
+        got = g.decode_batch(inst.seed, ids=d_ids, first_id=first, n=n)
+        torch.cuda.synchronize()
+        for key in want:
+            a = got[key].cpu().numpy()
+            if a.dtype == np.int16: a = a.view(np.uint16)
+            assert np.array_equal(a, want[key]), f"{name}/{label}: plan array {key} differs"
+
+
+@pytest.mark.parametrize("name,budget", [("toy", 1 << 16), ("small", 1 << 17), ("medium", 1 << 16),
+                                         ("large", 1 << 13), ("sweep", 1 << 12)])
+def test_search_matches_oracle_argmin(ctxs, name, budget):
+    inst, o, g = ctxs(name)
+    want_c, want_i = o.search(inst.seed, budget)
+    got_c, got_i = g.search(inst.seed, budget)
+    assert got_i == want_i and got_c == want_c
+    # a window that does not start at 0 (multi-GPU shards use these)
+    first = inst.budget - budget
+    want_c, want_i = o.search(inst.seed, budget // 4, first_id=first)
+    got_c, got_i = g.search(inst.seed, budget // 4, first_id=first)
+    assert got_i == want_i and got_c == want_c
+
+
+def test_search_equals_min_of_eval_batch_at_scale(ctxs):
+    """Self-consistency beyond the oracle's reach: search over 2^22 ids of Medium equals the
+    ordered min of eval_batch outputs, and the winner re-scores to the same cost in the oracle."""
+    inst, o, g = ctxs("medium")
+    n = 1 << 22
+    cost = g.eval_batch(inst.seed, first_id=0, n=n)[0]
+    c, i = g.search(inst.seed, n)
+    cmin = cost.min().item()
+    assert c == cmin and i == int((cost == cmin).nonzero()[0].item())
+    assert o.score(o.decode(inst.seed, i))["cost"] == c
+
+
+def test_full_budget_tail_ids_sampled(ctxs):
+    """At the full budgets (2^30, 2^32) single sampled ids near the top of the range decode
+    and score identically (64-bit id handling)."""
+    for name in ("large", "sweep"):
+        inst, o, g = ctxs(name)
+        ids = np.array([inst.budget - 1, inst.budget - 2, (1 << 31) + 5, (1 << 31) - 1, inst.budget // 2 + 1], dtype=np.uint64)
+        want = o.eval_batch(inst.seed, ids=ids)
+        got = [t.cpu().numpy() for t in g.eval_batch(inst.seed, ids=torch.from_numpy(ids.astype(np.int64)).cuda())]
+        assert np.array_equal(got[3], want[3])
+        assert np.array_equal(got[0], want[0])
+    # ids beyond 2^32 and a non-zero seed
+    inst, o, g = ctxs("small")
+    ids = np.array([(1 << 40) + 3, (1 << 63) + 11, 2**64 - 1], dtype=np.uint64)
+    seed = 0xDEADBEEFCAFEF00D
+    want = o.eval_batch(seed, ids=ids)
+    got = [t.cpu().numpy() for t in g.eval_batch(seed, ids=torch.from_numpy(ids.view(np.int64)).cuda())]
+    assert np.array_equal(got[3], want[3]) and np.array_equal(got[0], want[0])
+
+
+def test_edge_cases(ctxs):
+    # hand toy A through the CUDA path: every candidate is the same plan up to field order
+    a = mk_instance((0, 0), [(3, 4, 25, 1), (6, 8, 40, 2)], [(6, 0, 60)], [2.0], [10.0, 10.0], 1)
+    g = binding.Instance(a); o = lgo.Oracle(a)
+    cost, path, mk, fe = [t.cpu().numpy() for t in g.eval_batch(0, first_id=0, n=100)]
+    assert np.all(fe == 1) and np.all(path == 154.0) and np.all(mk == 2.0) and np.all(cost == 156.0)
+    assert g.search(0, 100, first_id=7) == (156.0, 7)          # ties: lowest id
+    # all infeasible: +inf and the lowest id
+    b = mk_instance((0, 0), [(3, 4, 25, 1), (6, 8, 40, 2)], [(6, 0, 66)], [2.0], [10.0, 10.0], 1)
+    gb = binding.Instance(b)
+    c, i = gb.search(0, 1000, first_id=5)
+    assert np.isinf(c) and i == 5
+    out = [t.cpu().numpy() for t in gb.eval_batch(0, first_id=0, n=33)]
+    assert np.all(out[3] == 0) and np.all(np.isinf(out[0])) and np.all(np.isinf(out[1])) and np.all(np.isinf(out[2]))
+    # n = 0 is a no-op; budget 0 is an error
+    g.eval_batch(0, first_id=0, n=0)
+    with pytest.raises(binding.LgxError):
+        g.search(0, 0)
+    # ragged sizes around the block/grid granularity
+    inst, om, gm = ctxs("medium")
+    for n in (1, 31, 33, 511, 513, 148 * 512 + 1):
+        want = om.eval_batch(0, first_id=3, n=min(n, 2000))
+        got = [t.cpu().numpy() for t in gm.eval_batch(0, first_id=3, n=n)]
+        assert np.array_equal(got[0][:2000], want[0]) and np.array_equal(got[3][:2000], want[3])
+    # zero-demand BPs and thresh extremes (decoder degenerate paths)
+    for thresh in (0, 0xFFFFFFFF, 0x40000000):
+        z = wl.make("small"); z.bp_demand_t = z.bp_demand_t.copy(); z.bp_demand_t[[1, 3]] = 0.0
+        z.extra_field_thresh = thresh
+        oz, gz = lgo.Oracle(z), binding.Instance(z)
+        want = oz.eval_batch(1, first_id=0, n=4096)
+        got = [t.cpu().numpy() for t in gz.eval_batch(1, first_id=0, n=4096)]
+        assert np.array_equal(got[3], want[3]) and np.array_equal(got[0], want[0])
+        wd = oz.decode_batch(1, first_id=0, n=512); gd = gz.decode_batch(1, first_id=0, n=512)
+        for key in wd:
+            a_ = gd[key].cpu().numpy()
+            if a_.dtype == np.int16: a_ = a_.view(np.uint16)
+            assert np.array_equal(a_, wd[key]), key
+    # N_T = N_B = N_HU = N_SU (every bin exactly one item) and N_T = 1
+    for nt in (1, 5):
+        z = wl.make("small"); z.n_tours = nt
+        if nt == 5:
+            z.hu_rate_ha_per_h = z.hu_rate_ha_per_h[:5].copy(); z.su_capacity_t = z.su_capacity_t[:5].copy()
+        oz, gz = lgo.Oracle(z), binding.Instance(z)
+        want = oz.eval_batch(2, first_id=0, n=2048)
+        got = [t.cpu().numpy() for t in gz.eval_batch(2, first_id=0, n=2048)]
+        assert np.array_equal(got[3], want[3]) and np.array_equal(got[0], want[0])
+
+
+def test_eval_batch_host_buffers(ctxs):
+    inst, o, g = ctxs("small")
+    ids = wl.sample_ids(inst.budget, 5000)
+    want = o.eval_batch(inst.seed, ids=ids)
+    got = g.eval_batch_host(inst.seed, ids=ids)
+    assert np.array_equal(got[3], want[3]) and np.array_equal(got[0], want[0])
+    got = g.eval_batch_host(inst.seed, first_id=10, n=(1 << 22) + 17)       # crosses a chunk boundary
+    want = o.eval_batch(inst.seed, first_id=10 + (1 << 22) - 8, n=25)
+    assert np.array_equal(got[0][(1 << 22) - 8:], want[0])
+
+
+def test_paper_scale_workload(ctxs):
+    """NEXT row N4: the paper's own problem shape (1200 fields, 20 BPs, 7 tours; L267)."""
+    inst, o, g = ctxs("paper_scale")
+    n = N_ORACLE["paper_scale"]
+    want = o.eval_batch(inst.seed, first_id=0, n=n)
+    got = [t.cpu().numpy() for t in g.eval_batch(inst.seed, first_id=0, n=n)]
+    assert np.array_equal(got[3], want[3]) and np.array_equal(got[0], want[0])
