@@ -1,0 +1,281 @@
+#!/usr/bin/env python
+"""bench.py — candidates/s of the lgx hot path on B200 (BASELINE.json metric).
+
+A "step" is one pass of the whole hot path (SURVEY §8(a) rows a2..a7 in one persistent
+kernel over the shared-memory image built by a1) over one batch of candidates:
+`lgx_search` over the Medium config's full budget (2^28 ids, 100 fields / 8 BPs / 5 tours;
+the config the north_star target of >= 1e9 cand/s is quoted on).  Synthetic, seeded
+instance (paper_1909_10286_b200/workloads.py); nothing is read from /root/reference.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload medium]
+
+Prints ONE JSON line (rank 0).  `value` is device-timed (CUDA events on the launching
+stream, max over ranks) with the instance image resident in HBM; `e2e` re-creates the
+instance from HOST arrays (H2D of the image) and reads the result back to the host inside
+the timed region, through the C ABI.  `--impl reference` times the CPU oracle instead.
+"""
+from __future__ import annotations
+import argparse, json, os, subprocess, sys, threading, time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "candidate plans evaluated/sec"
+UNIT = "candidates/s"
+# Algorithmic thread-instructions per candidate (derived per config from
+# the minimal per-field / per-unit / per-move instruction counts of the method itself).
+W_ALG = {"toy": 2300, "small": 6200, "medium": 13900, "large": 42500, "sweep": 86500}
+SM_MAX_MHZ_FALLBACK = 1965.0
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        return json.load(open(p)), "measured"
+    except Exception:      # noqa: BLE001
+        return {"sm_max_mhz": SM_MAX_MHZ_FALLBACK, "hbm_gbs": 6650.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks/throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True); self.t.start()
+        except Exception:  # noqa: BLE001
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try: self.proc.wait(2)
+        except Exception: self.proc.kill()  # noqa: BLE001,E701
+        sm = sorted(float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit())
+        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for k, n in enumerate(names) if any(len(r) >= 7 and r[3 + k].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def oracle_rate(name, n_ids, procs):
+    """The oracle as it stands (single-threaded by design), run as `procs` independent
+    processes over disjoint contiguous id ranges on the host cores."""
+    import multiprocessing as mp
+    ctx = mp.get_context("fork")
+    per = max(1, n_ids // procs)
+    with ctx.Pool(procs) as pool:
+        t0 = time.perf_counter()
+        res = pool.starmap(_oracle_chunk, [(name, r * per, per) for r in range(procs)])
+        dt = time.perf_counter() - t0
+    best = min(res, key=lambda p: (p[0], p[1]))
+    return per * procs / dt, dt, best
+
+
+def _oracle_chunk(name, first, n):
+    from oracle import lgo
+    from paper_1909_10286_b200 import workloads as wl
+    inst = wl.make(name)
+    o = lgo.Oracle(inst)
+    return o.search(inst.seed, n, first_id=first)
+
+
+def run_reference(args):
+    """--impl reference: the oracle (the only reference implementation of this tier)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    cores = os.cpu_count() or 1
+    sample = 1 << 19          # ids per step; ~0.5 s per step on 8 cores for Medium
+    for _ in range(args.warmup):
+        oracle_rate(args.workload, sample // 4, cores)
+    tot_t, tot_n = 0.0, 0
+    for _ in range(args.steps):
+        r, dt, _ = oracle_rate(args.workload, sample, cores)
+        tot_t += dt; tot_n += (sample // cores) * cores
+    v = tot_n / tot_t
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": args.workload, "ids_per_step": sample},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": f"{sample} ids/step of the {args.workload} budget, {cores} processes"},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="lgx", choices=["lgx", "reference"])
+    ap.add_argument("--workload", default="medium")
+    ap.add_argument("--batch-log2", type=int, default=None, help="candidates per GPU per step (default: config budget, capped 2^28)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "lgx" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import numpy as np
+    import torch
+    from paper_1909_10286_b200 import binding, workloads as wl, sharding
+
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    inst = wl.make(args.workload)
+    per_gpu = 1 << (args.batch_log2 if args.batch_log2 is not None else min(28, inst.budget.bit_length() - 1))
+    total = per_gpu * world                      # weak scaling: fixed ids per GPU
+    g = binding.Instance(inst)
+    info = g.info()
+    stream = torch.cuda.current_stream()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step(first_total=0):
+        # this rank's contiguous share of [0, total); one 16-byte exchange when world > 1
+        if world == 1:
+            return g.search(inst.seed, per_gpu, first_id=first_total)
+        return sharding.search_sharded(lambda s, n, f: g.search(s, n, first_id=f), inst.seed, total, rank, world, first_total)
+
+    for _ in range(args.warmup):
+        step()
+    # ---- timed: EXACTLY K steps, device time from CUDA events on the launching stream
+    sampler = ClockSampler(local); sampler.start()
+    launches0 = g.query(7)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    t_wall0 = time.perf_counter()
+    best = None
+    for k in range(args.steps):
+        flush.fill_(k & 0xFF)                    # L2 flush between timed iterations (untimed)
+        ev[k][0].record(stream)
+        best = step()
+        ev[k][1].record(stream)
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    launches = g.query(7) - launches0
+    clocks = sampler.stop()
+    dev_ms = sum(a.elapsed_time(b) for a, b in ev)
+    if dist is not None:
+        t = torch.tensor([dev_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX); dev_ms = float(t.item())
+    value = total * args.steps / (dev_ms * 1e-3)
+
+    # ---- e2e: host arrays -> lgx_instance_create (H2D image) -> lgx_search -> host result
+    e2e_steps = max(2, min(args.steps, 3))
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        g2 = binding.Instance(inst)
+        if world == 1:
+            r2 = g2.search(inst.seed, per_gpu)
+        else:
+            r2 = sharding.search_sharded(lambda s, n, f: g2.search(s, n, first_id=f), inst.seed, total, rank, world)
+        g2.close()
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    if dist is not None:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX); e2e_s = float(t.item())
+    e2e_value = total * e2e_steps / e2e_s
+    assert r2 == best, "e2e result differs from the device-timed result"
+
+    # ---- eval_batch (per-candidate outputs) timed separately, device and host buffers
+    extra = {}
+    if rank == 0:
+        n_ev = 1 << 24
+        out = g.eval_batch(inst.seed, first_id=0, n=n_ev)
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream); g.eval_batch(inst.seed, first_id=0, n=n_ev, out=out); b.record(stream)
+        torch.cuda.synchronize()
+        ev_ms = a.elapsed_time(b)
+        n_h = 1 << 22
+        host_out = (np.empty(n_h), np.empty(n_h), np.empty(n_h), np.empty(n_h, np.uint8))
+        g.eval_batch_host(inst.seed, first_id=0, n=n_h, out=host_out)
+        t0 = time.perf_counter(); g.eval_batch_host(inst.seed, first_id=0, n=n_h, out=host_out); th = time.perf_counter() - t0
+        extra["eval_batch"] = {"value": n_ev / ev_ms * 1e3, "unit": UNIT, "ids": n_ev,
+                               "feasible_fraction": float(out[3].float().mean().item()),
+                               "e2e_host_buffers": {"value": n_h / th, "unit": UNIT, "ids": n_h,
+                                                    "d2h_bytes": 25 * n_h, "h2d_bytes": 0}}
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    pk, pk_src = peaks()
+    sm_max = float(pk.get("sm_max_mhz", SM_MAX_MHZ_FALLBACK))
+    n_sm = info["sm_count"]
+    peak_ginst = n_sm * 4 * 32 * sm_max * 1e6 / 1e9          # thread-instructions/s at max clock
+    per_launch_ms = dev_ms / args.steps
+    w_alg = W_ALG.get(args.workload)
+    achieved = (per_gpu * w_alg / (per_launch_ms * 1e-3) / 1e9) if w_alg else None
+    roofline = {"bound": "alu", "achieved": achieved, "peak": peak_ginst, "unit": "Ginst/s (thread instructions)",
+                "frac": (achieved / peak_ginst) if achieved else None, "traffic": None,
+                "kernel": "lgx_candidates<MODE_SEARCH>", "launch_ms": per_launch_ms,
+                "w_alg_thread_inst_per_candidate": w_alg,
+                "peak_source": f"{n_sm} SMs x 4 schedulers x 32 lanes x {sm_max:.0f} MHz ({pk_src} sm_max_mhz; DESIGN.md)",
+                "frac_at_observed_clock": (achieved / (peak_ginst * clocks["sm_mhz"] / sm_max)) if achieved and clocks.get("sm_mhz") else None}
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        cores = os.cpu_count() or 1
+        n_cpu = 1 << 21 if args.workload in ("toy", "small", "medium") else 1 << 18
+        rate, dt, cbest = oracle_rate(args.workload, n_cpu, cores)
+        cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"ids [0, {n_cpu // cores * cores}) of the {args.workload} budget, {cores} processes, {dt:.1f} s wall"}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": dev_ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{args.workload}: N_T={inst.n_tours} N_B={inst.n_bps} N_F={inst.n_fields} "
+                                   f"N_HU={inst.n_hu} N_SU={inst.n_su}",
+                       "candidates_per_gpu_per_step": per_gpu, "seed": inst.seed,
+                       "l2": "flushed between timed iterations (256 MiB write)",
+                       "parallelism": f"id-range shards x{world}", "threads_per_block": info["threads"],
+                       "grid": info["grid"], "smem_bytes": info["smem_bytes"]},
+            "best": {"cost": best[0], "id": best[1]},
+            "clocks": clocks, "gpu_launches": launches,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": info["image_bytes"],
+                    "d2h_bytes_per_step": 16, "steps": e2e_steps,
+                    "what": "lgx_instance_create(host arrays) + lgx_search + lgx_instance_destroy, wall clock"},
+            "wall_s_timed_region": t_wall, "roofline": roofline, "cpu_baseline": cpu}
+    line.update(extra)
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,60 @@
+"""Multi-GPU sharding of a search: candidates are independent functions of
+(seed, id), so [0, budget) is split into contiguous id ranges, one per rank; every rank holds
+a replica of the (<100 KB) instance and runs the same kernels; ONE exchange of 16 bytes per
+rank (cost bit pattern, id) follows and the ordered minimum is taken locally.  Contiguous,
+ordered ranges keep the lowest-id tie-break (R29).  No data-path collective."""
+from __future__ import annotations
+import struct
+
+
+def split_range(budget: int, world: int, rank: int, first_id: int = 0):
+    """Contiguous share of [first_id, first_id+budget) for `rank`: (first, n); n may be 0."""
+    if budget < 0 or world < 1 or not (0 <= rank < world):
+        raise ValueError("bad shard arguments")
+    base, rem = divmod(budget, world)
+    n = base + (1 if rank < rem else 0)
+    first = first_id + rank * base + min(rank, rem)
+    return first, n
+
+
+def cost_bits(cost: float) -> int:
+    """IEEE-754 bit pattern; for costs >= 0 (or +inf) it orders like the value."""
+    return struct.unpack("<Q", struct.pack("<d", cost))[0]
+
+
+def combine(pairs):
+    """Ordered minimum of (cost, id) pairs on (cost bits, id); ranks with no ids pass None."""
+    best = None
+    for p in pairs:
+        if p is None:
+            continue
+        key = (cost_bits(p[0]), p[1])
+        if best is None or key < best[0]:
+            best = (key, p)
+    if best is None:
+        raise ValueError("no rank evaluated any candidate")
+    return best[1]
+
+
+def search_sharded(search_fn, seed: int, budget: int, rank: int, world: int, first_id: int = 0):
+    """Run this rank's share through `search_fn(seed, n, first_id) -> (cost, id)` and
+    all-gather the 16-byte results with torch.distributed (NCCL on GPUs, gloo on CPU)."""
+    import torch
+    import torch.distributed as dist
+    first, n = split_range(budget, world, rank, first_id)
+    local = search_fn(seed, n, first) if n > 0 else None
+    if world == 1:
+        return combine([local])
+    dev = torch.device("cuda", torch.cuda.current_device()) if dist.get_backend() == "nccl" else torch.device("cpu")
+    # (valid, cost bits, id) as int64 words; bit patterns are moved, never re-rounded
+    def s64(v):
+        return v - (1 << 64) if v >= (1 << 63) else v
+    mine = torch.tensor([1 if local else 0, s64(cost_bits(local[0])) if local else 0,
+                         s64(local[1]) if local else 0], dtype=torch.int64, device=dev)
+    allr = [torch.empty_like(mine) for _ in range(world)]
+    dist.all_gather(allr, mine)
+    pairs = []
+    for t in allr:
+        v, b, i = (int(x) for x in t.cpu())
+        pairs.append((struct.unpack("<d", struct.pack("<Q", b % (1 << 64)))[0], i % (1 << 64)) if v else None)
+    return combine(pairs)
