@@ -75,7 +75,7 @@ int launch(const lgx_instance *I, KernelFn fn, KParams &P, cudaStream_t st)
 {
   if (!fn) return LGX_EINVAL;
   CU(cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)I->smem_bytes));
-  P.image = I->d_image; P.image_bytes = I->hdr.image_bytes;
+  P.image = I->d_image; P.H = I->hdr;
   const uint64_t blocks_needed = (P.n + (uint64_t)I->threads - 1) / (uint64_t)I->threads;
   const unsigned grid = (unsigned)std::min<uint64_t>((uint64_t)I->grid, std::max<uint64_t>(blocks_needed, 1));
   void *args[] = { (void *)&P };
@@ -166,7 +166,7 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   // ---- image: packed distance tables when they leave room for >= 256 candidates per SM,
   //      else vertex coordinates
   const uint64_t tri_bytes = (uint64_t)(nf + 1) * (uint64_t)nf / 2 * 8, dfb_bytes = (uint64_t)nf * nb * 8;
-  const uint64_t small_bytes = sizeof(ImgHdr) + 8ull * nf + 4ull * (nb + nhu + nsu) + 2ull * nsu + 256;
+  const uint64_t small_bytes = sizeof(ImgHdr) + 16ull * nf + 4ull * (nb + nhu + nsu) + 2ull * nsu + 8ull * (nb + nhu) + 256;
   const uint64_t state_256 = 256ull * 4ull * H.words_per_thread;
   H.coords = (small_bytes + tri_bytes + dfb_bytes + state_256 > (uint64_t)kMaxSmem - 1024) ? 1 : 0;
 
@@ -185,7 +185,11 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   H.off_cs   = off; off = align16(off + 4u * (uint32_t)nsu);
   H.off_rank = off; off = align16(off + (uint32_t)nsu);
   H.off_unit = off; off = align16(off + (uint32_t)nsu);
+  const int n_rcp = std::max(nf, std::max(nb, nhu)) + 1;
+  H.off_rcp  = off; off = align16(off + 8u * (uint32_t)n_rcp);
   H.image_bytes = off;
+  // stream-4 draws taken up front: (N_B-1) failures + geometric extras, with slack; <= 64
+  H.n_extra_blocks = (uint32_t)std::min(16, ((nb - 1) * 4 / 3 + 8 + 3) / 4);
 
   I->image.assign(off, 0);
   uint8_t *img = I->image.data();
@@ -219,6 +223,9 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return c_q[a] < c_q[b]; });
   uint32_t *cs = reinterpret_cast<uint32_t *>(img + H.off_cs);
   for (int r = 0; r < nsu; ++r) { cs[r] = (uint32_t)c_q[order[r]]; img[H.off_unit + r] = (uint8_t)order[r]; img[H.off_rank + order[r]] = (uint8_t)r; }
+  double *rcp = reinterpret_cast<double *>(img + H.off_rcp);
+  rcp[0] = 0.0;
+  for (int k = 1; k < n_rcp; ++k) rcp[k] = 1.0 / (double)k;          // correctly rounded reciprocals
   std::memcpy(img, &H, sizeof(ImgHdr));
 
   // ---- device: launch configuration and upload

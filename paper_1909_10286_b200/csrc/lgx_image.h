@@ -53,11 +53,12 @@ struct ImgHdr {
   uint32_t off_cs;          // u32 [n_su]             SU capacity quanta, ascending (c_q, unit)
   uint32_t off_rank;        // u8  [n_su]             unit -> rank
   uint32_t off_unit;        // u8  [n_su]             rank -> unit
+  uint32_t off_rcp;         // f64 [max(n_f,n_b,n_hu)+1]  RN(1/k), for the exact small-divisor division
   uint32_t row_perm, row_bpseq, row_segend, row_scra, row_scrb, row_tour;
   uint32_t tour_words, words_per_thread;
   uint32_t image_bytes;
   uint32_t mask_words;      // 64-bit words per SU mask (1 or 2)
-  uint32_t pad[2];
+  uint32_t n_extra_blocks;  // Philox blocks of stream 4 drawn up front (<= 16)
 };
 static_assert(sizeof(ImgHdr) % 16 == 0, "image header must keep 16-byte alignment");
 
