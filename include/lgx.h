@@ -103,10 +103,12 @@ int lgx_decode_batch(const lgx_instance *inst, uint64_t seed,
                      uint8_t *d_hu_tour, uint8_t *d_su_tour_init, uint8_t *d_su_tour_final,
                      void *cuda_stream);
 
-/* Introspection for bench.py / tests: what = 0 image bytes, 1 threads per block,
- * 2 blocks in the persistent grid, 3 dynamic shared memory bytes per block,
- * 4 distance mode (0 = packed table in smem, 1 = coordinates), 5 per-candidate state bytes,
- * 6 SM count, 7 kernel launches issued so far through this instance.                       */
+/* Introspection for bench.py / tests: what = 0 image bytes (both images), 1 threads per block
+ * of the decode/walk kernel, 2 blocks in the persistent grid, 3 its dynamic shared memory
+ * bytes per block, 4 distance mode (0 = packed tables in smem, 1 = coordinates),
+ * 5 per-candidate state bytes of the decode/walk kernel, 6 SM count, 7 kernel launches issued
+ * so far through this instance, 8 / 9 threads per block / shared memory bytes of the finish
+ * kernel, 10 candidates per kernel pair (chunk), 11 bytes per queue record.                 */
 int lgx_instance_query(const lgx_instance *inst, int what, int64_t *out);
 
 const char *lgx_strerror(int code);

@@ -139,7 +139,8 @@ class Instance:
         return v.value
 
     def info(self):
-        keys = ["image_bytes", "threads", "grid", "smem_bytes", "coords", "state_bytes", "sm_count", "launches"]
+        keys = ["image_bytes", "threads", "grid", "smem_bytes", "coords", "state_bytes", "sm_count", "launches",
+                "threads_finish", "smem_bytes_finish", "chunk", "record_bytes"]
         return {k: self.query(i) for i, k in enumerate(keys)}
 
     # -- lgx_eval_batch: device tensors in/out (torch), asynchronous on `stream`

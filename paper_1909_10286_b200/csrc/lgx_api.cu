@@ -19,11 +19,12 @@ using namespace lgx;
 
 struct lgx_instance {
   ImgHdr hdr{};
-  std::vector<uint8_t> image;      // host copy of the image
-  uint8_t *d_image = nullptr;      // device copy
+  std::vector<uint8_t> image, image_c;       // host copies of the two images
+  uint8_t *d_image = nullptr, *d_image_c = nullptr;
   int device = 0, sm_count = 0;
-  int threads = 0, grid = 0;       // launch configuration of the persistent kernels
-  size_t smem_bytes = 0;
+  int threads_a = 0, threads_c = 0, grid = 0;  // launch configuration of the persistent kernels
+  size_t smem_a = 0, smem_c = 0;
+  uint64_t chunk = 0;                          // candidates per decode/finish kernel pair
   mutable std::atomic<long long> launches{0};
 };
 
@@ -41,8 +42,8 @@ int cuda_fail(cudaError_t e, const char *where)
 
 inline bool fin_nonneg(double v) { return std::isfinite(v) && v >= 0.0; }
 inline int64_t quantise(double v) { return (int64_t)std::llrint(v * (double)kQ); }   // round-half-even (R18)
-
 inline uint32_t align16(uint32_t v) { return (v + 15u) & ~15u; }
+inline uint32_t cdiv(uint32_t a, uint32_t b) { return (a + b - 1u) / b; }
 
 // Straight-line edge, one rounding per operation (compiled with -ffp-contract=off).
 inline double edge(double ax, double ay, double bx, double by)
@@ -55,33 +56,20 @@ inline double edge(double ax, double ay, double bx, double by)
 
 using KernelFn = void (*)(const KParams);
 
-template <int MODE> KernelFn pick_kernel(const ImgHdr &h)
+template <int MODE> void pick_kernels(const ImgHdr &h, KernelFn &ka, KernelFn &kc)
 {
   const bool p16 = h.perm16 != 0, co = h.coords != 0; const int mw = (int)h.mask_words;
-#define LGX_PICK(P, C, M) if (p16 == P && co == C && mw == M) return lgx_candidates<P, C, M, MODE>;
+  ka = kc = nullptr;
+#define LGX_PICK(P, C, M) if (p16 == P && co == C && mw == M) { ka = lgx_decode_walk<P, C, M, MODE>; kc = lgx_finish<P, C, M, MODE>; }
   LGX_PICK(false, false, 1) LGX_PICK(false, false, 2) LGX_PICK(false, true, 1) LGX_PICK(false, true, 2)
   LGX_PICK(true,  false, 1) LGX_PICK(true,  false, 2) LGX_PICK(true,  true, 1) LGX_PICK(true,  true, 2)
 #undef LGX_PICK
-  return nullptr;
 }
 
 void fill_round_keys(KParams &P, uint64_t seed)
 {
   uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
   for (int r = 0; r < 10; ++r) { P.rk[2 * r] = k0; P.rk[2 * r + 1] = k1; k0 += kPhiloxW0; k1 += kPhiloxW1; }
-}
-
-int launch(const lgx_instance *I, KernelFn fn, KParams &P, cudaStream_t st)
-{
-  if (!fn) return LGX_EINVAL;
-  CU(cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)I->smem_bytes));
-  P.image = I->d_image; P.H = I->hdr;
-  const uint64_t blocks_needed = (P.n + (uint64_t)I->threads - 1) / (uint64_t)I->threads;
-  const unsigned grid = (unsigned)std::min<uint64_t>((uint64_t)I->grid, std::max<uint64_t>(blocks_needed, 1));
-  void *args[] = { (void *)&P };
-  CU(cudaLaunchKernel((const void *)fn, dim3(grid), dim3((unsigned)I->threads), args, I->smem_bytes, st));
-  I->launches.fetch_add(1);
-  return LGX_OK;
 }
 
 }  // namespace
@@ -149,28 +137,82 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   H.w_path = d->w_path; H.w_time = d->w_time;
   H.perm16 = nf > 255 ? 1 : 0;
   H.mask_words = nsu > 64 ? 2u : 1u;
+  const uint32_t MW = H.mask_words;
+  // stream-4 draws taken up front: (N_B-1) failures + geometric extras, with slack; <= 64
+  H.n_extra_blocks = (uint32_t)std::min(16, ((nb - 1) * 4 / 3 + 8 + 3) / 4);
 
-  // ---- per-candidate state rows (32-bit words per thread)
-  const uint32_t per_word = H.perm16 ? 2u : 4u;
+  // ---- permutation array: right-aligned inside its words so that consumption position
+  //      p = EPW*q + t always sits in a static lane of word row wtop - q
+  const uint32_t EPW = H.perm16 ? 2u : 4u;
+  H.perm_pad = (EPW - (uint32_t)nf % EPW) % EPW;
+  H.n_perm_words = ((uint32_t)nf + H.perm_pad) / EPW;
+  {
+    uint32_t w0 = 0;
+    for (uint32_t t = 0; t < EPW; ++t) {
+      const uint32_t v = (t >= H.perm_pad) ? (t - H.perm_pad) : 0u;
+      w0 |= (v & (H.perm16 ? 0xFFFFu : 0xFFu)) << (t * (H.perm16 ? 16u : 8u));
+    }
+    H.perm_w0 = w0;
+  }
+  H.n_bpseq_words  = cdiv((uint32_t)nb, 4u);
+  H.n_segend_words = cdiv((uint32_t)nb, EPW);
+
+  // ---- state rows of the decode/walk kernel
   const uint32_t n_small = (uint32_t)std::max(nb, std::max(nhu, nsu));
-  uint32_t row = 0;
-  H.row_perm   = row; row += ((uint32_t)nf + per_word - 1) / per_word;
-  H.row_bpseq  = row; row += ((uint32_t)nb + 3) / 4;
-  H.row_segend = row; row += ((uint32_t)nb + per_word - 1) / per_word;
-  H.row_scra   = row; row += (n_small + 3) / 4;
-  H.row_scrb   = row; row += ((uint32_t)nb + 3) / 4;
-  H.tour_words = TR_MASK + 2u * H.mask_words;
-  H.row_tour   = row; row += (uint32_t)nt * H.tour_words;
-  H.words_per_thread = row;
+  {
+    uint32_t r = 0;
+    H.a64_sd = r; r += (uint32_t)nb;
+    H.a64_lt = r; r += (uint32_t)nt;
+    H.a64_mask = r; r += (uint32_t)nt * MW;
+    H.a64_rows = r;
+    r = 0;
+    H.a32_perm = r;   r += H.n_perm_words;
+    H.a32_bpseq = r;  r += H.n_bpseq_words;
+    H.a32_segend = r; r += H.n_segend_words;
+    H.a32_scra = r;   r += (n_small + 3u) / 4u + 1u;       // + 1: right-alignment padding
+    H.a32_scrb = r;   r += cdiv((uint32_t)nb, 4u);
+    H.a32_hq = r;     r += (uint32_t)nt;
+    H.a32_s = r;      r += (uint32_t)nt;
+    H.a32_r = r;      r += (uint32_t)nt;
+    H.a32_cnt = r;    r += (uint32_t)nt;
+    H.a32_rows = r;
+  }
+  // ---- state rows of the finish kernel
+  {
+    uint32_t r = 0;
+    H.c64_w = r; r += (uint32_t)nt;
+    H.c64_e = r; r += (uint32_t)nt;
+    H.c64_mask = r; r += (uint32_t)nt * MW;
+    H.c64_rows = r;
+    r = 0;
+    H.c32_s = r; r += (uint32_t)nt;
+    H.c32_nhu = r; r += (uint32_t)nt;
+    H.c32_ng = r; r += (uint32_t)nt;
+    H.c32_magic = r; r += (uint32_t)nt;
+    H.c32_bpseq = r; r += H.n_bpseq_words;
+    H.c32_segend = r; r += H.n_segend_words;
+    H.c32_rows = r;
+  }
+  // ---- queue record
+  {
+    uint32_t w = 2;
+    H.rec_tw = 6u + 2u * MW;
+    H.rec_tour = w;   w += (uint32_t)nt * H.rec_tw;
+    H.rec_sd = w;     w += 2u * (uint32_t)nb;
+    H.rec_bpseq = w;  w += H.n_bpseq_words;
+    H.rec_segend = w; w += H.n_segend_words;
+    H.rec_perm = w;   w += H.n_perm_words;
+    H.rec_words = w;
+  }
+  const uint64_t a_state = 8ull * H.a64_rows + 4ull * H.a32_rows;
+  const uint64_t c_state = 8ull * H.c64_rows + 4ull * H.c32_rows;
 
-  // ---- image: packed distance tables when they leave room for >= 256 candidates per SM,
+  // ---- image AB: packed distance tables when they leave room for >= 256 candidates per SM,
   //      else vertex coordinates
   const uint64_t tri_bytes = (uint64_t)(nf + 1) * (uint64_t)nf / 2 * 8, dfb_bytes = (uint64_t)nf * nb * 8;
-  const uint64_t small_bytes = sizeof(ImgHdr) + 16ull * nf + 4ull * (nb + nhu + nsu) + 2ull * nsu + 8ull * (nb + nhu) + 256;
-  const uint64_t state_256 = 256ull * 4ull * H.words_per_thread;
-  H.coords = (small_bytes + tri_bytes + dfb_bytes + state_256 > (uint64_t)kMaxSmem - 1024) ? 1 : 0;
-
-  uint32_t off = (uint32_t)sizeof(ImgHdr);
+  const uint64_t small_bytes = 8ull * nf + 4ull * (nb + nhu + nsu) + 1ull * nsu + 128;
+  H.coords = (small_bytes + tri_bytes + dfb_bytes + 256ull * a_state > (uint64_t)kMaxSmem - 1024) ? 1 : 0;
+  uint32_t off = 0;
   if (!H.coords) {
     H.off_dtri = off; off = align16(off + (uint32_t)tri_bytes);
     H.off_dfb  = off; off = align16(off + (uint32_t)dfb_bytes);
@@ -184,15 +226,21 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   H.off_rq   = off; off = align16(off + 4u * (uint32_t)nhu);
   H.off_cs   = off; off = align16(off + 4u * (uint32_t)nsu);
   H.off_rank = off; off = align16(off + (uint32_t)nsu);
-  H.off_unit = off; off = align16(off + (uint32_t)nsu);
-  const int n_rcp = std::max(nf, std::max(nb, nhu)) + 1;
-  H.off_rcp  = off; off = align16(off + 8u * (uint32_t)n_rcp);
   H.image_bytes = off;
-  // stream-4 draws taken up front: (N_B-1) failures + geometric extras, with slack; <= 64
-  H.n_extra_blocks = (uint32_t)std::min(16, ((nb - 1) * 4 / 3 + 8 + 3) / 4);
+  // ---- image C
+  const int n_rcp = std::max(nf, std::max(nb, nhu)) + 1;
+  off = 0;
+  if (!H.coords) { H.offc_dfb = off; off = align16(off + (uint32_t)dfb_bytes); H.offc_xy = 0; }
+  else           { H.offc_dfb = 0; H.offc_xy = off; off = align16(off + 16u * (uint32_t)(1 + nb + nf)); }
+  H.offc_s    = off; off = align16(off + 4u * (uint32_t)nf);
+  H.offc_cs   = off; off = align16(off + 4u * (uint32_t)nsu);
+  H.offc_rcp  = off; off = align16(off + 8u * (uint32_t)n_rcp);
+  H.offc_unit = off; off = align16(off + (uint32_t)nsu);
+  H.imagec_bytes = off;
 
-  I->image.assign(off, 0);
-  uint8_t *img = I->image.data();
+  I->image.assign(H.image_bytes, 0);
+  I->image_c.assign(H.imagec_bytes, 0);
+  uint8_t *img = I->image.data(), *imc = I->image_c.data();
   if (!H.coords) {
     // strict lower triangle over {HQ = 0, field f = f + 1}: entry (hi, lo) at hi(hi-1)/2 + lo
     double *tri = reinterpret_cast<double *>(img + H.off_dtri);
@@ -202,17 +250,19 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
         const double bx = lo ? d->field_x[lo - 1] : d->hq_x, by = lo ? d->field_y[lo - 1] : d->hq_y;
         tri[(size_t)hi * (hi - 1) / 2 + lo] = edge(ax, ay, bx, by);
       }
-    double *dfb = reinterpret_cast<double *>(img + H.off_dfb);
+    double *dfb = reinterpret_cast<double *>(img + H.off_dfb), *dfc = reinterpret_cast<double *>(imc + H.offc_dfb);
     for (int f = 0; f < nf; ++f)
-      for (int b = 0; b < nb; ++b) dfb[(size_t)f * nb + b] = edge(d->field_x[f], d->field_y[f], d->bp_x[b], d->bp_y[b]);
+      for (int b = 0; b < nb; ++b)
+        dfb[(size_t)f * nb + b] = dfc[(size_t)f * nb + b] = edge(d->field_x[f], d->field_y[f], d->bp_x[b], d->bp_y[b]);
   } else {
-    double *xy = reinterpret_cast<double *>(img + H.off_xy);
-    xy[0] = d->hq_x; xy[1] = d->hq_y;
-    for (int b = 0; b < nb; ++b) { xy[2 * (1 + b)] = d->bp_x[b]; xy[2 * (1 + b) + 1] = d->bp_y[b]; }
-    for (int f = 0; f < nf; ++f) { xy[2 * (1 + nb + f)] = d->field_x[f]; xy[2 * (1 + nb + f) + 1] = d->field_y[f]; }
+    for (double *xy : { reinterpret_cast<double *>(img + H.off_xy), reinterpret_cast<double *>(imc + H.offc_xy) }) {
+      xy[0] = d->hq_x; xy[1] = d->hq_y;
+      for (int b = 0; b < nb; ++b) { xy[2 * (1 + b)] = d->bp_x[b]; xy[2 * (1 + b) + 1] = d->bp_y[b]; }
+      for (int f = 0; f < nf; ++f) { xy[2 * (1 + nb + f)] = d->field_x[f]; xy[2 * (1 + nb + f) + 1] = d->field_y[f]; }
+    }
   }
-  uint32_t *sh = reinterpret_cast<uint32_t *>(img + H.off_sh);
-  for (int f = 0; f < nf; ++f) { sh[2 * f] = (uint32_t)s_q[f]; sh[2 * f + 1] = (uint32_t)h_q[f]; }
+  uint32_t *sh = reinterpret_cast<uint32_t *>(img + H.off_sh), *sc = reinterpret_cast<uint32_t *>(imc + H.offc_s);
+  for (int f = 0; f < nf; ++f) { sh[2 * f] = sc[f] = (uint32_t)s_q[f]; sh[2 * f + 1] = (uint32_t)h_q[f]; }
   uint32_t *dq = reinterpret_cast<uint32_t *>(img + H.off_dq);
   for (int b = 0; b < nb; ++b) dq[b] = (uint32_t)d_q[b];
   uint32_t *rq = reinterpret_cast<uint32_t *>(img + H.off_rq);
@@ -221,12 +271,14 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   std::vector<int> order(nsu);
   std::iota(order.begin(), order.end(), 0);
   std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return c_q[a] < c_q[b]; });
-  uint32_t *cs = reinterpret_cast<uint32_t *>(img + H.off_cs);
-  for (int r = 0; r < nsu; ++r) { cs[r] = (uint32_t)c_q[order[r]]; img[H.off_unit + r] = (uint8_t)order[r]; img[H.off_rank + order[r]] = (uint8_t)r; }
-  double *rcp = reinterpret_cast<double *>(img + H.off_rcp);
+  uint32_t *cs = reinterpret_cast<uint32_t *>(img + H.off_cs), *cc = reinterpret_cast<uint32_t *>(imc + H.offc_cs);
+  for (int r = 0; r < nsu; ++r) {
+    cs[r] = cc[r] = (uint32_t)c_q[order[r]];
+    imc[H.offc_unit + r] = (uint8_t)order[r]; img[H.off_rank + order[r]] = (uint8_t)r;
+  }
+  double *rcp = reinterpret_cast<double *>(imc + H.offc_rcp);
   rcp[0] = 0.0;
   for (int k = 1; k < n_rcp; ++k) rcp[k] = 1.0 / (double)k;          // correctly rounded reciprocals
-  std::memcpy(img, &H, sizeof(ImgHdr));
 
   // ---- device: launch configuration and upload
   int ndev = 0;
@@ -237,15 +289,28 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   cudaDeviceGetAttribute(&I->sm_count, cudaDevAttrMultiProcessorCount, I->device);
   cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, I->device);
   const int64_t budget = std::min<int64_t>(smem_optin, kMaxSmem) - 1024;   // static smem of the reduction
-  int64_t t = (budget - (int64_t)H.image_bytes) / (4ll * H.words_per_thread);
-  t = std::min<int64_t>(t, kMaxThreads) / 32 * 32;
-  if (t < 32) { delete I; return LGX_ETOOBIG; }
-  I->threads = (int)t;
+  int64_t ta = (budget - (int64_t)H.image_bytes) / (int64_t)a_state;
+  int64_t tc = (budget - (int64_t)H.imagec_bytes) / (int64_t)c_state;
+  ta = std::min<int64_t>(ta, kMaxThreads) / 32 * 32;
+  tc = std::min<int64_t>(tc, kMaxThreads) / 32 * 32;
+  if (ta < 32 || tc < 32) { delete I; return LGX_ETOOBIG; }
+  I->threads_a = (int)ta; I->threads_c = (int)tc;
   I->grid = I->sm_count;                       // one persistent block per SM
-  I->smem_bytes = (size_t)H.image_bytes + 4ull * H.words_per_thread * (size_t)I->threads;
+  I->smem_a = (size_t)H.image_bytes + a_state * (size_t)ta;
+  I->smem_c = (size_t)H.imagec_bytes + c_state * (size_t)tc;
+  // candidates per kernel pair: queue of at most 192 MiB, a whole number of grid rounds
+  {
+    const uint64_t round = (uint64_t)I->grid * (uint64_t)ta;
+    uint64_t cap = (192ull << 20) / (4ull * H.rec_words);
+    cap = std::min<uint64_t>(cap, 1ull << 21);
+    cap = std::max<uint64_t>(cap / round, 1) * round;
+    I->chunk = cap;
+  }
   if ((e = cudaMalloc((void **)&I->d_image, H.image_bytes)) != cudaSuccess) { delete I; return cuda_fail(e, "cudaMalloc(image)"); }
-  if ((e = cudaMemcpy(I->d_image, img, H.image_bytes, cudaMemcpyHostToDevice)) != cudaSuccess) {
-    cudaFree(I->d_image); delete I; return cuda_fail(e, "cudaMemcpy(image)");
+  if ((e = cudaMalloc((void **)&I->d_image_c, H.imagec_bytes)) != cudaSuccess) { cudaFree(I->d_image); delete I; return cuda_fail(e, "cudaMalloc(image C)"); }
+  if ((e = cudaMemcpy(I->d_image, img, H.image_bytes, cudaMemcpyHostToDevice)) != cudaSuccess ||
+      (e = cudaMemcpy(I->d_image_c, imc, H.imagec_bytes, cudaMemcpyHostToDevice)) != cudaSuccess) {
+    cudaFree(I->d_image); cudaFree(I->d_image_c); delete I; return cuda_fail(e, "cudaMemcpy(image)");
   }
   *out = I;
   return LGX_OK;
@@ -255,22 +320,86 @@ int lgx_instance_destroy(lgx_instance *I)
 {
   if (!I) return LGX_EINVAL;
   if (I->d_image) cudaFree(I->d_image);
+  if (I->d_image_c) cudaFree(I->d_image_c);
   delete I;
   return LGX_OK;
 }
+
+}  // extern "C"
+
+namespace {
+
+// One call = chunks of at most I->chunk candidates; per chunk the decode/walk kernel fills the
+// queue and the finish kernel drains it (same stream, so the pair is ordered).  The workspace
+// is allocated stream-ordered per call, so concurrent calls on different streams are legal.
+struct Workspace {
+  uint8_t *base = nullptr;
+  unsigned int *q_count = nullptr, *done = nullptr;
+  unsigned long long *result = nullptr, *block_best = nullptr;
+  uint32_t *queue = nullptr;
+  uint64_t cap = 0;
+};
+
+int ws_alloc(const lgx_instance *I, uint64_t n, bool search, cudaStream_t st, Workspace &W)
+{
+  W.cap = std::min<uint64_t>(I->chunk, n);
+  const size_t head = 64 + 16ull * (size_t)I->grid;
+  const size_t qoff = (head + 255) & ~(size_t)255;
+  const size_t bytes = qoff + 4ull * I->hdr.rec_words * W.cap;
+  CU(cudaMallocAsync((void **)&W.base, bytes, st));
+  W.q_count = reinterpret_cast<unsigned int *>(W.base);
+  W.done = W.q_count + 1;
+  W.result = reinterpret_cast<unsigned long long *>(W.base + 16);
+  W.block_best = reinterpret_cast<unsigned long long *>(W.base + 64);
+  W.queue = reinterpret_cast<uint32_t *>(W.base + qoff);
+  cudaError_t e = cudaMemsetAsync(W.base, 0, 16, st);
+  if (e == cudaSuccess && search) e = cudaMemsetAsync(W.result, 0xFF, 16, st);
+  if (e != cudaSuccess) { cudaFreeAsync(W.base, st); W.base = nullptr; return cuda_fail(e, "cudaMemsetAsync(workspace)"); }
+  return LGX_OK;
+}
+
+int run_chunks(const lgx_instance *I, KernelFn ka, KernelFn kc, KParams &P, uint64_t n, const Workspace &W, cudaStream_t st)
+{
+  if (!ka || !kc) return LGX_EINVAL;
+  CU(cudaFuncSetAttribute((const void *)ka, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)I->smem_a));
+  CU(cudaFuncSetAttribute((const void *)kc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)I->smem_c));
+  P.H = I->hdr; P.image = I->d_image; P.image_c = I->d_image_c;
+  P.queue = W.queue; P.cap = (uint32_t)W.cap; P.q_count = W.q_count;
+  P.done_counter = W.done; P.block_best = W.block_best; P.result = W.result;
+  void *args[] = { (void *)&P };
+  for (uint64_t base = 0; base < n; base += W.cap) {
+    P.base_i = base; P.n = std::min<uint64_t>(W.cap, n - base);
+    const uint64_t blocks_a = (P.n + (uint64_t)I->threads_a - 1) / (uint64_t)I->threads_a;
+    const unsigned grid_a = (unsigned)std::min<uint64_t>((uint64_t)I->grid, blocks_a);
+    const uint64_t blocks_c = (P.n + (uint64_t)I->threads_c - 1) / (uint64_t)I->threads_c;
+    const unsigned grid_c = (unsigned)std::min<uint64_t>((uint64_t)I->grid, blocks_c);
+    CU(cudaLaunchKernel((const void *)ka, dim3(grid_a), dim3((unsigned)I->threads_a), args, I->smem_a, st));
+    CU(cudaLaunchKernel((const void *)kc, dim3(grid_c), dim3((unsigned)I->threads_c), args, I->smem_c, st));
+    I->launches.fetch_add(2);
+  }
+  return LGX_OK;
+}
+
+}  // namespace
+
+extern "C" {
 
 int lgx_instance_query(const lgx_instance *I, int what, int64_t *out)
 {
   if (!I || !out) return LGX_EINVAL;
   switch (what) {
-    case 0: *out = I->hdr.image_bytes; break;
-    case 1: *out = I->threads; break;
+    case 0: *out = (int64_t)I->hdr.image_bytes + I->hdr.imagec_bytes; break;
+    case 1: *out = I->threads_a; break;
     case 2: *out = I->grid; break;
-    case 3: *out = (int64_t)I->smem_bytes; break;
+    case 3: *out = (int64_t)I->smem_a; break;
     case 4: *out = I->hdr.coords; break;
-    case 5: *out = 4ll * I->hdr.words_per_thread; break;
+    case 5: *out = 8ll * I->hdr.a64_rows + 4ll * I->hdr.a32_rows; break;
     case 6: *out = I->sm_count; break;
     case 7: *out = I->launches.load(); break;
+    case 8: *out = I->threads_c; break;
+    case 9: *out = (int64_t)I->smem_c; break;
+    case 10: *out = (int64_t)I->chunk; break;
+    case 11: *out = 4ll * I->hdr.rec_words; break;
     default: return LGX_EINVAL;
   }
   return LGX_OK;
@@ -281,11 +410,18 @@ int lgx_eval_batch(const lgx_instance *I, uint64_t seed, const uint64_t *d_ids, 
 {
   if (!I) return LGX_EINVAL;
   if (n == 0) return LGX_OK;
+  cudaStream_t st = (cudaStream_t)stream;
   KParams P{};
   fill_round_keys(P, seed);
-  P.ids = d_ids; P.first_id = first_id; P.n = n;
+  P.ids = d_ids; P.first_id = first_id;
   P.cost = d_cost; P.path_km = d_path_km; P.makespan_h = d_makespan_h; P.feasible = d_feasible;
-  return launch(I, pick_kernel<MODE_EVAL>(I->hdr), P, (cudaStream_t)stream);
+  KernelFn ka, kc; pick_kernels<MODE_EVAL>(I->hdr, ka, kc);
+  Workspace W;
+  int rc = ws_alloc(I, n, false, st, W);
+  if (rc != LGX_OK) return rc;
+  rc = run_chunks(I, ka, kc, P, n, W, st);
+  cudaFreeAsync(W.base, st);
+  return rc;
 }
 
 int lgx_decode_batch(const lgx_instance *I, uint64_t seed, const uint64_t *d_ids, uint64_t first_id, uint64_t n,
@@ -294,12 +430,19 @@ int lgx_decode_batch(const lgx_instance *I, uint64_t seed, const uint64_t *d_ids
 {
   if (!I) return LGX_EINVAL;
   if (n == 0) return LGX_OK;
+  cudaStream_t st = (cudaStream_t)stream;
   KParams P{};
   fill_round_keys(P, seed);
-  P.ids = d_ids; P.first_id = first_id; P.n = n;
+  P.ids = d_ids; P.first_id = first_id;
   P.bp_tour = d_bp_tour; P.bp_pos = d_bp_pos; P.field_bp = d_field_bp; P.field_pos = d_field_pos;
   P.hu_tour = d_hu_tour; P.su_init = d_su_tour_init; P.su_final = d_su_tour_final;
-  return launch(I, pick_kernel<MODE_DECODE>(I->hdr), P, (cudaStream_t)stream);
+  KernelFn ka, kc; pick_kernels<MODE_DECODE>(I->hdr, ka, kc);
+  Workspace W;
+  int rc = ws_alloc(I, n, false, st, W);
+  if (rc != LGX_OK) return rc;
+  rc = run_chunks(I, ka, kc, P, n, W, st);
+  cudaFreeAsync(W.base, st);
+  return rc;
 }
 
 int lgx_search_range(const lgx_instance *I, uint64_t seed, uint64_t first_id, uint64_t n,
@@ -307,26 +450,25 @@ int lgx_search_range(const lgx_instance *I, uint64_t seed, uint64_t first_id, ui
 {
   if (!I || !h_best_cost || !h_best_id || n == 0) return LGX_EINVAL;
   cudaStream_t st = (cudaStream_t)stream;
-  // scratch: [grid][2] block minima, [2] result, done counter
-  const size_t words = 2ull * (size_t)I->grid + 2 + 1;
-  unsigned long long *d_scratch = nullptr;
-  CU(cudaMallocAsync((void **)&d_scratch, words * sizeof(unsigned long long), st));
-  cudaError_t e = cudaMemsetAsync(d_scratch, 0, words * sizeof(unsigned long long), st);
-  if (e != cudaSuccess) { cudaFreeAsync(d_scratch, st); return cuda_fail(e, "cudaMemsetAsync"); }
   KParams P{};
   fill_round_keys(P, seed);
-  P.ids = nullptr; P.first_id = first_id; P.n = n;
-  P.block_best = d_scratch; P.result = d_scratch + 2ull * I->grid;
-  P.done_counter = reinterpret_cast<unsigned int *>(d_scratch + 2ull * I->grid + 2);
-  int rc = launch(I, pick_kernel<MODE_SEARCH>(I->hdr), P, st);
+  P.ids = nullptr; P.first_id = first_id;
+  KernelFn ka, kc; pick_kernels<MODE_SEARCH>(I->hdr, ka, kc);
+  Workspace W;
+  int rc = ws_alloc(I, n, true, st, W);
+  if (rc != LGX_OK) return rc;
+  rc = run_chunks(I, ka, kc, P, n, W, st);
   unsigned long long res[2] = {0, 0};
   if (rc == LGX_OK) {
-    e = cudaMemcpyAsync(res, P.result, sizeof res, cudaMemcpyDeviceToHost, st);
+    cudaError_t e = cudaMemcpyAsync(res, W.result, sizeof res, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) rc = cuda_fail(e, "lgx_search: copy/synchronize");
   }
-  cudaFreeAsync(d_scratch, st);
+  cudaFreeAsync(W.base, st);
   if (rc != LGX_OK) return rc;
+  if (res[0] == ~0ull && res[1] == ~0ull) {          // no feasible candidate: +inf, lowest id (R19, R29)
+    res[0] = 0x7FF0000000000000ull; res[1] = first_id;
+  }
   std::memcpy(h_best_cost, &res[0], 8);
   *h_best_id = res[1];
   return LGX_OK;

@@ -1,17 +1,21 @@
-// lgx_image.h — layout of the instance image that lives in shared memory.
+// lgx_image.h — layout of the instance images that live in shared memory,
+// of the per-candidate state rows, and of the queue record that carries a feasible
+// candidate from the decode/walk kernel to the finish kernel.
 // Product code (CUDA path).  Shares nothing with oracle/.
 //
-// The image is one contiguous, 16-byte aligned blob built on the host by
-// lgx_instance_create and copied global -> shared once per (persistent) block:
+// Image AB (decode + pass 1):   distance tables or coordinates | {s_q,h_q} per field |
+//                               demand quanta | HU rate quanta | SU capacities by rank | unit->rank
+// Image C  (Alg. 2 + pass 2):   field x BP table or coordinates | s_q per field |
+//                               SU capacities by rank | RN(1/k) table | rank->unit
+// Both are contiguous, 16-byte aligned blobs built on the host by lgx_instance_create and
+// copied global -> shared once per (persistent) block.
 //
-//   ImgHdr | distance tables or coordinates | per-field quanta | per-BP demand quanta |
-//   HU rate quanta | SU capacities sorted by (capacity, unit) | unit<->rank maps
-//
-// It is followed in shared memory by the per-candidate state: `words_per_thread` rows of
-// blockDim.x 32-bit words, row-major, so that word r of thread t sits at
-// state[r * blockDim.x + t] — every dynamically indexed per-thread access (Fisher-Yates
-// swaps, per-tour accumulators) then hits bank t % 32 whatever the index: conflict-free
-// by construction.
+// Per-candidate state follows the image in shared memory as ROWS of blockDim.x cells:
+// cell (row r, thread t) of the 64-bit region at  state64 + (r*blockDim.x + t)*8,
+// cell (row r, thread t) of the 32-bit region at  state32 + (r*blockDim.x + t)*4,
+// so every dynamically indexed per-thread access (Fisher-Yates swaps, per-BP / per-tour
+// accumulators) hits bank(s) fixed by t alone: conflict-free whatever the index
+// (SURVEY §7 H2).
 #pragma once
 #include <stdint.h>
 
@@ -25,25 +29,18 @@ constexpr uint32_t kPhiloxW1    = 0xBB67AE85u;
 constexpr int      kMaxSmem     = 227 * 1024;    // opt-in dynamic shared memory per block, sm_100a
 constexpr int      kMaxThreads  = 512;           // __launch_bounds__ of the candidate kernels
 
-// Per-tour rows of the per-candidate state (32-bit words).
-enum TourRow : uint32_t {
-  TR_LT   = 0,   // f64  closed HU route length L_tour(g)             (pass 1)
-  TR_E    = 2,   // f64  sumE during pass 1, then E(g)                (Alg. 2 step 1)
-  TR_W    = 4,   // f64  T_wait(g) cache                              (Alg. 2)
-  TR_SH   = 6,   // f64  shuttle distance sum of the tour             (pass 2)
-  TR_HQ   = 8,   // u32  harvested area quanta H_q(g)
-  TR_R    = 9,   // u32  sum of HU rate quanta R_g
-  TR_S    = 10,  // u32  sum of SU capacity quanta S_g = C_g
-  TR_CNT  = 11,  // u32  n_HU(g) | m(g) << 16
-  TR_MASK = 12,  // u64 x MASKW  SU membership by capacity rank
-};
-
 struct ImgHdr {
   int32_t  n_f, n_b, n_hu, n_su, n_t;
   uint32_t thresh;
   int32_t  coords;          // 0: packed HQ+field triangle + field x BP table; 1: coordinates
   int32_t  perm16;          // field ids / segment ends stored as u16 instead of u8
   double   v_hu, v_su, kappa, w_path, w_time;
+  uint32_t mask_words;      // 64-bit words per SU mask (1 or 2)
+  uint32_t n_extra_blocks;  // Philox blocks of stream 4 drawn up front (<= 16)
+  uint32_t perm_pad;        // right-alignment of the permutation array inside its words
+  uint32_t perm_w0;         // initial value of permutation word 0 (bytes below perm_pad unused)
+
+  // ---- image AB (byte offsets)
   uint32_t off_dtri;        // f64 [(n_f+1) n_f / 2]  strict lower triangle over {HQ, fields}
   uint32_t off_dfb;         // f64 [n_f][n_b]         field -> BP legs
   uint32_t off_xy;          // f64x2 [1 + n_b + n_f]  vertex coordinates (coords mode)
@@ -52,13 +49,26 @@ struct ImgHdr {
   uint32_t off_rq;          // u32 [n_hu]             HU rate quanta
   uint32_t off_cs;          // u32 [n_su]             SU capacity quanta, ascending (c_q, unit)
   uint32_t off_rank;        // u8  [n_su]             unit -> rank
-  uint32_t off_unit;        // u8  [n_su]             rank -> unit
-  uint32_t off_rcp;         // f64 [max(n_f,n_b,n_hu)+1]  RN(1/k), for the exact small-divisor division
-  uint32_t row_perm, row_bpseq, row_segend, row_scra, row_scrb, row_tour;
-  uint32_t tour_words, words_per_thread;
   uint32_t image_bytes;
-  uint32_t mask_words;      // 64-bit words per SU mask (1 or 2)
-  uint32_t n_extra_blocks;  // Philox blocks of stream 4 drawn up front (<= 16)
+
+  // ---- image C (byte offsets inside image C)
+  uint32_t offc_dfb, offc_xy, offc_s, offc_cs, offc_rcp, offc_unit;
+  uint32_t imagec_bytes;
+
+  // ---- state rows of the decode/walk kernel
+  uint32_t a64_sd, a64_lt, a64_mask, a64_rows;
+  uint32_t a32_perm, a32_bpseq, a32_segend, a32_scra, a32_scrb, a32_hq, a32_s, a32_r, a32_cnt, a32_rows;
+
+  // ---- state rows of the finish kernel
+  uint32_t c64_w, c64_e, c64_mask, c64_rows;
+  uint32_t c32_s, c32_nhu, c32_ng, c32_magic, c32_bpseq, c32_segend, c32_rows;
+
+  // ---- queue record (32-bit words, stored transposed: word w of slot q at queue[w*cap + q])
+  //   0,1 index i | per tour g at rec_tour + g*rec_tw: LT lo,hi, H_q, R_g, S_g, n_HU, MASK words |
+  //   SD[j] lo,hi at rec_sd + 2j | bpseq words | segend words | perm words
+  uint32_t rec_tour, rec_tw, rec_sd, rec_bpseq, rec_segend, rec_perm, rec_words;
+  uint32_t n_bpseq_words, n_segend_words, n_perm_words;
+  uint32_t pad_[3];
 };
 static_assert(sizeof(ImgHdr) % 16 == 0, "image header must keep 16-byte alignment");
 
