@@ -161,16 +161,17 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   const uint32_t n_small = (uint32_t)std::max(nb, std::max(nhu, nsu));
   {
     uint32_t r = 0;
-    H.a64_sd = r; r += (uint32_t)nb;
+    H.a64_sd = r; H.a64_ent = r; r += (uint32_t)nb;    // entry j is consumed before SD[j] is flushed: same rows
     H.a64_lt = r; r += (uint32_t)nt;
     H.a64_mask = r; r += (uint32_t)nt * MW;
     H.a64_rows = r;
     r = 0;
     H.a32_perm = r;   r += H.n_perm_words;
     H.a32_bpseq = r;  r += H.n_bpseq_words;
-    H.a32_segend = r; r += H.n_segend_words;
-    H.a32_scra = r;   r += (n_small + 3u) / 4u + 1u;       // + 1: right-alignment padding
-    H.a32_scrb = r;   r += cdiv((uint32_t)nb, 4u);
+    // partition scratch (dead once the field loop starts) shares its rows with the segment ends
+    const uint32_t scra_words = (n_small + 3u) / 4u + 1u, scrb_words = cdiv((uint32_t)nb, 4u);
+    H.a32_scra = r; H.a32_segend = r; H.a32_scrb = r + scra_words;
+    r += std::max(scra_words + scrb_words, (uint32_t)nb);
     H.a32_hq = r;     r += (uint32_t)nt;
     H.a32_s = r;      r += (uint32_t)nt;
     H.a32_r = r;      r += (uint32_t)nt;

@@ -56,7 +56,7 @@ struct ImgHdr {
   uint32_t imagec_bytes;
 
   // ---- state rows of the decode/walk kernel
-  uint32_t a64_sd, a64_lt, a64_mask, a64_rows;
+  uint32_t a64_sd, a64_lt, a64_mask, a64_ent, a64_rows;
   uint32_t a32_perm, a32_bpseq, a32_segend, a32_scra, a32_scrb, a32_hq, a32_s, a32_r, a32_cnt, a32_rows;
 
   // ---- state rows of the finish kernel
@@ -68,7 +68,7 @@ struct ImgHdr {
   //   SD[j] lo,hi at rec_sd + 2j | bpseq words | segend words | perm words
   uint32_t rec_tour, rec_tw, rec_sd, rec_bpseq, rec_segend, rec_perm, rec_words;
   uint32_t n_bpseq_words, n_segend_words, n_perm_words;
-  uint32_t pad_[3];
+  uint32_t pad_[2];
 };
 static_assert(sizeof(ImgHdr) % 16 == 0, "image header must keep 16-byte alignment");
 
