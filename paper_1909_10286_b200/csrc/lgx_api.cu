@@ -9,6 +9,7 @@
 #include <atomic>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <numeric>
@@ -291,7 +292,8 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, I->device);
   const int64_t budget = std::min<int64_t>(smem_optin, kMaxSmem) - 1024;   // static smem of the reduction
   int64_t ta = (budget - (int64_t)H.image_bytes) / (int64_t)a_state;
-  int64_t tc = (budget - (int64_t)H.imagec_bytes) / (int64_t)c_state;
+  // finish kernel: kFinishBlocksPerSM blocks per SM (each with its own copy of image C)
+  int64_t tc = ((budget + 1024) / kFinishBlocksPerSM - 1024 - (int64_t)H.imagec_bytes) / (int64_t)c_state;
   ta = std::min<int64_t>(ta, kMaxThreads) / 32 * 32;
   tc = std::min<int64_t>(tc, kMaxThreads) / 32 * 32;
   if (ta < 32 || tc < 32) { delete I; return LGX_ETOOBIG; }
@@ -304,6 +306,10 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
     const uint64_t round = (uint64_t)I->grid * (uint64_t)ta;
     uint64_t cap = (192ull << 20) / (4ull * H.rec_words);
     cap = std::min<uint64_t>(cap, 1ull << 21);
+    if (const char *ev = std::getenv("LGX_CHUNK_LOG2")) {      // tuning knob (bench sweeps); default above
+      const int lg = std::atoi(ev);
+      if (lg >= 10 && lg <= 26) cap = 1ull << lg;
+    }
     cap = std::max<uint64_t>(cap / round, 1) * round;
     I->chunk = cap;
   }
@@ -344,7 +350,7 @@ struct Workspace {
 int ws_alloc(const lgx_instance *I, uint64_t n, bool search, cudaStream_t st, Workspace &W)
 {
   W.cap = std::min<uint64_t>(I->chunk, n);
-  const size_t head = 64 + 16ull * (size_t)I->grid;
+  const size_t head = 64 + 16ull * (size_t)I->grid * kFinishBlocksPerSM;
   const size_t qoff = (head + 255) & ~(size_t)255;
   const size_t bytes = qoff + 4ull * I->hdr.rec_words * W.cap;
   CU(cudaMallocAsync((void **)&W.base, bytes, st));
@@ -373,7 +379,7 @@ int run_chunks(const lgx_instance *I, KernelFn ka, KernelFn kc, KParams &P, uint
     const uint64_t blocks_a = (P.n + (uint64_t)I->threads_a - 1) / (uint64_t)I->threads_a;
     const unsigned grid_a = (unsigned)std::min<uint64_t>((uint64_t)I->grid, blocks_a);
     const uint64_t blocks_c = (P.n + (uint64_t)I->threads_c - 1) / (uint64_t)I->threads_c;
-    const unsigned grid_c = (unsigned)std::min<uint64_t>((uint64_t)I->grid, blocks_c);
+    const unsigned grid_c = (unsigned)std::min<uint64_t>((uint64_t)I->grid * kFinishBlocksPerSM, blocks_c);
     CU(cudaLaunchKernel((const void *)ka, dim3(grid_a), dim3((unsigned)I->threads_a), args, I->smem_a, st));
     CU(cudaLaunchKernel((const void *)kc, dim3(grid_c), dim3((unsigned)I->threads_c), args, I->smem_c, st));
     I->launches.fetch_add(2);

@@ -28,6 +28,7 @@ constexpr uint32_t kPhiloxW0    = 0x9E3779B9u;   // key increments
 constexpr uint32_t kPhiloxW1    = 0xBB67AE85u;
 constexpr int      kMaxSmem     = 227 * 1024;    // opt-in dynamic shared memory per block, sm_100a
 constexpr int      kMaxThreads  = 512;           // __launch_bounds__ of the candidate kernels
+constexpr int      kFinishBlocksPerSM = 2;       // the finish kernel's image is small: two blocks share an SM
 
 struct ImgHdr {
   int32_t  n_f, n_b, n_hu, n_su, n_t;
