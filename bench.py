@@ -1,8 +1,9 @@
 #!/usr/bin/env python
 """bench.py — candidates/s of the lgx hot path on B200 (BASELINE.json metric).
 
-A "step" is one pass of the whole hot path (SURVEY §8(a) rows a2..a7 in one persistent
-kernel over the shared-memory image built by a1) over one batch of candidates:
+A "step" is one pass of the whole hot path (the persistent kernel
+pair lgx_decode_walk + lgx_finish per chunk, over the shared-memory images built by a1) over
+one batch of candidates:
 `lgx_search` over the Medium config's full budget (2^28 ids, 100 fields / 8 BPs / 5 tours;
 the config the north_star target of >= 1e9 cand/s is quoted on).  Synthetic, seeded
 instance (paper_1909_10286_b200/workloads.py); nothing is read from /root/reference.
@@ -22,9 +23,22 @@ sys.path.insert(0, ROOT)
 
 METRIC = "candidate plans evaluated/sec"
 UNIT = "candidates/s"
-# Algorithmic thread-instructions per candidate (derived per config from
-# the minimal per-field / per-unit / per-move instruction counts of the method itself).
-W_ALG = {"toy": 2300, "small": 6200, "medium": 13900, "large": 42500, "sweep": 86500}
+# Algorithmic thread-instructions per candidate: what the method itself needs,
+# split into the part every candidate pays (decode + pass 1: kernel lgx_decode_walk) and the part
+# only feasible candidates pay (tour statistics, Algorithm 2, pass 2, cost: kernel lgx_finish).
+ALG2_ITERS = {"toy": 2.3, "small": 5.6, "medium": 9.9, "large": 12.7, "sweep": 19.5}   # oracle-measured means
+
+
+def w_alg(inst, workload):
+    nf, nb, nt, nhu, nsu = inst.n_fields, inst.n_bps, inst.n_tours, inst.n_hu, inst.n_su
+    cd = lambda a, b: -(-a // b)
+    blocks = cd(nf, 4) + sum(cd(n, 4) + cd(n - nt, 4) for n in (nb, nhu, nsu)) + cd((nb - 1) * 4 // 3 + 8, 4)
+    decode_walk = (40 * blocks + 7 * (nf + nb + nhu + nsu) + 2 * (nb + nhu + nsu - 3 * nt)
+                   + 6 * nb + 6 * nhu + 10 * nsu + 14 * nf + 10 * (nb + nt))
+    finish = 6 * nb + 92 * nt + 110 * ALG2_ITERS.get(workload, 10.0) + 18 * nf + 10 * (nb + nt) + 9 * nt + 5
+    return decode_walk, finish
+
+
 SM_MAX_MHZ_FALLBACK = 1965.0
 
 
@@ -100,7 +114,7 @@ def run_reference(args):
     if rank != 0:
         return 0
     cores = os.cpu_count() or 1
-    sample = 1 << 19          # ids per step; ~0.5 s per step on 8 cores for Medium
+    sample = 1 << 21          # ids per step; ~1 s per step on 16 cores for Medium
     for _ in range(args.warmup):
         oracle_rate(args.workload, sample // 4, cores)
     tot_t, tot_n = 0.0, 0
@@ -170,6 +184,7 @@ def main():
         step()
     # ---- timed: EXACTLY K steps, device time from CUDA events on the launching stream
     sampler = ClockSampler(local); sampler.start()
+    g.set_timing(True)                           # CUDA events around every kernel launch, on the launching stream
     launches0 = g.query(7)
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     barrier()
@@ -183,6 +198,8 @@ def main():
     barrier()
     t_wall = time.perf_counter() - t_wall0
     launches = g.query(7) - launches0
+    ns_a, ns_c, n_pairs = g.kernel_times()
+    g.set_timing(False)
     clocks = sampler.stop()
     dev_ms = sum(a.elapsed_time(b) for a, b in ev)
     if dist is not None:
@@ -237,15 +254,27 @@ def main():
     sm_max = float(pk.get("sm_max_mhz", SM_MAX_MHZ_FALLBACK))
     n_sm = info["sm_count"]
     peak_ginst = n_sm * 4 * 32 * sm_max * 1e6 / 1e9          # thread-instructions/s at max clock
-    per_launch_ms = dev_ms / args.steps
-    w_alg = W_ALG.get(args.workload)
-    achieved = (per_gpu * w_alg / (per_launch_ms * 1e-3) / 1e9) if w_alg else None
-    roofline = {"bound": "alu", "achieved": achieved, "peak": peak_ginst, "unit": "Ginst/s (thread instructions)",
-                "frac": (achieved / peak_ginst) if achieved else None, "traffic": None,
-                "kernel": "lgx_candidates<MODE_SEARCH>", "launch_ms": per_launch_ms,
-                "w_alg_thread_inst_per_candidate": w_alg,
-                "peak_source": f"{n_sm} SMs x 4 schedulers x 32 lanes x {sm_max:.0f} MHz ({pk_src} sm_max_mhz; DESIGN.md)",
-                "frac_at_observed_clock": (achieved / (peak_ginst * clocks["sm_mhz"] / sm_max)) if achieved and clocks.get("sm_mhz") else None}
+    feas = extra.get("eval_batch", {}).get("feasible_fraction", 1.0)
+    w_dw, w_fin = w_alg(inst, args.workload)
+    cand_timed = per_gpu * args.steps                         # this rank's candidates in the timed region
+    per_launch = cand_timed / max(n_pairs, 1)                 # candidates per launch of each kernel
+    ms_a = ns_a * 1e-6 / max(n_pairs, 1); ms_c = ns_c * 1e-6 / max(n_pairs, 1)
+    ach_a = per_launch * w_dw / (ms_a * 1e-3) / 1e9 if ms_a > 0 else None
+    ach_c = per_launch * feas * w_fin / (ms_c * 1e-3) / 1e9 if ms_c > 0 else None
+    ach_all = (w_dw + feas * w_fin) * value / world / 1e9
+    obs = clocks.get("sm_mhz") or sm_max
+    roofline = {"bound": "alu", "kernel": "lgx_decode_walk (dominant: %.0f %% of the kernel time of a step)" % (100.0 * ns_a / max(ns_a + ns_c, 1)),
+                "achieved": ach_a, "peak": peak_ginst, "unit": "G thread-inst/s", "frac": ach_a / peak_ginst if ach_a else None,
+                "traffic": None, "launch_ms": ms_a, "launches_timed": n_pairs, "candidates_per_launch": per_launch,
+                "w_alg_thread_inst_per_candidate": w_dw,
+                "peak_source": f"{n_sm} SMs x 4 schedulers x 32 lanes x {sm_max:.0f} MHz ({pk_src} sm_max_mhz; DESIGN.md s8)",
+                "frac_at_observed_clock": ach_a / (peak_ginst * obs / sm_max) if ach_a else None,
+                "other_kernels": [{"kernel": "lgx_finish", "launch_ms": ms_c, "achieved": ach_c,
+                                   "frac": ach_c / peak_ginst if ach_c else None,
+                                   "w_alg_thread_inst_per_feasible_candidate": w_fin, "feasible_fraction": feas}],
+                "whole_step": {"w_alg_thread_inst_per_candidate": w_dw + feas * w_fin, "achieved": ach_all,
+                               "frac": ach_all / peak_ginst},
+                "hbm_note": "queue traffic ~%.0f B per candidate; dram bytes per launch in profiles/ (negligible)" % (feas * info["record_bytes"])}
 
     cpu = None
     if not args.no_cpu_baseline:

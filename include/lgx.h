@@ -111,6 +111,13 @@ int lgx_decode_batch(const lgx_instance *inst, uint64_t seed,
  * kernel, 10 candidates per kernel pair (chunk), 11 bytes per queue record.                 */
 int lgx_instance_query(const lgx_instance *inst, int what, int64_t *out);
 
+/* Per-kernel timing for bench.py's roofline: when enabled, every lgx_search(_range) call
+ * brackets each kernel launch with CUDA events on the caller's stream and accumulates the
+ * device time; lgx_instance_query what = 12 / 13 return the nanoseconds spent in the
+ * decode/walk / finish kernels, 14 the number of kernel pairs timed.  Enabling or disabling
+ * resets the counters.                                                                     */
+int lgx_instance_set_timing(lgx_instance *inst, int enable);
+
 const char *lgx_strerror(int code);
 
 #ifdef __cplusplus

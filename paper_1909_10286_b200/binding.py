@@ -34,7 +34,8 @@ class lgx_instance_desc(C.Structure):
 
 
 EXPORTS = ("lgx_instance_create", "lgx_instance_destroy", "lgx_eval_batch", "lgx_eval_batch_host",
-           "lgx_search_range", "lgx_search", "lgx_decode_batch", "lgx_instance_query", "lgx_strerror")
+           "lgx_search_range", "lgx_search", "lgx_decode_batch", "lgx_instance_query", "lgx_instance_set_timing",
+           "lgx_strerror")
 
 _lib = None
 
@@ -58,6 +59,7 @@ def load(rebuild_if_stale: bool = True):
     lib.lgx_search.argtypes = [vp, u64, u64, C.POINTER(C.c_double), C.POINTER(u64), vp]
     lib.lgx_decode_batch.argtypes = [vp, u64, vp, u64, u64] + [vp] * 7 + [vp]
     lib.lgx_instance_query.argtypes = [vp, i32, C.POINTER(C.c_int64)]
+    lib.lgx_instance_set_timing.argtypes = [vp, i32]
     lib.lgx_strerror.argtypes = [i32]
     lib.lgx_strerror.restype = C.c_char_p
     for f in EXPORTS:
@@ -137,6 +139,13 @@ class Instance:
         v = C.c_int64()
         _check(self._lib.lgx_instance_query(self._h, what, C.byref(v)))
         return v.value
+
+    def set_timing(self, enable: bool):
+        _check(self._lib.lgx_instance_set_timing(self._h, 1 if enable else 0))
+
+    def kernel_times(self):
+        """(ns in lgx_decode_walk, ns in lgx_finish, kernel pairs timed) since set_timing(True)."""
+        return self.query(12), self.query(13), self.query(14)
 
     def info(self):
         keys = ["image_bytes", "threads", "grid", "smem_bytes", "coords", "state_bytes", "sm_count", "launches",

@@ -27,6 +27,9 @@ struct lgx_instance {
   size_t smem_a = 0, smem_c = 0;
   uint64_t chunk = 0;                          // candidates per decode/finish kernel pair
   mutable std::atomic<long long> launches{0};
+  // optional per-kernel timing (lgx_instance_set_timing): CUDA events around every launch of a search
+  mutable std::atomic<int> timing{0};
+  mutable std::atomic<long long> ns_a{0}, ns_c{0}, timed_pairs{0};
 };
 
 namespace {
@@ -365,7 +368,8 @@ int ws_alloc(const lgx_instance *I, uint64_t n, bool search, cudaStream_t st, Wo
   return LGX_OK;
 }
 
-int run_chunks(const lgx_instance *I, KernelFn ka, KernelFn kc, KParams &P, uint64_t n, const Workspace &W, cudaStream_t st)
+int run_chunks(const lgx_instance *I, KernelFn ka, KernelFn kc, KParams &P, uint64_t n, const Workspace &W, cudaStream_t st,
+               std::vector<cudaEvent_t> *evs = nullptr)
 {
   if (!ka || !kc) return LGX_EINVAL;
   CU(cudaFuncSetAttribute((const void *)ka, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)I->smem_a));
@@ -380,8 +384,12 @@ int run_chunks(const lgx_instance *I, KernelFn ka, KernelFn kc, KParams &P, uint
     const unsigned grid_a = (unsigned)std::min<uint64_t>((uint64_t)I->grid, blocks_a);
     const uint64_t blocks_c = (P.n + (uint64_t)I->threads_c - 1) / (uint64_t)I->threads_c;
     const unsigned grid_c = (unsigned)std::min<uint64_t>((uint64_t)I->grid * kFinishBlocksPerSM, blocks_c);
+    cudaEvent_t e3[3] = {nullptr, nullptr, nullptr};
+    if (evs) { for (auto &e : e3) { CU(cudaEventCreate(&e)); evs->push_back(e); } CU(cudaEventRecord(e3[0], st)); }
     CU(cudaLaunchKernel((const void *)ka, dim3(grid_a), dim3((unsigned)I->threads_a), args, I->smem_a, st));
+    if (evs) CU(cudaEventRecord(e3[1], st));
     CU(cudaLaunchKernel((const void *)kc, dim3(grid_c), dim3((unsigned)I->threads_c), args, I->smem_c, st));
+    if (evs) CU(cudaEventRecord(e3[2], st));
     I->launches.fetch_add(2);
   }
   return LGX_OK;
@@ -407,8 +415,19 @@ int lgx_instance_query(const lgx_instance *I, int what, int64_t *out)
     case 9: *out = (int64_t)I->smem_c; break;
     case 10: *out = (int64_t)I->chunk; break;
     case 11: *out = 4ll * I->hdr.rec_words; break;
+    case 12: *out = I->ns_a.load(); break;
+    case 13: *out = I->ns_c.load(); break;
+    case 14: *out = I->timed_pairs.load(); break;
     default: return LGX_EINVAL;
   }
+  return LGX_OK;
+}
+
+int lgx_instance_set_timing(lgx_instance *I, int enable)
+{
+  if (!I) return LGX_EINVAL;
+  I->timing.store(enable ? 1 : 0);
+  I->ns_a.store(0); I->ns_c.store(0); I->timed_pairs.store(0);
   return LGX_OK;
 }
 
@@ -464,13 +483,25 @@ int lgx_search_range(const lgx_instance *I, uint64_t seed, uint64_t first_id, ui
   Workspace W;
   int rc = ws_alloc(I, n, true, st, W);
   if (rc != LGX_OK) return rc;
-  rc = run_chunks(I, ka, kc, P, n, W, st);
+  std::vector<cudaEvent_t> evs;
+  const bool timed = I->timing.load() != 0;
+  rc = run_chunks(I, ka, kc, P, n, W, st, timed ? &evs : nullptr);
   unsigned long long res[2] = {0, 0};
   if (rc == LGX_OK) {
     cudaError_t e = cudaMemcpyAsync(res, W.result, sizeof res, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) rc = cuda_fail(e, "lgx_search: copy/synchronize");
   }
+  if (rc == LGX_OK) {
+    for (size_t k = 0; k + 3 <= evs.size(); k += 3) {
+      float ma = 0.f, mc = 0.f;
+      if (cudaEventElapsedTime(&ma, evs[k], evs[k + 1]) == cudaSuccess &&
+          cudaEventElapsedTime(&mc, evs[k + 1], evs[k + 2]) == cudaSuccess) {
+        I->ns_a.fetch_add((long long)(ma * 1e6)); I->ns_c.fetch_add((long long)(mc * 1e6)); I->timed_pairs.fetch_add(1);
+      }
+    }
+  }
+  for (cudaEvent_t e : evs) cudaEventDestroy(e);
   cudaFreeAsync(W.base, st);
   if (rc != LGX_OK) return rc;
   if (res[0] == ~0ull && res[1] == ~0ull) {          // no feasible candidate: +inf, lowest id (R19, R29)
