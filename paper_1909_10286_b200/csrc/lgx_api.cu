@@ -299,6 +299,8 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   int64_t tc = ((budget + 1024) / kFinishBlocksPerSM - 1024 - (int64_t)H.imagec_bytes) / (int64_t)c_state;
   ta = std::min<int64_t>(ta, kMaxThreads) / 32 * 32;
   tc = std::min<int64_t>(tc, kMaxThreads) / 32 * 32;
+  if (const char *ev = std::getenv("LGX_THREADS_A")) { const int v = std::atoi(ev); if (v >= 32 && v <= ta) ta = v / 32 * 32; }  // tuning knobs
+  if (const char *ev = std::getenv("LGX_THREADS_C")) { const int v = std::atoi(ev); if (v >= 32 && v <= tc) tc = v / 32 * 32; }
   if (ta < 32 || tc < 32) { delete I; return LGX_ETOOBIG; }
   I->threads_a = (int)ta; I->threads_c = (int)tc;
   I->grid = I->sm_count;                       // one persistent block per SM

@@ -188,3 +188,37 @@ def test_paper_scale_workload(ctxs):
     want = o.eval_batch(inst.seed, first_id=0, n=n)
     got = [t.cpu().numpy() for t in g.eval_batch(inst.seed, first_id=0, n=n)]
     assert np.array_equal(got[3], want[3]) and np.array_equal(got[0], want[0])
+
+
+def test_timing_hook_and_query(ctxs):
+    inst, o, g = ctxs("small")
+    info = g.info()
+    assert info["threads"] % 32 == 0 and info["threads_finish"] % 32 == 0 and info["grid"] == info["sm_count"]
+    assert info["smem_bytes"] <= 227 * 1024 and info["record_bytes"] > 0 and info["chunk"] % info["threads"] == 0
+    l0 = g.query(7)
+    g.set_timing(True)
+    want = g.search(inst.seed, 3 * info["chunk"] + 5)
+    ns_a, ns_c, pairs = g.kernel_times()
+    assert pairs == 4 and ns_a > 0 and ns_c > 0 and g.query(7) - l0 == 8      # 4 chunks x 2 kernels
+    g.set_timing(False)
+    assert g.kernel_times() == (0, 0, 0)
+    assert g.search(inst.seed, 3 * info["chunk"] + 5) == want                 # timing does not change results
+
+
+def test_concurrent_streams_share_an_instance(ctxs):
+    """The instance is immutable and every call owns its workspace: calls on different
+    streams may overlap (include/lgx.h)."""
+    inst, o, g = ctxs("small")
+    n = 1 << 18
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    with torch.cuda.stream(s1):
+        a = g.eval_batch(inst.seed, first_id=0, n=n, stream=s1)
+    with torch.cuda.stream(s2):
+        b = g.eval_batch(inst.seed, first_id=n, n=n, stream=s2)
+    torch.cuda.synchronize()
+    ref = g.eval_batch(inst.seed, first_id=0, n=2 * n)
+    torch.cuda.synchronize()
+    assert torch.equal(torch.cat([a[0], b[0]]), ref[0]) and torch.equal(torch.cat([a[3], b[3]]), ref[3])
+    want = o.eval_batch(inst.seed, first_id=n - 100, n=200)
+    got = ref[0][n - 100:n + 100].cpu().numpy()
+    assert np.array_equal(got, want[0])
