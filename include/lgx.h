@@ -105,7 +105,7 @@ int lgx_decode_batch(const lgx_instance *inst, uint64_t seed,
 
 /* Introspection for bench.py / tests: what = 0 image bytes (both images), 1 threads per block
  * of the decode/walk kernel, 2 blocks in the persistent grid, 3 its dynamic shared memory
- * bytes per block, 4 distance mode (0 = packed tables in smem, 1 = coordinates),
+ * bytes per block, 4 distance mode (0 = packed tables in smem, 1 = coordinates, 2 = field x BP table + coordinates),
  * 5 per-candidate state bytes of the decode/walk kernel, 6 SM count, 7 kernel launches issued
  * so far through this instance, 8 / 9 threads per block / shared memory bytes of the finish
  * kernel, 10 candidates per kernel pair (chunk), 11 bytes per queue record.                 */

@@ -62,11 +62,12 @@ using KernelFn = void (*)(const KParams);
 
 template <int MODE> void pick_kernels(const ImgHdr &h, KernelFn &ka, KernelFn &kc)
 {
-  const bool p16 = h.perm16 != 0, co = h.coords != 0; const int mw = (int)h.mask_words;
+  const bool p16 = h.perm16 != 0; const int dm = h.coords, mw = (int)h.mask_words;
   ka = kc = nullptr;
-#define LGX_PICK(P, C, M) if (p16 == P && co == C && mw == M) { ka = lgx_decode_walk<P, C, M, MODE>; kc = lgx_finish<P, C, M, MODE>; }
-  LGX_PICK(false, false, 1) LGX_PICK(false, false, 2) LGX_PICK(false, true, 1) LGX_PICK(false, true, 2)
-  LGX_PICK(true,  false, 1) LGX_PICK(true,  false, 2) LGX_PICK(true,  true, 1) LGX_PICK(true,  true, 2)
+  // the finish kernel only distinguishes "field x BP table" (DM 0 / 2 -> 0) from coordinates (1)
+#define LGX_PICK(P, D, M) if (p16 == P && dm == D && mw == M) { ka = lgx_decode_walk<P, D, M, MODE>; kc = lgx_finish<P, (D == 1 ? 1 : 0), M, MODE>; }
+  LGX_PICK(false, 0, 1) LGX_PICK(false, 0, 2) LGX_PICK(false, 1, 1) LGX_PICK(false, 1, 2) LGX_PICK(false, 2, 1) LGX_PICK(false, 2, 2)
+  LGX_PICK(true,  0, 1) LGX_PICK(true,  0, 2) LGX_PICK(true,  1, 1) LGX_PICK(true,  1, 2) LGX_PICK(true,  2, 1) LGX_PICK(true,  2, 2)
 #undef LGX_PICK
 }
 
@@ -216,16 +217,22 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   //      else vertex coordinates
   const uint64_t tri_bytes = (uint64_t)(nf + 1) * (uint64_t)nf / 2 * 8, dfb_bytes = (uint64_t)nf * nb * 8;
   const uint64_t small_bytes = 8ull * nf + 4ull * (nb + nhu + nsu) + 1ull * nsu + 128;
-  H.coords = (small_bytes + tri_bytes + dfb_bytes + 256ull * a_state > (uint64_t)kMaxSmem - 1024) ? 1 : 0;
-  uint32_t off = 0;
-  if (!H.coords) {
-    H.off_dtri = off; off = align16(off + (uint32_t)tri_bytes);
-    H.off_dfb  = off; off = align16(off + (uint32_t)dfb_bytes);
-    H.off_xy = 0;
-  } else {
-    H.off_dtri = H.off_dfb = 0;
-    H.off_xy = off; off = align16(off + 16u * (uint32_t)(1 + nb + nf));
+  // distance mode: 0 = both tables, 2 = field x BP table + coordinates for the HU legs, 1 = coordinates only
+  const uint64_t xy_bytes = 16ull * (1 + nb + nf), room = (uint64_t)kMaxSmem - 1024;
+  if (small_bytes + tri_bytes + dfb_bytes + 256ull * a_state <= room) H.coords = 0;
+  else {
+    // Measured on B200 (Large config): at the 8-9 resident warps per SM these sizes allow, the
+    // kernels are latency-bound and recomputing sqrt from coordinates (one conflict-prone
+    // LDS.128 shared by both legs) beats a second conflict-prone table look-up (1.4e8 vs 0.9e8
+    // cand/s), so mode 2 is never picked automatically; LGX_DIST_MODE=2 selects it for tuning.
+    H.coords = 1;
   }
+  if (const char *ev = std::getenv("LGX_DIST_MODE")) { const int v = std::atoi(ev); if (v == 1 || v == 2) H.coords = v; }  // tuning knob
+  uint32_t off = 0;
+  H.off_dtri = H.off_dfb = H.off_xy = 0;
+  if (H.coords == 0) { H.off_dtri = off; off = align16(off + (uint32_t)tri_bytes); }
+  if (H.coords != 1) { H.off_dfb = off; off = align16(off + (uint32_t)dfb_bytes); }
+  if (H.coords != 0) { H.off_xy = off; off = align16(off + (uint32_t)xy_bytes); }
   H.off_sh   = off; off = align16(off + 8u * (uint32_t)nf);
   H.off_dq   = off; off = align16(off + 4u * (uint32_t)nb);
   H.off_rq   = off; off = align16(off + 4u * (uint32_t)nhu);
@@ -235,8 +242,9 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   // ---- image C
   const int n_rcp = std::max(nf, std::max(nb, nhu)) + 1;
   off = 0;
-  if (!H.coords) { H.offc_dfb = off; off = align16(off + (uint32_t)dfb_bytes); H.offc_xy = 0; }
-  else           { H.offc_dfb = 0; H.offc_xy = off; off = align16(off + 16u * (uint32_t)(1 + nb + nf)); }
+  H.offc_dfb = H.offc_xy = 0;
+  if (H.coords != 1) { H.offc_dfb = off; off = align16(off + (uint32_t)dfb_bytes); }
+  else               { H.offc_xy = off; off = align16(off + (uint32_t)xy_bytes); }
   H.offc_s    = off; off = align16(off + 4u * (uint32_t)nf);
   H.offc_cs   = off; off = align16(off + 4u * (uint32_t)nsu);
   H.offc_rcp  = off; off = align16(off + 8u * (uint32_t)n_rcp);
@@ -246,7 +254,7 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   I->image.assign(H.image_bytes, 0);
   I->image_c.assign(H.imagec_bytes, 0);
   uint8_t *img = I->image.data(), *imc = I->image_c.data();
-  if (!H.coords) {
+  if (H.coords == 0) {
     // strict lower triangle over {HQ = 0, field f = f + 1}: entry (hi, lo) at hi(hi-1)/2 + lo
     double *tri = reinterpret_cast<double *>(img + H.off_dtri);
     for (int hi = 1; hi <= nf; ++hi)
@@ -255,12 +263,18 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
         const double bx = lo ? d->field_x[lo - 1] : d->hq_x, by = lo ? d->field_y[lo - 1] : d->hq_y;
         tri[(size_t)hi * (hi - 1) / 2 + lo] = edge(ax, ay, bx, by);
       }
+  }
+  if (H.coords != 1) {
     double *dfb = reinterpret_cast<double *>(img + H.off_dfb), *dfc = reinterpret_cast<double *>(imc + H.offc_dfb);
     for (int f = 0; f < nf; ++f)
       for (int b = 0; b < nb; ++b)
         dfb[(size_t)f * nb + b] = dfc[(size_t)f * nb + b] = edge(d->field_x[f], d->field_y[f], d->bp_x[b], d->bp_y[b]);
-  } else {
-    for (double *xy : { reinterpret_cast<double *>(img + H.off_xy), reinterpret_cast<double *>(imc + H.offc_xy) }) {
+  }
+  {
+    std::vector<double *> dst;
+    if (H.coords != 0) dst.push_back(reinterpret_cast<double *>(img + H.off_xy));
+    if (H.coords == 1) dst.push_back(reinterpret_cast<double *>(imc + H.offc_xy));
+    for (double *xy : dst) {
       xy[0] = d->hq_x; xy[1] = d->hq_y;
       for (int b = 0; b < nb; ++b) { xy[2 * (1 + b)] = d->bp_x[b]; xy[2 * (1 + b) + 1] = d->bp_y[b]; }
       for (int f = 0; f < nf; ++f) { xy[2 * (1 + nb + f)] = d->field_x[f]; xy[2 * (1 + nb + f) + 1] = d->field_y[f]; }

@@ -33,7 +33,7 @@ constexpr int      kFinishBlocksPerSM = 2;       // the finish kernel's image is
 struct ImgHdr {
   int32_t  n_f, n_b, n_hu, n_su, n_t;
   uint32_t thresh;
-  int32_t  coords;          // 0: packed HQ+field triangle + field x BP table; 1: coordinates
+  int32_t  coords;          // distance mode 0: HQ+field triangle + field x BP table; 1: coordinates; 2: field x BP table + coordinates
   int32_t  perm16;          // field ids / segment ends stored as u16 instead of u8
   double   v_hu, v_su, kappa, w_path, w_time;
   uint32_t mask_words;      // 64-bit words per SU mask (1 or 2)

@@ -222,3 +222,18 @@ def test_concurrent_streams_share_an_instance(ctxs):
     want = o.eval_batch(inst.seed, first_id=n - 100, n=200)
     got = ref[0][n - 100:n + 100].cpu().numpy()
     assert np.array_equal(got, want[0])
+
+
+@pytest.mark.parametrize("mode", ["1", "2"])
+def test_distance_modes_agree(ctxs, mode, monkeypatch):
+    """The three distance modes (tables / coordinates / mixed) compute the same D(u,v) bit for bit."""
+    monkeypatch.setenv("LGX_DIST_MODE", mode)
+    for name in ("small", "large"):
+        inst = wl.make(name)
+        g2 = binding.Instance(inst)
+        assert g2.info()["coords"] == int(mode)
+        _, o, _ = ctxs(name)
+        want = o.eval_batch(inst.seed, first_id=0, n=4096)
+        got = [t.cpu().numpy() for t in g2.eval_batch(inst.seed, first_id=0, n=4096)]
+        assert np.array_equal(got[3], want[3]) and np.array_equal(got[0], want[0])
+        assert g2.search(inst.seed, 4096) == o.search(inst.seed, 4096)
