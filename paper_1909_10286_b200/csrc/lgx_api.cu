@@ -162,25 +162,23 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   H.n_bpseq_words  = cdiv((uint32_t)nb, 4u);
   H.n_segend_words = cdiv((uint32_t)nb, EPW);
 
-  // ---- state rows of the decode/walk kernel
-  const uint32_t n_small = (uint32_t)std::max(nb, std::max(nhu, nsu));
+  // ---- state rows of the decode/walk kernel (BP partition + field loop only: the HU / SU
+  //      partitions run in the finish kernel, for the candidates that pass eq. (2))
+  const uint32_t n_units = (uint32_t)std::max(nhu, nsu);
   {
     uint32_t r = 0;
     H.a64_sd = r; H.a64_ent = r; r += (uint32_t)nb;    // entry j is consumed before SD[j] is flushed: same rows
     H.a64_lt = r; r += (uint32_t)nt;
-    H.a64_mask = r; r += (uint32_t)nt * MW;
     H.a64_rows = r;
     r = 0;
     H.a32_perm = r;   r += H.n_perm_words;
     H.a32_bpseq = r;  r += H.n_bpseq_words;
-    // partition scratch (dead once the field loop starts) shares its rows with the segment ends
-    const uint32_t scra_words = (n_small + 3u) / 4u + 1u, scrb_words = cdiv((uint32_t)nb, 4u);
+    // partition scratch (dead once the field loop starts) shares its rows with the segment ends;
+    // the diagnostic decode mode also runs the unit partitions through scratch A
+    const uint32_t scra_words = ((uint32_t)std::max(nb, (int)n_units) + 3u) / 4u + 1u, scrb_words = cdiv((uint32_t)nb, 4u);
     H.a32_scra = r; H.a32_segend = r; H.a32_scrb = r + scra_words;
     r += std::max(scra_words + scrb_words, (uint32_t)nb);
     H.a32_hq = r;     r += (uint32_t)nt;
-    H.a32_s = r;      r += (uint32_t)nt;
-    H.a32_r = r;      r += (uint32_t)nt;
-    H.a32_cnt = r;    r += (uint32_t)nt;
     H.a32_rows = r;
   }
   // ---- state rows of the finish kernel
@@ -193,16 +191,18 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
     r = 0;
     H.c32_s = r; r += (uint32_t)nt;
     H.c32_nhu = r; r += (uint32_t)nt;
+    H.c32_r = r; r += (uint32_t)nt;
     H.c32_ng = r; r += (uint32_t)nt;
     H.c32_magic = r; r += (uint32_t)nt;
     H.c32_bpseq = r; r += H.n_bpseq_words;
     H.c32_segend = r; r += H.n_segend_words;
+    H.c32_scra = r; r += (n_units + 3u) / 4u + 1u;
     H.c32_rows = r;
   }
   // ---- queue record
   {
     uint32_t w = 2;
-    H.rec_tw = 6u + 2u * MW;
+    H.rec_tw = 3u;
     H.rec_tour = w;   w += (uint32_t)nt * H.rec_tw;
     H.rec_sd = w;     w += 2u * (uint32_t)nb;
     H.rec_bpseq = w;  w += H.n_bpseq_words;
@@ -216,7 +216,7 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   // ---- image AB: packed distance tables when they leave room for >= 256 candidates per SM,
   //      else vertex coordinates
   const uint64_t tri_bytes = (uint64_t)(nf + 1) * (uint64_t)nf / 2 * 8, dfb_bytes = (uint64_t)nf * nb * 8;
-  const uint64_t small_bytes = 8ull * nf + 4ull * (nb + nhu + nsu) + 1ull * nsu + 128;
+  const uint64_t small_bytes = 8ull * nf + 4ull * nb + 64;
   // distance mode: 0 = both tables, 2 = field x BP table + coordinates for the HU legs, 1 = coordinates only
   const uint64_t xy_bytes = 16ull * (1 + nb + nf), room = (uint64_t)kMaxSmem - 1024;
   if (small_bytes + tri_bytes + dfb_bytes + 256ull * a_state <= room) H.coords = 0;
@@ -235,9 +235,6 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   if (H.coords != 0) { H.off_xy = off; off = align16(off + (uint32_t)xy_bytes); }
   H.off_sh   = off; off = align16(off + 8u * (uint32_t)nf);
   H.off_dq   = off; off = align16(off + 4u * (uint32_t)nb);
-  H.off_rq   = off; off = align16(off + 4u * (uint32_t)nhu);
-  H.off_cs   = off; off = align16(off + 4u * (uint32_t)nsu);
-  H.off_rank = off; off = align16(off + (uint32_t)nsu);
   H.image_bytes = off;
   // ---- image C
   const int n_rcp = std::max(nf, std::max(nb, nhu)) + 1;
@@ -249,6 +246,8 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   H.offc_cs   = off; off = align16(off + 4u * (uint32_t)nsu);
   H.offc_rcp  = off; off = align16(off + 8u * (uint32_t)n_rcp);
   H.offc_unit = off; off = align16(off + (uint32_t)nsu);
+  H.offc_rank = off; off = align16(off + (uint32_t)nsu);
+  H.offc_rq   = off; off = align16(off + 4u * (uint32_t)nhu);
   H.imagec_bytes = off;
 
   I->image.assign(H.image_bytes, 0);
@@ -284,16 +283,16 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   for (int f = 0; f < nf; ++f) { sh[2 * f] = sc[f] = (uint32_t)s_q[f]; sh[2 * f + 1] = (uint32_t)h_q[f]; }
   uint32_t *dq = reinterpret_cast<uint32_t *>(img + H.off_dq);
   for (int b = 0; b < nb; ++b) dq[b] = (uint32_t)d_q[b];
-  uint32_t *rq = reinterpret_cast<uint32_t *>(img + H.off_rq);
+  uint32_t *rq = reinterpret_cast<uint32_t *>(imc + H.offc_rq);
   for (int u = 0; u < nhu; ++u) rq[u] = (uint32_t)r_q[u];
   // SUs ascending by (capacity quanta, unit index): "rising fill times" (R16, R17)
   std::vector<int> order(nsu);
   std::iota(order.begin(), order.end(), 0);
   std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return c_q[a] < c_q[b]; });
-  uint32_t *cs = reinterpret_cast<uint32_t *>(img + H.off_cs), *cc = reinterpret_cast<uint32_t *>(imc + H.offc_cs);
+  uint32_t *cc = reinterpret_cast<uint32_t *>(imc + H.offc_cs);
   for (int r = 0; r < nsu; ++r) {
-    cs[r] = cc[r] = (uint32_t)c_q[order[r]];
-    imc[H.offc_unit + r] = (uint8_t)order[r]; img[H.off_rank + order[r]] = (uint8_t)r;
+    cc[r] = (uint32_t)c_q[order[r]];
+    imc[H.offc_unit + r] = (uint8_t)order[r]; imc[H.offc_rank + order[r]] = (uint8_t)r;
   }
   double *rcp = reinterpret_cast<double *>(imc + H.offc_rcp);
   rcp[0] = 0.0;
@@ -311,7 +310,7 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   int64_t ta = (budget - (int64_t)H.image_bytes) / (int64_t)a_state;
   // finish kernel: kFinishBlocksPerSM blocks per SM (each with its own copy of image C)
   int64_t tc = ((budget + 1024) / kFinishBlocksPerSM - 1024 - (int64_t)H.imagec_bytes) / (int64_t)c_state;
-  ta = std::min<int64_t>(ta, kMaxThreads) / 32 * 32;
+  ta = std::min<int64_t>(ta, kMaxThreadsA) / 32 * 32;
   tc = std::min<int64_t>(tc, kMaxThreads) / 32 * 32;
   if (const char *ev = std::getenv("LGX_THREADS_A")) { const int v = std::atoi(ev); if (v >= 32 && v <= ta) ta = v / 32 * 32; }  // tuning knobs
   if (const char *ev = std::getenv("LGX_THREADS_C")) { const int v = std::atoi(ev); if (v >= 32 && v <= tc) tc = v / 32 * 32; }

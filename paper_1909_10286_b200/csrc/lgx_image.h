@@ -3,10 +3,9 @@
 // candidate from the decode/walk kernel to the finish kernel.
 // Product code (CUDA path).  Shares nothing with oracle/.
 //
-// Image AB (decode + pass 1):   distance tables or coordinates | {s_q,h_q} per field |
-//                               demand quanta | HU rate quanta | SU capacities by rank | unit->rank
-// Image C  (Alg. 2 + pass 2):   field x BP table or coordinates | s_q per field |
-//                               SU capacities by rank | RN(1/k) table | rank->unit
+// Image AB (decode + pass 1):   distance tables or coordinates | {s_q,h_q} per field | demand quanta
+// Image C  (Alg. 2 + pass 2):   field x BP table or coordinates | s_q per field | HU rate quanta |
+//                               SU capacities by rank | RN(1/k) table | unit<->rank maps
 // Both are contiguous, 16-byte aligned blobs built on the host by lgx_instance_create and
 // copied global -> shared once per (persistent) block.
 //
@@ -27,7 +26,8 @@ constexpr uint32_t kPhiloxM1    = 0xCD9E8D57u;
 constexpr uint32_t kPhiloxW0    = 0x9E3779B9u;   // key increments
 constexpr uint32_t kPhiloxW1    = 0xBB67AE85u;
 constexpr int      kMaxSmem     = 227 * 1024;    // opt-in dynamic shared memory per block, sm_100a
-constexpr int      kMaxThreads  = 512;           // __launch_bounds__ of the candidate kernels
+constexpr int      kMaxThreads  = 512;           // __launch_bounds__ of the finish kernel
+constexpr int      kMaxThreadsA = 640;           // __launch_bounds__ of the decode/walk kernel (<= 96 registers)
 constexpr int      kFinishBlocksPerSM = 2;       // the finish kernel's image is small: two blocks share an SM
 
 struct ImgHdr {
@@ -47,29 +47,28 @@ struct ImgHdr {
   uint32_t off_xy;          // f64x2 [1 + n_b + n_f]  vertex coordinates (coords mode)
   uint32_t off_sh;          // u32x2 [n_f]            {s_q, h_q}
   uint32_t off_dq;          // u32 [n_b]              demand quanta
-  uint32_t off_rq;          // u32 [n_hu]             HU rate quanta
-  uint32_t off_cs;          // u32 [n_su]             SU capacity quanta, ascending (c_q, unit)
-  uint32_t off_rank;        // u8  [n_su]             unit -> rank
   uint32_t image_bytes;
 
   // ---- image C (byte offsets inside image C)
   uint32_t offc_dfb, offc_xy, offc_s, offc_cs, offc_rcp, offc_unit;
+  uint32_t offc_rq;         // u32 [n_hu]  HU rate quanta
+  uint32_t offc_rank;       // u8  [n_su]  unit -> rank
   uint32_t imagec_bytes;
 
   // ---- state rows of the decode/walk kernel
-  uint32_t a64_sd, a64_lt, a64_mask, a64_ent, a64_rows;
-  uint32_t a32_perm, a32_bpseq, a32_segend, a32_scra, a32_scrb, a32_hq, a32_s, a32_r, a32_cnt, a32_rows;
+  uint32_t a64_sd, a64_lt, a64_ent, a64_rows;
+  uint32_t a32_perm, a32_bpseq, a32_segend, a32_scra, a32_scrb, a32_hq, a32_rows;
 
   // ---- state rows of the finish kernel
   uint32_t c64_w, c64_e, c64_mask, c64_rows;
-  uint32_t c32_s, c32_nhu, c32_ng, c32_magic, c32_bpseq, c32_segend, c32_rows;
+  uint32_t c32_s, c32_nhu, c32_r, c32_ng, c32_magic, c32_bpseq, c32_segend, c32_scra, c32_rows;
 
   // ---- queue record (32-bit words, stored transposed: word w of slot q at queue[w*cap + q])
-  //   0,1 index i | per tour g at rec_tour + g*rec_tw: LT lo,hi, H_q, R_g, S_g, n_HU, MASK words |
+  //   0,1 index i | per tour g at rec_tour + g*rec_tw: LT lo,hi, H_q |
   //   SD[j] lo,hi at rec_sd + 2j | bpseq words | segend words | perm words
   uint32_t rec_tour, rec_tw, rec_sd, rec_bpseq, rec_segend, rec_perm, rec_words;
   uint32_t n_bpseq_words, n_segend_words, n_perm_words;
-  uint32_t pad_[2];
+  uint32_t pad_[1];
 };
 static_assert(sizeof(ImgHdr) % 16 == 0, "image header must keep 16-byte alignment");
 
