@@ -194,8 +194,7 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
     H.c32_r = r; r += (uint32_t)nt;
     H.c32_ng = r; r += (uint32_t)nt;
     H.c32_magic = r; r += (uint32_t)nt;
-    H.c32_bpseq = r; r += H.n_bpseq_words;
-    H.c32_segend = r; r += H.n_segend_words;
+    H.c32_ent = r; r += (uint32_t)nb;
     H.c32_scra = r; r += (n_units + 3u) / 4u + 1u;
     H.c32_rows = r;
   }

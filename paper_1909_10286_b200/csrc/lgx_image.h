@@ -61,14 +61,14 @@ struct ImgHdr {
 
   // ---- state rows of the finish kernel
   uint32_t c64_w, c64_e, c64_mask, c64_rows;
-  uint32_t c32_s, c32_nhu, c32_r, c32_ng, c32_magic, c32_bpseq, c32_segend, c32_scra, c32_rows;
+  uint32_t c32_s, c32_nhu, c32_r, c32_ng, c32_magic, c32_ent, c32_scra, c32_rows;
 
   // ---- queue record (32-bit words, stored transposed: word w of slot q at queue[w*cap + q])
   //   0,1 index i | per tour g at rec_tour + g*rec_tw: LT lo,hi, H_q |
   //   SD[j] lo,hi at rec_sd + 2j | bpseq words | segend words | perm words
   uint32_t rec_tour, rec_tw, rec_sd, rec_bpseq, rec_segend, rec_perm, rec_words;
   uint32_t n_bpseq_words, n_segend_words, n_perm_words;
-  uint32_t pad_[1];
+  uint32_t pad_[2];
 };
 static_assert(sizeof(ImgHdr) % 16 == 0, "image header must keep 16-byte alignment");
 
