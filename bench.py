@@ -32,10 +32,14 @@ ALG2_ITERS = {"toy": 2.3, "small": 5.6, "medium": 9.9, "large": 12.7, "sweep": 1
 def w_alg(inst, workload):
     nf, nb, nt, nhu, nsu = inst.n_fields, inst.n_bps, inst.n_tours, inst.n_hu, inst.n_su
     cd = lambda a, b: -(-a // b)
-    blocks = cd(nf, 4) + sum(cd(n, 4) + cd(n - nt, 4) for n in (nb, nhu, nsu)) + cd((nb - 1) * 4 // 3 + 8, 4)
-    decode_walk = (40 * blocks + 7 * (nf + nb + nhu + nsu) + 2 * (nb + nhu + nsu - 3 * nt)
-                   + 6 * nb + 6 * nhu + 10 * nsu + 14 * nf + 10 * (nb + nt))
-    finish = 6 * nb + 92 * nt + 110 * ALG2_ITERS.get(workload, 10.0) + 18 * nf + 10 * (nb + nt) + 9 * nt + 5
+    part_blocks = lambda n: cd(n, 4) + cd(n - nt, 4)            # Philox blocks of one ordered partition
+    # every candidate: BP partition, field permutation + extras, pass 1  (kernel lgx_decode_walk)
+    blocks_a = cd(nf, 4) + part_blocks(nb) + cd((nb - 1) * 4 // 3 + 8, 4)
+    decode_walk = 40 * blocks_a + 7 * (nf + nb) + 2 * (nb - nt) + 6 * nb + 14 * nf + 10 * (nb + nt)
+    # feasible candidates only: HU / SU partitions, tour statistics, Algorithm 2, pass 2, cost  (lgx_finish)
+    blocks_c = part_blocks(nhu) + part_blocks(nsu)
+    finish = (40 * blocks_c + 7 * (nhu + nsu) + 2 * (nhu + nsu - 2 * nt) + 6 * nhu + 10 * nsu
+              + 6 * nb + 92 * nt + 110 * ALG2_ITERS.get(workload, 10.0) + 18 * nf + 10 * (nb + nt) + 9 * nt + 5)
     return decode_walk, finish
 
 
