@@ -600,3 +600,247 @@ int lgo_search(const lgo_instance *I, uint64_t seed, uint64_t first_id, uint64_t
   plan_free(&P);
   return LGO_OK;
 }
+
+/* ================================================================== NEXT rows: Algorithm 1 */
+
+/* Explicit plan as ordered lists (built from / written back to the array form). */
+typedef struct {
+  int n_t, n_b, n_f;
+  int *tour_len, *tour_bp;      /* tour_bp[g*n_b + pos] */
+  int *bp_len, *bp_field;       /* bp_field[b*n_f + pos] */
+} plan_lists;
+
+static int lists_from_arrays(const lgo_instance *I, plan_lists *L, const uint8_t *bp_tour, const uint8_t *bp_pos,
+                             const uint16_t *field_bp, const uint16_t *field_pos)
+{
+  L->n_t = I->n_t; L->n_b = I->n_b; L->n_f = I->n_f;
+  L->tour_len = (int *)calloc((size_t)I->n_t, sizeof(int));
+  L->tour_bp = (int *)malloc(sizeof(int) * (size_t)I->n_t * (size_t)I->n_b);
+  L->bp_len = (int *)calloc((size_t)I->n_b, sizeof(int));
+  L->bp_field = (int *)malloc(sizeof(int) * (size_t)I->n_b * (size_t)I->n_f);
+  for (int b = 0; b < I->n_b; b++) {
+    if (bp_tour[b] >= I->n_t || bp_pos[b] >= I->n_b) return LGO_EINVAL;
+    L->tour_bp[bp_tour[b] * I->n_b + bp_pos[b]] = b; L->tour_len[bp_tour[b]]++;
+  }
+  for (int f = 0; f < I->n_f; f++) {
+    if (field_bp[f] >= I->n_b || field_pos[f] >= I->n_f) return LGO_EINVAL;
+    L->bp_field[field_bp[f] * I->n_f + field_pos[f]] = f; L->bp_len[field_bp[f]]++;
+  }
+  return LGO_OK;
+}
+static void lists_to_arrays(const plan_lists *L, uint8_t *bp_tour, uint8_t *bp_pos, uint16_t *field_bp, uint16_t *field_pos)
+{
+  for (int g = 0; g < L->n_t; g++)
+    for (int q = 0; q < L->tour_len[g]; q++) { int b = L->tour_bp[g * L->n_b + q]; bp_tour[b] = (uint8_t)g; bp_pos[b] = (uint8_t)q; }
+  for (int b = 0; b < L->n_b; b++)
+    for (int q = 0; q < L->bp_len[b]; q++) { int f = L->bp_field[b * L->n_f + q]; field_bp[f] = (uint16_t)b; field_pos[f] = (uint16_t)q; }
+}
+static void lists_free(plan_lists *L) { free(L->tour_len); free(L->tour_bp); free(L->bp_len); free(L->bp_field); }
+
+static void list_remove(int *list, int *len, int value)
+{
+  int k = 0;
+  while (list[k] != value) k++;
+  for (; k + 1 < *len; k++) list[k] = list[k + 1];
+  (*len)--;
+}
+static void list_insert(int *list, int *len, int pos, int value)
+{
+  for (int k = *len; k > pos; k--) list[k] = list[k - 1];
+  list[pos] = value; (*len)++;
+}
+
+/* Algorithm 1, steps 1-3. */
+int lgo_init_plan(const lgo_instance *I, uint8_t *bp_tour, uint8_t *bp_pos, uint16_t *field_bp, uint16_t *field_pos,
+                  uint8_t *hu_tour, uint8_t *su_tour)
+{
+  if (!I || !bp_tour || !bp_pos || !field_bp || !field_pos || !hu_tour || !su_tour) return LGO_EINVAL;
+  const int nt = I->n_t, nb = I->n_b, nf = I->n_f;
+  /* Step 1 (i) (L122): "approximately equal number of HUs to each tour ... N_HU(N_T) capturing
+   * the integer residual" (the printed N_B/N_T is read as N_HU^total/N_T, R25): units in index
+   * order, floor(N_HU/N_T) per tour, the rest on the last tour. */
+  { int per = I->n_hu / nt;
+    for (int u = 0; u < I->n_hu; u++) { int g = u / per; hu_tour[u] = (uint8_t)(g < nt ? g : nt - 1); } }
+  /* SUs: Case 1 gives every tour the same number of each class (L273: 2 small + 4 large):
+   * units sorted by (capacity, index) are dealt round-robin (R31). */
+  { int *ord = (int *)malloc(sizeof(int) * (size_t)I->n_su); char *used = (char *)calloc((size_t)I->n_su, 1);
+    for (int r = 0; r < I->n_su; r++) {
+      int u = -1;
+      for (int w = 0; w < I->n_su; w++) if (!used[w] && (u < 0 || I->c_q[w] < I->c_q[u])) u = w;
+      used[u] = 1; ord[r] = u;
+    }
+    for (int r = 0; r < I->n_su; r++) su_tour[ord[r]] = (uint8_t)(r % nt);
+    free(ord); free(used); }
+  /* Step 1 (ii) (L122): nearest-neighbour chain over the BPs starting at HQ; the chain is cut
+   * into N_T consecutive runs, tour g taking chain[floor(g N_B/N_T) .. floor((g+1) N_B/N_T)) (R32). */
+  { char *used = (char *)calloc((size_t)nb, 1); int *chain = (int *)malloc(sizeof(int) * (size_t)nb);
+    int cur = 0 /* HQ */;
+    for (int k = 0; k < nb; k++) {
+      int best = -1; double bd = 0.0;
+      for (int b = 0; b < nb; b++) if (!used[b]) { double d = D(I, cur, 1 + b); if (best < 0 || d < bd) { best = b; bd = d; } }
+      used[best] = 1; chain[k] = best; cur = 1 + best;
+    }
+    for (int g = 0; g < nt; g++) {
+      int lo = (int)(((long)g * nb) / nt), hi = (int)(((long)(g + 1) * nb) / nt);
+      for (int k = lo; k < hi; k++) { bp_tour[chain[k]] = (uint8_t)g; bp_pos[chain[k]] = (uint8_t)(k - lo); }
+    }
+    free(used); free(chain); }
+  /* Step 2 (L124): fields, in identification order (L173), go to their closest BP not yet
+   * supplied up to its minimum demand; once every BP is supplied, to their closest BP. */
+  int64_t *Sq = (int64_t *)calloc((size_t)nb, sizeof(int64_t));
+  int *fb = (int *)malloc(sizeof(int) * (size_t)nf);
+  for (int f = 0; f < nf; f++) {
+    int best = -1; double bd = 0.0;
+    for (int b = 0; b < nb; b++) if (Sq[b] < I->d_q[b]) { double d = D(I, 1 + nb + f, 1 + b); if (best < 0 || d < bd) { best = b; bd = d; } }
+    if (best < 0)
+      for (int b = 0; b < nb; b++) { double d = D(I, 1 + nb + f, 1 + b); if (best < 0 || d < bd) { best = b; bd = d; } }
+    fb[f] = best; Sq[best] += I->s_q[f];
+  }
+  /* Step 3 (L126, L171): per BP, nearest-neighbour order "from the HQ to the first field of its
+   * assigned BP, from that field to a closest second field assigned to the same BP, and so forth". */
+  { char *used = (char *)calloc((size_t)nf, 1);
+    for (int b = 0; b < nb; b++) {
+      int cur = 0 /* HQ */, k = 0;
+      for (;;) {
+        int best = -1; double bd = 0.0;
+        for (int f = 0; f < nf; f++) if (fb[f] == b && !used[f]) { double d = D(I, cur, 1 + nb + f); if (best < 0 || d < bd) { best = f; bd = d; } }
+        if (best < 0) break;
+        used[best] = 1; field_bp[best] = (uint16_t)b; field_pos[best] = (uint16_t)k++; cur = 1 + nb + best;
+      }
+    }
+    free(used); }
+  free(Sq); free(fb);
+  return LGO_OK;
+}
+
+/* Step 8: "a simple remove- and reinsert-operation for vertices, which can
+ * represent either a field or a BP".  A field may go to any BP at any position; a BP may go to
+ * any tour or to another index of its tour, and takes all its fields with it (L184).  The vertex
+ * is drawn uniformly over fields and BPs ("since N_F >> N_B, it is more likely to draw fields").
+ * R35: v = below(w0, N_F+N_B); target = below(w1, N_B or N_T); position = below(w2, len+1) with
+ * len the target list's length after the removal. */
+int lgo_apply_move(const lgo_instance *I, uint32_t w0, uint32_t w1, uint32_t w2,
+                   uint8_t *bp_tour, uint8_t *bp_pos, uint16_t *field_bp, uint16_t *field_pos)
+{
+  if (!I) return LGO_EINVAL;
+  plan_lists L;
+  int rc = lists_from_arrays(I, &L, bp_tour, bp_pos, field_bp, field_pos);
+  if (rc == LGO_OK) {
+    const int nf = I->n_f, nb = I->n_b, nt = I->n_t;
+    uint32_t v = below(w0, (uint32_t)(nf + nb));
+    if ((int)v < nf) {
+      int f = (int)v, a = field_bp[f];
+      list_remove(L.bp_field + (size_t)a * nf, &L.bp_len[a], f);
+      int t = (int)below(w1, (uint32_t)nb);
+      int q = (int)below(w2, (uint32_t)(L.bp_len[t] + 1));
+      list_insert(L.bp_field + (size_t)t * nf, &L.bp_len[t], q, f);
+    } else {
+      int b = (int)v - nf, g = bp_tour[b];
+      list_remove(L.tour_bp + (size_t)g * nb, &L.tour_len[g], b);
+      int t = (int)below(w1, (uint32_t)nt);
+      int q = (int)below(w2, (uint32_t)(L.tour_len[t] + 1));
+      list_insert(L.tour_bp + (size_t)t * nb, &L.tour_len[t], q, b);
+    }
+    lists_to_arrays(&L, bp_tour, bp_pos, field_bp, field_pos);
+  }
+  lists_free(&L);
+  return rc;
+}
+
+/* One worker (L163-165): x_i = move(x), then constraint check and cost as in lgo_score. */
+static void worker_eval(const lgo_instance *I, const plan_buf *X, plan_buf *Y, uint64_t seed, uint64_t id, double *sc)
+{
+  uint32_t ctr[4] = { (uint32_t)id, (uint32_t)(id >> 32), 5u, 0u }, key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) }, w[4];
+  lgo_philox4x32_10(ctr, key, w);
+  memcpy(Y->bp_tour, X->bp_tour, (size_t)I->n_b); memcpy(Y->bp_pos, X->bp_pos, (size_t)I->n_b);
+  memcpy(Y->field_bp, X->field_bp, sizeof(uint16_t) * (size_t)I->n_f);
+  memcpy(Y->field_pos, X->field_pos, sizeof(uint16_t) * (size_t)I->n_f);
+  memcpy(Y->hu_tour, X->hu_tour, (size_t)I->n_hu); memcpy(Y->su_init, X->su_init, (size_t)I->n_su);
+  lgo_apply_move(I, w[0], w[1], w[2], Y->bp_tour, Y->bp_pos, Y->field_bp, Y->field_pos);
+  lgo_score(I, Y->bp_tour, Y->bp_pos, Y->field_bp, Y->field_pos, Y->hu_tour, Y->su_init, sc,
+            NULL, NULL, NULL, NULL, NULL, NULL, NULL, Y->su_final);
+}
+
+int lgo_move_eval_batch(const lgo_instance *I,
+                        const uint8_t *bp_tour, const uint8_t *bp_pos, const uint16_t *field_bp, const uint16_t *field_pos,
+                        const uint8_t *hu_tour, const uint8_t *su_tour,
+                        uint64_t seed, uint64_t first_id, uint64_t n,
+                        double *cost, double *path_km, double *makespan_h, uint8_t *feasible)
+{
+  if (!I) return LGO_EINVAL;
+  plan_buf X, Y;
+  if (plan_alloc(I, &X) != LGO_OK || plan_alloc(I, &Y) != LGO_OK) return LGO_ENOMEM;
+  memcpy(X.bp_tour, bp_tour, (size_t)I->n_b); memcpy(X.bp_pos, bp_pos, (size_t)I->n_b);
+  memcpy(X.field_bp, field_bp, sizeof(uint16_t) * (size_t)I->n_f); memcpy(X.field_pos, field_pos, sizeof(uint16_t) * (size_t)I->n_f);
+  memcpy(X.hu_tour, hu_tour, (size_t)I->n_hu); memcpy(X.su_init, su_tour, (size_t)I->n_su);
+  for (uint64_t i = 0; i < n; i++) {
+    double sc[8];
+    worker_eval(I, &X, &Y, seed, first_id + i, sc);
+    if (cost) cost[i] = sc[6];
+    if (path_km) path_km[i] = sc[4];
+    if (makespan_h) makespan_h[i] = sc[5];
+    if (feasible) feasible[i] = (uint8_t)(sc[0] != 0.0);
+  }
+  plan_free(&X); plan_free(&Y);
+  return LGO_OK;
+}
+
+/* Algorithm 1, steps 4-16.  R36: worker ids of iteration k are
+ * k*n_workers .. (k+1)*n_workers-1; the exploration draw u of iteration k is word 0 of the Philox
+ * block (seed; k, stream 6, block 0), u < eps  <=>  draw < eps_thresh (eq. (5)).
+ * R37: an adopted x_i carries the SU assignment Alg. 2 left it with; if every worker of an
+ * iteration is infeasible (C_i* = inf), x_old is kept. */
+int lgo_local_search(const lgo_instance *I,
+                     uint8_t *bp_tour, uint8_t *bp_pos, uint16_t *field_bp, uint16_t *field_pos,
+                     uint8_t *hu_tour, uint8_t *su_tour,
+                     uint64_t seed, uint32_t n_iters, uint32_t n_workers, uint32_t eps_thresh,
+                     double *best_cost, double *hist_cost, uint64_t *hist_id)
+{
+  if (!I || !best_cost || n_workers == 0) return LGO_EINVAL;
+  plan_buf best, old, cur, Y, win;
+  if (plan_alloc(I, &best) || plan_alloc(I, &old) || plan_alloc(I, &cur) || plan_alloc(I, &Y) || plan_alloc(I, &win)) return LGO_ENOMEM;
+  const size_t nb = (size_t)I->n_b, nf2 = sizeof(uint16_t) * (size_t)I->n_f;
+#define PLAN_COPY(dst, src) do { memcpy((dst).bp_tour, (src).bp_tour, nb); memcpy((dst).bp_pos, (src).bp_pos, nb); \
+    memcpy((dst).field_bp, (src).field_bp, nf2); memcpy((dst).field_pos, (src).field_pos, nf2); \
+    memcpy((dst).hu_tour, (src).hu_tour, (size_t)I->n_hu); memcpy((dst).su_init, (src).su_init, (size_t)I->n_su); } while (0)
+  /* Step 4 (L133): x* = x_0 with cost C*, x_old = x*. */
+  memcpy(best.bp_tour, bp_tour, nb); memcpy(best.bp_pos, bp_pos, nb);
+  memcpy(best.field_bp, field_bp, nf2); memcpy(best.field_pos, field_pos, nf2);
+  memcpy(best.hu_tour, hu_tour, (size_t)I->n_hu); memcpy(best.su_init, su_tour, (size_t)I->n_su);
+  double sc[8];
+  int rc = lgo_score(I, best.bp_tour, best.bp_pos, best.field_bp, best.field_pos, best.hu_tour, best.su_init, sc,
+                     NULL, NULL, NULL, NULL, NULL, NULL, NULL, best.su_final);
+  if (rc != LGO_OK) goto out;
+  memcpy(best.su_init, best.su_final, (size_t)I->n_su);
+  double c_star = sc[6];
+  PLAN_COPY(old, best);
+  for (uint32_t k = 0; k < n_iters; k++) {
+    /* Step 6, eq. (5): x = x* if u < eps else x_old (on the host, L231). */
+    uint32_t u = lgo_draw(seed, (uint64_t)k, 6u, 0u);
+    if (u < eps_thresh) PLAN_COPY(cur, best); else PLAN_COPY(cur, old);
+    /* Steps 9-13: every worker moves x once and evaluates; i* = arg min C_i (lowest id on ties). */
+    uint64_t bbits = 0, bid = 0; int have = 0;
+    for (uint32_t i = 0; i < n_workers; i++) {
+      uint64_t id = (uint64_t)k * n_workers + i;
+      worker_eval(I, &cur, &Y, seed, id, sc);
+      uint64_t bits; memcpy(&bits, &sc[6], 8);
+      if (!have || bits < bbits) { bbits = bits; bid = id; have = 1; PLAN_COPY(win, Y); memcpy(win.su_init, Y.su_final, (size_t)I->n_su); }
+    }
+    double c_win; memcpy(&c_win, &bbits, 8);
+    if (hist_cost) hist_cost[k] = c_win;
+    if (hist_id) hist_id[k] = bid;
+    /* Steps 14-15 (L169): update x*, C* if improving; x_old <- x_i*. */
+    if (isfinite(c_win)) {
+      if (c_win < c_star) { c_star = c_win; PLAN_COPY(best, win); }
+      PLAN_COPY(old, win);
+    }
+  }
+  memcpy(bp_tour, best.bp_tour, nb); memcpy(bp_pos, best.bp_pos, nb);
+  memcpy(field_bp, best.field_bp, nf2); memcpy(field_pos, best.field_pos, nf2);
+  memcpy(hu_tour, best.hu_tour, (size_t)I->n_hu); memcpy(su_tour, best.su_init, (size_t)I->n_su);
+  *best_cost = c_star;
+out:
+  plan_free(&best); plan_free(&old); plan_free(&cur); plan_free(&Y); plan_free(&win);
+  return rc;
+#undef PLAN_COPY
+}

@@ -96,6 +96,39 @@ int lgo_decode_batch(const lgo_instance *inst, uint64_t seed, const uint64_t *id
 int lgo_search(const lgo_instance *inst, uint64_t seed, uint64_t first_id, uint64_t budget,
                double *best_cost, uint64_t *best_id);
 
+/* ---- NEXT rows of the scope table: the paper's own search loop --------- */
+
+/* Algorithm 1 steps 1-3: the nearest-neighbour initialisation
+ * "a human scheduler may implicitly conduct".  Writes an explicit plan (same arrays as
+ * lgo_decode).  Readings R31-R34 in DESIGN.md.                                           */
+int lgo_init_plan(const lgo_instance *inst,
+                  uint8_t *bp_tour, uint8_t *bp_pos, uint16_t *field_bp, uint16_t *field_pos,
+                  uint8_t *hu_tour, uint8_t *su_tour);
+
+/* Step 8 (L158, L184): remove one vertex (field or BP) and reinsert it.  The three draws
+ * w0,w1,w2 choose the vertex, the target BP / tour and the position (R35).  In place.    */
+int lgo_apply_move(const lgo_instance *inst, uint32_t w0, uint32_t w1, uint32_t w2,
+                   uint8_t *bp_tour, uint8_t *bp_pos, uint16_t *field_bp, uint16_t *field_pos);
+
+/* Workers i = first_id .. first_id+n-1 of one iteration: x_i = move_i(x), C_i = cost(x_i)
+ * (L163-165).  Draws = Philox block (seed; id, stream 5, block 0).                        */
+int lgo_move_eval_batch(const lgo_instance *inst,
+                        const uint8_t *bp_tour, const uint8_t *bp_pos,
+                        const uint16_t *field_bp, const uint16_t *field_pos,
+                        const uint8_t *hu_tour, const uint8_t *su_tour,
+                        uint64_t seed, uint64_t first_id, uint64_t n,
+                        double *cost, double *path_km, double *makespan_h, uint8_t *feasible);
+
+/* Algorithm 1 steps 5-16 (L136-169) with the exploration rule eq. (5) (L177): n_iters
+ * iterations of n_workers workers.  The plan arrays hold x_0 on entry (its SU assignment
+ * is replaced by Alg. 2's result) and x* on return; hist_cost/hist_id (may be NULL) receive
+ * (C_i*, i*) of every iteration.  eps_thresh = eps * 2^32 (u < eps <=> draw < eps_thresh). */
+int lgo_local_search(const lgo_instance *inst,
+                     uint8_t *bp_tour, uint8_t *bp_pos, uint16_t *field_bp, uint16_t *field_pos,
+                     uint8_t *hu_tour, uint8_t *su_tour,
+                     uint64_t seed, uint32_t n_iters, uint32_t n_workers, uint32_t eps_thresh,
+                     double *best_cost, double *hist_cost, uint64_t *hist_id);
+
 #ifdef __cplusplus
 }
 #endif

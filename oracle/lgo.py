@@ -50,6 +50,18 @@ _lib.lgo_decode_batch.argtypes = [C.c_void_p, C.c_uint64, C.c_void_p, C.c_uint64
 _lib.lgo_search.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint64, C.POINTER(C.c_double),
                             C.POINTER(C.c_uint64)]
 _lib.lgo_philox4x32_10.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+_lib.lgo_init_plan.argtypes = [C.c_void_p] + [C.c_void_p] * 6
+_lib.lgo_apply_move.argtypes = [C.c_void_p, C.c_uint32, C.c_uint32, C.c_uint32] + [C.c_void_p] * 4
+_lib.lgo_move_eval_batch.argtypes = [C.c_void_p] + [C.c_void_p] * 6 + [C.c_uint64, C.c_uint64, C.c_uint64] + [C.c_void_p] * 4
+_lib.lgo_local_search.argtypes = [C.c_void_p] + [C.c_void_p] * 6 + [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32,
+                                                                    C.POINTER(C.c_double), C.c_void_p, C.c_void_p]
+
+PLAN_KEYS = (("bp_tour", np.uint8), ("bp_pos", np.uint8), ("field_bp", np.uint16), ("field_pos", np.uint16),
+             ("hu_tour", np.uint8), ("su_tour", np.uint8))
+
+
+def _plan_arrays(plan):
+    return [np.ascontiguousarray(plan[k], dtype=t).copy() for k, t in PLAN_KEYS]
 
 
 class OracleError(RuntimeError):
@@ -178,3 +190,35 @@ class Oracle:
         rc = _lib.lgo_search(self._h, seed, first_id, budget, C.byref(c), C.byref(i))
         if rc: raise OracleError(rc)
         return c.value, i.value
+
+    # ---- NEXT rows: Algorithm 1 (initialisation, moves, local search)
+    def init_plan(self):
+        bt = np.zeros(self.n_b, np.uint8); bp = np.zeros(self.n_b, np.uint8)
+        fb = np.zeros(self.n_f, np.uint16); fp = np.zeros(self.n_f, np.uint16)
+        hu = np.zeros(self.n_hu, np.uint8); su = np.zeros(self.n_su, np.uint8)
+        rc = _lib.lgo_init_plan(self._h, bt.ctypes.data, bp.ctypes.data, fb.ctypes.data, fp.ctypes.data,
+                                hu.ctypes.data, su.ctypes.data)
+        if rc: raise OracleError(rc)
+        return dict(bp_tour=bt, bp_pos=bp, field_bp=fb, field_pos=fp, hu_tour=hu, su_tour=su)
+
+    def apply_move(self, plan, w0, w1, w2):
+        a = _plan_arrays(plan)
+        rc = _lib.lgo_apply_move(self._h, w0, w1, w2, *[x.ctypes.data for x in a[:4]])
+        if rc: raise OracleError(rc)
+        return dict(zip([k for k, _ in PLAN_KEYS], a))
+
+    def move_eval_batch(self, plan, seed, first_id, n):
+        a = _plan_arrays(plan)
+        cost = np.zeros(n); path = np.zeros(n); mk = np.zeros(n); fe = np.zeros(n, np.uint8)
+        rc = _lib.lgo_move_eval_batch(self._h, *[x.ctypes.data for x in a], seed, first_id, n,
+                                      cost.ctypes.data, path.ctypes.data, mk.ctypes.data, fe.ctypes.data)
+        if rc: raise OracleError(rc)
+        return cost, path, mk, fe
+
+    def local_search(self, plan, seed, n_iters, n_workers, eps_thresh):
+        a = _plan_arrays(plan)
+        c = C.c_double(); hc = np.zeros(n_iters); hi = np.zeros(n_iters, np.uint64)
+        rc = _lib.lgo_local_search(self._h, *[x.ctypes.data for x in a], seed, n_iters, n_workers, eps_thresh,
+                                   C.byref(c), hc.ctypes.data, hi.ctypes.data)
+        if rc: raise OracleError(rc)
+        return dict(zip([k for k, _ in PLAN_KEYS], a)), c.value, hc, hi

@@ -1,0 +1,138 @@
+"""Pins for the NEXT rows: Algorithm 1's nearest-neighbour initialisation
+(PAPER.md:L122-126, L171-173), the remove/reinsert move (L158, L184) and the iteration with the
+exploration rule eq. (5) (L136-169, L177)."""
+import numpy as np
+import pytest
+from oracle import lgo
+from paper_1909_10286_b200 import workloads as wl
+from helpers import mk_instance
+
+
+def hand_instance():
+    # HQ (0,0); BPs B0 (10,0), B1 (0,20), B2 (30,0): chain HQ -> B0 (10) -> B2 (20 < 22.4) -> B1
+    fields = [(11, 1, 30, 1), (9, -1, 30, 1), (29, 2, 40, 1), (1, 19, 10, 1), (12, 0, 5, 1), (2, 21, 50, 1)]
+    bps = [(10, 0, 50), (0, 20, 40), (30, 0, 40)]
+    return mk_instance((0, 0), fields, bps, [2.0, 2.0, 2.0], [20, 10, 10, 20], 2)
+
+
+def test_init_plan_hand_example():
+    """Worked by hand: BP chain B0,B2,B1 cut into [B0] | [B2,B1]; fields in index order to the
+    closest BP still short of its demand (F4 goes to the far B1 because B0 and B2 are already
+    supplied); per-BP order by nearest neighbour starting at HQ; HUs 1 + residual 2; SUs dealt
+    round-robin over the capacity order."""
+    o = lgo.Oracle(hand_instance())
+    p = o.init_plan()
+    assert list(p["bp_tour"]) == [0, 1, 1] and list(p["bp_pos"]) == [0, 1, 0]
+    assert list(p["field_bp"]) == [0, 0, 2, 1, 1, 1]
+    assert list(p["field_pos"]) == [1, 0, 0, 1, 0, 2]         # B0: F1,F0;  B1: F4,F3,F5;  B2: F2
+    assert list(p["hu_tour"]) == [0, 1, 1]
+    assert list(p["su_tour"]) == [0, 0, 1, 1]                  # capacity order u1,u2,u0,u3 -> tours 0,1,0,1
+    r = o.score(p)
+    assert r["feasible"] and list(r["bp_supply_q"]) == [60 * 1024, 65 * 1024, 40 * 1024]
+
+
+@pytest.mark.parametrize("name", ["toy", "small", "medium", "paper_scale"])
+def test_init_plan_invariants(name):
+    inst = wl.make(name); o = lgo.Oracle(inst)
+    p = o.init_plan()
+    nt = o.n_t
+    # every tour gets floor/ceil(N_B/N_T) BPs with contiguous positions; unit counts per the rules
+    cnt = np.bincount(p["bp_tour"], minlength=nt)
+    assert cnt.min() >= o.n_b // nt and cnt.max() <= -(-o.n_b // nt)
+    for g in range(nt):
+        assert sorted(p["bp_pos"][p["bp_tour"] == g]) == list(range(cnt[g]))
+    hu = np.bincount(p["hu_tour"], minlength=nt)
+    assert list(hu[:-1]) == [o.n_hu // nt] * (nt - 1) and hu.sum() == o.n_hu
+    su = np.bincount(p["su_tour"], minlength=nt)
+    assert su.max() - su.min() <= 1
+    for b in range(o.n_b):
+        assert sorted(p["field_pos"][p["field_bp"] == b]) == list(range(int((p["field_bp"] == b).sum())))
+    # the greedy fill supplies every BP when supply is ample (the paper's setting: 6000 ha of fields
+    # for 5000 ha of demand, L267); the tight 11-field toy is the exception
+    r = o.score(p)
+    assert r["feasible"] == (name != "toy")
+    # step 3: within a BP each next field is the nearest remaining one
+    nb = o.n_b
+    for b in range(min(nb, 3)):
+        fs = [int(f) for f in np.argsort(p["field_pos"] + 100000 * (p["field_bp"] != b))[: int((p["field_bp"] == b).sum())]]
+        cur = 0
+        for k, f in enumerate(fs):
+            d = o.distance(cur, 1 + nb + f)
+            assert all(d <= o.distance(cur, 1 + nb + g) for g in fs[k:])
+            cur = 1 + nb + f
+
+
+def w_for(v, n):
+    """smallest 32-bit draw with below(w, n) == v"""
+    return -(-(v << 32) // n)
+
+
+def test_moves_hand_examples():
+    o = lgo.Oracle(hand_instance()); p = o.init_plan()
+    nf, nb, nt = 6, 3, 2
+    # field F4 (vertex 4) from B1 [F4,F3,F5] to B0 [F1,F0] at position 1 -> B0 [F1,F4,F0], B1 [F3,F5]
+    q = o.apply_move(p, w_for(4, nf + nb), w_for(0, nb), w_for(1, 3))
+    assert list(q["field_bp"]) == [0, 0, 2, 1, 0, 1] and list(q["field_pos"]) == [2, 0, 0, 0, 1, 1]
+    assert list(q["bp_tour"]) == list(p["bp_tour"]) and list(q["bp_pos"]) == list(p["bp_pos"])
+    # a field reinserted into its own BP: B1 [F4,F3,F5], F3 removed -> [F4,F5], position 2 -> [F4,F5,F3]
+    q = o.apply_move(p, w_for(3, nf + nb), w_for(1, nb), w_for(2, 3))
+    assert list(q["field_pos"]) == [1, 0, 0, 2, 0, 1]
+    # BP B1 (vertex 6+1) from tour 1 [B2,B1] to tour 0 [B0] at position 0 -> tour 0 [B1,B0], tour 1 [B2];
+    # its fields stay attached (L184)
+    q = o.apply_move(p, w_for(nf + 1, nf + nb), w_for(0, nt), w_for(0, 2))
+    assert list(q["bp_tour"]) == [0, 0, 1] and list(q["bp_pos"]) == [1, 0, 0]
+    assert list(q["field_bp"]) == list(p["field_bp"]) and list(q["field_pos"]) == list(p["field_pos"])
+    # the only BP of a tour may leave it: the tour becomes inactive (L184) and costs nothing
+    q = o.apply_move(p, w_for(nf + 0, nf + nb), w_for(1, nt), w_for(2, 3))
+    assert list(q["bp_tour"]) == [1, 1, 1] and list(q["bp_pos"]) == [2, 1, 0]
+    r = o.score(q)
+    assert r["route"][0] == 0.0 and r["T"][0] == 0.0 and r["feasible"]
+
+
+def test_moves_keep_plans_valid_and_are_uniform():
+    inst = wl.make("small"); o = lgo.Oracle(inst); p = o.init_plan()
+    rng = np.random.default_rng(5)
+    moved = np.zeros(o.n_f + o.n_b, int)
+    for _ in range(3000):
+        w = rng.integers(0, 2**32, 3)
+        q = o.apply_move(p, int(w[0]), int(w[1]), int(w[2]))
+        v = (int(w[0]) * (o.n_f + o.n_b)) >> 32
+        moved[v] += 1
+        for b in range(o.n_b):
+            assert sorted(q["field_pos"][q["field_bp"] == b]) == list(range(int((q["field_bp"] == b).sum())))
+        for g in range(o.n_t):
+            assert sorted(q["bp_pos"][q["bp_tour"] == g]) == list(range(int((q["bp_tour"] == g).sum())))
+        if v < o.n_f:   # only field v may change BP
+            assert np.array_equal(np.delete(q["field_bp"], v), np.delete(p["field_bp"], v))
+        else:
+            assert np.array_equal(q["field_bp"], p["field_bp"]) and np.array_equal(q["field_pos"], p["field_pos"])
+    exp = 3000 / (o.n_f + o.n_b)
+    assert ((moved - exp) ** 2 / exp).sum() < 95.0      # chi-square, 44 dof, p ~ 1e-5
+
+
+def test_move_eval_batch_is_move_then_score():
+    inst = wl.make("small"); o = lgo.Oracle(inst); p = o.init_plan()
+    cost, path, mk, fe = o.move_eval_batch(p, 7, 100, 64)
+    for i in (0, 13, 63):
+        blk = lgo.philox4x32_10([100 + i, 0, 5, 0], [7, 0])
+        r = o.score(o.apply_move(p, int(blk[0]), int(blk[1]), int(blk[2])))
+        assert r["feasible"] == bool(fe[i]) and (r["cost"] == cost[i] or (np.isinf(cost[i]) and np.isinf(r["cost"])))
+    assert 0 < fe.mean() <= 1
+
+
+@pytest.mark.parametrize("eps", [0, 0x80000000, 0xFFFFFFFF])
+def test_local_search_improves_and_is_consistent(eps):
+    inst = wl.make("small"); o = lgo.Oracle(inst); p0 = o.init_plan()
+    c0 = o.score(p0)["cost"]
+    best, c, hc, hi = o.local_search(p0, 3, 60, 256, eps)
+    fin = hc[np.isfinite(hc)]
+    assert c == min(c0, fin.min()) and c < c0                  # the nearest-neighbour start is improved
+    r = o.score(best)
+    assert r["cost"] == c and r["moves"] == 0                   # x* carries Alg. 2's SU assignment (R37)
+    assert np.all(hi // 256 == np.arange(60))                   # the winner of iteration k is one of its workers
+    # replaying iteration 0 from x_0 gives the recorded winner
+    p0s = dict(p0); p0s["su_tour"] = o.score(p0)["su_tour_final"]
+    cost, _, _, _ = o.move_eval_batch(p0s, 3, 0, 256)
+    assert cost.min() == hc[0] and int(np.argmin(cost)) == int(hi[0])
+    best2, c2, hc2, hi2 = o.local_search(p0, 3, 60, 256, eps)
+    assert c2 == c and np.array_equal(hc2, hc) and np.array_equal(hi2, hi)   # deterministic
