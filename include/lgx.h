@@ -108,7 +108,8 @@ int lgx_decode_batch(const lgx_instance *inst, uint64_t seed,
  * bytes per block, 4 distance mode (0 = packed tables in smem, 1 = coordinates, 2 = field x BP table + coordinates),
  * 5 per-candidate state bytes of the decode/walk kernel, 6 SM count, 7 kernel launches issued
  * so far through this instance, 8 / 9 threads per block / shared memory bytes of the finish
- * kernel, 10 candidates per kernel pair (chunk), 11 bytes per queue record.                 */
+ * kernel, 10 candidates per kernel pair (chunk), 11 bytes per queue record, 15 / 16 threads per
+ * block / shared memory bytes of the move kernels (Algorithm 1 entry points below).         */
 int lgx_instance_query(const lgx_instance *inst, int what, int64_t *out);
 
 /* Per-kernel timing for bench.py's roofline: when enabled, every lgx_search(_range) call
@@ -117,6 +118,54 @@ int lgx_instance_query(const lgx_instance *inst, int what, int64_t *out);
  * decode/walk / finish kernels, 14 the number of kernel pairs timed.  Enabling or disabling
  * resets the counters.                                                                     */
 int lgx_instance_set_timing(lgx_instance *inst, int enable);
+
+/* ---- The paper's own search loop, Algorithm 1 -----------
+ * A plan x is six HOST arrays (the layouts of lgx_decode_batch, one row): h_bp_tour/h_bp_pos [N_B],
+ * h_field_bp/h_field_pos [N_F], h_hu_tour [N_HU], h_su_tour [N_SU].  A plan passed IN must be valid
+ * (every BP on one tour at a unique position 0..len-1, every field on one BP likewise, every tour with
+ * >= 1 HU and >= 1 SU; tours without BPs and BPs without fields are allowed, L184), else LGX_EINVAL.
+ * LGX_ETOOBIG when the move kernels' state does not fit in shared memory (what = 15 reports 0).
+ * Readings R31-R37 cover what the paper leaves open.                                 */
+
+/* Steps 1-3 (L122-126, L171-173): the nearest-neighbour initialisation "a human scheduler may tacitly
+ * conduct" (Case 1, L273).  HUs: floor(N_HU/N_T) per tour in index order, the residual on the last tour;
+ * SUs dealt round-robin over the (capacity, unit) order; BPs: nearest-neighbour chain from HQ cut into
+ * N_T consecutive runs; fields, in index order, to their closest BP still short of its demand, else to
+ * their closest BP; per BP a nearest-neighbour order from HQ.  Runs on the device (one block); writes
+ * the six host arrays; synchronises cuda_stream.                                                    */
+int lgx_init_plan(const lgx_instance *inst,
+                  uint8_t *h_bp_tour, uint8_t *h_bp_pos, uint16_t *h_field_bp, uint16_t *h_field_pos,
+                  uint8_t *h_hu_tour, uint8_t *h_su_tour, void *cuda_stream);
+
+/* Steps 8-12 for workers i = first_id .. first_id+n-1 (L158-165, L184): x_i = x with ONE vertex removed
+ * and reinserted, scored like lgx_eval_batch (eq. (2), Algorithm 2 starting from x's SU sets, cost).
+ * Worker i draws Philox block (seed; counter = (i, stream 5, block 0)) = (w0, w1, w2, -):
+ * v = floor(w0 (N_F+N_B) / 2^32) is a field (v < N_F) or BP v-N_F; a field goes to BP floor(w1 N_B / 2^32),
+ * a BP (with all its fields) to tour floor(w1 N_T / 2^32); position floor(w2 (len+1) / 2^32), len = the
+ * target list's length after the removal.  Outputs are DEVICE pointers (any may be NULL), row i-first_id.
+ * The plan is copied before the call returns; the kernel is asynchronous on cuda_stream.            */
+int lgx_move_eval_batch(const lgx_instance *inst,
+                        const uint8_t *h_bp_tour, const uint8_t *h_bp_pos,
+                        const uint16_t *h_field_bp, const uint16_t *h_field_pos,
+                        const uint8_t *h_hu_tour, const uint8_t *h_su_tour,
+                        uint64_t seed, uint64_t first_id, uint64_t n,
+                        double *d_cost, double *d_path_km, double *d_makespan_h, uint8_t *d_feasible,
+                        void *cuda_stream);
+
+/* Steps 4-16 (L133-169) with the exploration rule eq. (5) (L177), all n_iters iterations inside ONE
+ * persistent cooperative kernel.  x_0 comes in through the plan arrays (its SU sets are replaced by what
+ * Algorithm 2 leaves them with) and x* goes out through them; *h_best_cost = C*.  Iteration k starts from
+ * x* if word 0 of Philox block (seed; (k, stream 6, block 0)) < eps_thresh (= eps 2^32), else from the
+ * winner of iteration k-1; its workers are ids k n_workers .. (k+1) n_workers - 1 of lgx_move_eval_batch;
+ * i* = the ordered minimum of (cost bits, id).  If C_i* is finite x_old <- x_i* (with the SU sets
+ * Algorithm 2 gave it) and x* <- x_i* when C_i* < C*.  h_hist_cost / h_hist_id [n_iters] (may be NULL)
+ * receive (C_i*, i*) of every iteration.  HU sets stay as given (R20).  Synchronises cuda_stream.
+ * n_workers == 0 => LGX_EINVAL; n_iters == 0 scores x_0 only.                                        */
+int lgx_local_search(const lgx_instance *inst,
+                     uint8_t *h_bp_tour, uint8_t *h_bp_pos, uint16_t *h_field_bp, uint16_t *h_field_pos,
+                     uint8_t *h_hu_tour, uint8_t *h_su_tour,
+                     uint64_t seed, uint32_t n_iters, uint32_t n_workers, uint32_t eps_thresh,
+                     double *h_best_cost, double *h_hist_cost, uint64_t *h_hist_id, void *cuda_stream);
 
 const char *lgx_strerror(int code);
 

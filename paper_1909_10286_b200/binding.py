@@ -35,7 +35,7 @@ class lgx_instance_desc(C.Structure):
 
 EXPORTS = ("lgx_instance_create", "lgx_instance_destroy", "lgx_eval_batch", "lgx_eval_batch_host",
            "lgx_search_range", "lgx_search", "lgx_decode_batch", "lgx_instance_query", "lgx_instance_set_timing",
-           "lgx_strerror")
+           "lgx_init_plan", "lgx_move_eval_batch", "lgx_local_search", "lgx_strerror")
 
 _lib = None
 
@@ -60,6 +60,10 @@ def load(rebuild_if_stale: bool = True):
     lib.lgx_decode_batch.argtypes = [vp, u64, vp, u64, u64] + [vp] * 7 + [vp]
     lib.lgx_instance_query.argtypes = [vp, i32, C.POINTER(C.c_int64)]
     lib.lgx_instance_set_timing.argtypes = [vp, i32]
+    lib.lgx_init_plan.argtypes = [vp] + [vp] * 6 + [vp]
+    lib.lgx_move_eval_batch.argtypes = [vp] + [vp] * 6 + [u64, u64, u64, vp, vp, vp, vp, vp]
+    lib.lgx_local_search.argtypes = [vp] + [vp] * 6 + [u64, C.c_uint32, C.c_uint32, C.c_uint32,
+                                                      C.POINTER(C.c_double), vp, vp, vp]
     lib.lgx_strerror.argtypes = [i32]
     lib.lgx_strerror.restype = C.c_char_p
     for f in EXPORTS:
@@ -114,6 +118,15 @@ def make_desc(inst):
                           inst.su_fill_h_per_t, inst.w_path, inst.w_time,
                           inst.extra_field_thresh, inst.flags)
     return d, (fx, fy, bx, by, sup, area, dem, hu, su)
+
+
+PLAN_KEYS = (("bp_tour", np.uint8), ("bp_pos", np.uint8), ("field_bp", np.uint16), ("field_pos", np.uint16),
+             ("hu_tour", np.uint8), ("su_tour", np.uint8))
+
+
+def _plan_arrays(plan):
+    """The six host arrays of a plan (copies, contiguous, typed) in the C ABI's order."""
+    return [np.array(plan[k], dtype=dt, order="C", copy=True) for k, dt in PLAN_KEYS]
 
 
 class Instance:
@@ -201,3 +214,33 @@ class Instance:
                                           _ptr(o["hu_tour"]), _ptr(o["su_tour_init"]), _ptr(o["su_tour_final"]),
                                           _stream_ptr(stream)))
         return o
+
+    # -- Algorithm 1 (lgx_init_plan, lgx_move_eval_batch, lgx_local_search); plans are dicts of host arrays
+    def init_plan(self, stream=None):
+        a = [np.zeros(n, dt) for n, dt in ((self.n_b, np.uint8), (self.n_b, np.uint8), (self.n_f, np.uint16),
+                                           (self.n_f, np.uint16), (self.n_hu, np.uint8), (self.n_su, np.uint8))]
+        _check(self._lib.lgx_init_plan(self._h, *[x.ctypes.data for x in a], _stream_ptr(stream)))
+        return dict(zip([k for k, _ in PLAN_KEYS], a))
+
+    def move_eval_batch(self, plan, seed, first_id, n, out=None, stream=None):
+        import torch
+        a = _plan_arrays(plan)
+        dev = torch.device("cuda", torch.cuda.current_device())
+        if out is None:
+            out = (torch.empty(n, dtype=torch.float64, device=dev), torch.empty(n, dtype=torch.float64, device=dev),
+                   torch.empty(n, dtype=torch.float64, device=dev), torch.empty(n, dtype=torch.uint8, device=dev))
+        cost, path, mk, feas = out
+        _check(self._lib.lgx_move_eval_batch(self._h, *[x.ctypes.data for x in a], seed, first_id, n,
+                                             _ptr(cost), _ptr(path), _ptr(mk), _ptr(feas), _stream_ptr(stream)))
+        return out
+
+    def local_search(self, plan, seed, n_iters, n_workers, eps_thresh, history=True, stream=None):
+        """Returns (x*, C*, hist_cost, hist_id)."""
+        a = _plan_arrays(plan)
+        c = C.c_double()
+        hc = np.zeros(n_iters) if history else None
+        hi = np.zeros(n_iters, np.uint64) if history else None
+        _check(self._lib.lgx_local_search(self._h, *[x.ctypes.data for x in a], seed, n_iters, n_workers, eps_thresh,
+                                          C.byref(c), hc.ctypes.data if history else None,
+                                          hi.ctypes.data if history else None, _stream_ptr(stream)))
+        return dict(zip([k for k, _ in PLAN_KEYS], a)), c.value, hc, hi

@@ -11,7 +11,7 @@ CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "liblgx.so")
 SOURCES = [os.path.join(CSRC, "lgx_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "lgx_kernels.cuh"), os.path.join(CSRC, "lgx_image.h"),
+DEPS = SOURCES + [os.path.join(CSRC, "lgx_kernels.cuh"), os.path.join(CSRC, "lgx_moves.cuh"), os.path.join(CSRC, "lgx_image.h"),
                   os.path.join(ROOT, "include", "lgx.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

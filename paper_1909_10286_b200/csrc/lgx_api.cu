@@ -4,6 +4,7 @@
 #include "../../include/lgx.h"
 #include "lgx_image.h"
 #include "lgx_kernels.cuh"
+#include "lgx_moves.cuh"
 
 #include <algorithm>
 #include <atomic>
@@ -30,6 +31,10 @@ struct lgx_instance {
   // optional per-kernel timing (lgx_instance_set_timing): CUDA events around every launch of a search
   mutable std::atomic<int> timing{0};
   mutable std::atomic<long long> ns_a{0}, ns_c{0}, timed_pairs{0};
+  // move kernels (Algorithm 1: lgx_init_plan, lgx_move_eval_batch, lgx_local_search)
+  MvHdr mv{};
+  double2 *d_xy = nullptr;                     // vertex coordinates, every distance mode (lgx_init_plan)
+  int threads_mv = 0; size_t smem_mv = 0;
 };
 
 namespace {
@@ -336,6 +341,51 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
       (e = cudaMemcpy(I->d_image_c, imc, H.imagec_bytes, cudaMemcpyHostToDevice)) != cudaSuccess) {
     cudaFree(I->d_image); cudaFree(I->d_image_c); delete I; return cuda_fail(e, "cudaMemcpy(image)");
   }
+  // ---- move kernels: shared-memory layout (lgx_moves.cuh) and vertex coordinates for lgx_init_plan
+  {
+    MvHdr &M = I->mv;
+    uint32_t o = H.image_bytes;
+    M.off_c = o;     o = align16(o + (H.imagec_bytes - H.offc_s));
+    M.off_seq = o;   o = align16(o + 4u * (uint32_t)nf);
+    M.off_posf = o;  o = align16(o + 2u * (uint32_t)nf);
+    M.off_bp = o;    o = align16(o + 8u * (uint32_t)nb);
+    M.off_pre = o;   o = align16(o + 2u * ((uint32_t)nb + 1u));
+    M.off_bpat = o;  o = align16(o + (uint32_t)nb);
+    M.off_cnt = o;   o = align16(o + 4u * (uint32_t)nb);
+    M.off_tpl = o;   o = align16(o + 4u * (uint32_t)nt);
+    M.off_thu = o;   o = align16(o + 8u * (uint32_t)nt);
+    M.off_ts = o;    o = align16(o + 4u * (uint32_t)nt);
+    M.off_tmask = o; o = align16(o + 8u * (uint32_t)nt * MW);
+    M.off_misc = o;  o = align16(o + 64u);
+    uint32_t q = 0;
+    q += (uint32_t)nb; M.pl_bpos = q; q += (uint32_t)nb; q = (q + 1u) & ~1u;
+    M.pl_fbp = q; q += 2u * (uint32_t)nf; M.pl_fpos = q; q += 2u * (uint32_t)nf; q = (q + 7u) & ~7u;
+    M.pl_mask = q; q += 8u * (uint32_t)nt * MW;
+    M.plan_bytes = align16(q);
+    M.off_plans = o; o += 3u * M.plan_bytes;
+    M.off_state = o;
+    uint32_t r = 0;
+    M.m64_lt = r; r += (uint32_t)nt; M.m64_e = r; r += (uint32_t)nt; M.m64_w = r; r += (uint32_t)nt;
+    M.m64_mask = r; r += (uint32_t)nt * MW; M.m64_bmask = r; r += (uint32_t)nt * MW; M.m64_rows = r;
+    r = 0;
+    M.m32_hq = r; r += (uint32_t)nt; M.m32_s = r; r += (uint32_t)nt; M.m32_ng = r; r += (uint32_t)nt;
+    M.m32_magic = r; r += (uint32_t)nt; M.m32_rows = r;
+    M.slot_words = 2u + (uint32_t)nt * MW;
+    const int64_t mv_state = 8ll * M.m64_rows + 4ll * M.m32_rows;
+    int64_t tm = (budget - 256 - (int64_t)M.off_state) / mv_state;      // static smem of the reductions
+    tm = std::min<int64_t>(tm, kMvThreads) / 32 * 32;
+    if (const char *ev = std::getenv("LGX_THREADS_MV")) { const int v = std::atoi(ev); if (v >= 64 && v <= tm) tm = v / 32 * 32; }
+    I->threads_mv = tm >= 64 ? (int)tm : 0;                               // 0: the move kernels do not fit (LGX_ETOOBIG there)
+    I->smem_mv = (size_t)M.off_state + (size_t)mv_state * (size_t)std::max<int64_t>(tm, 0);
+    std::vector<double> xy(2 * (size_t)(1 + nb + nf));
+    xy[0] = d->hq_x; xy[1] = d->hq_y;
+    for (int b = 0; b < nb; ++b) { xy[2 * (1 + b)] = d->bp_x[b]; xy[2 * (1 + b) + 1] = d->bp_y[b]; }
+    for (int f = 0; f < nf; ++f) { xy[2 * (1 + nb + f)] = d->field_x[f]; xy[2 * (1 + nb + f) + 1] = d->field_y[f]; }
+    if ((e = cudaMalloc((void **)&I->d_xy, xy.size() * 8)) != cudaSuccess ||
+        (e = cudaMemcpy(I->d_xy, xy.data(), xy.size() * 8, cudaMemcpyHostToDevice)) != cudaSuccess) {
+      cudaFree(I->d_image); cudaFree(I->d_image_c); cudaFree(I->d_xy); delete I; return cuda_fail(e, "cudaMalloc/cudaMemcpy(xy)");
+    }
+  }
   *out = I;
   return LGX_OK;
 }
@@ -343,6 +393,7 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
 int lgx_instance_destroy(lgx_instance *I)
 {
   if (!I) return LGX_EINVAL;
+  if (I->d_xy) cudaFree(I->d_xy);
   if (I->d_image) cudaFree(I->d_image);
   if (I->d_image_c) cudaFree(I->d_image_c);
   delete I;
@@ -432,6 +483,8 @@ int lgx_instance_query(const lgx_instance *I, int what, int64_t *out)
     case 12: *out = I->ns_a.load(); break;
     case 13: *out = I->ns_c.load(); break;
     case 14: *out = I->timed_pairs.load(); break;
+    case 15: *out = I->threads_mv; break;
+    case 16: *out = (int64_t)I->smem_mv; break;
     default: return LGX_EINVAL;
   }
   return LGX_OK;
@@ -558,6 +611,226 @@ int lgx_eval_batch_host(const lgx_instance *I, uint64_t seed, const uint64_t *h_
     if ((e = cudaStreamSynchronize(0)) != cudaSuccess) { rc = cuda_fail(e, "cudaStreamSynchronize"); break; }
   }
   cleanup();
+  return rc;
+}
+
+}  // extern "C"
+
+// ================================================================== Algorithm 1
+
+namespace {
+
+using MvKernelFn = void (*)(const MvParams);
+
+void pick_move_kernels(const ImgHdr &h, MvKernelFn &kb, MvKernelFn &ks)
+{
+  const int dm = h.coords, mw = (int)h.mask_words;
+  kb = ks = nullptr;
+#define LGX_PICK(D, M) if (dm == D && mw == M) { kb = lgx_move_eval_k<D, M>; ks = lgx_local_search_k<D, M>; }
+  LGX_PICK(0, 1) LGX_PICK(0, 2) LGX_PICK(1, 1) LGX_PICK(1, 2) LGX_PICK(2, 1) LGX_PICK(2, 2)
+#undef LGX_PICK
+}
+
+// A plan is valid when every BP sits on exactly one tour at a unique position 0..len-1, every field on exactly
+// one BP likewise, and every tour has at least one HU and one SU (L69).
+bool plan_valid(const ImgHdr &H, const uint8_t *bt, const uint8_t *bq, const uint16_t *fb, const uint16_t *fq,
+                const uint8_t *hu, const uint8_t *su)
+{
+  const int nt = H.n_t, nb = H.n_b, nf = H.n_f;
+  std::vector<int> tlen(nt, 0), blen(nb, 0), nhu(nt, 0), nsu(nt, 0);
+  for (int b = 0; b < nb; ++b) { if (bt[b] >= nt) return false; ++tlen[bt[b]]; }
+  for (int f = 0; f < nf; ++f) { if (fb[f] >= nb) return false; ++blen[fb[f]]; }
+  std::vector<int> toff(nt + 1, 0), boff(nb + 1, 0);
+  for (int g = 0; g < nt; ++g) toff[g + 1] = toff[g] + tlen[g];
+  for (int b = 0; b < nb; ++b) boff[b + 1] = boff[b] + blen[b];
+  std::vector<char> seen_b(nb, 0), seen_f(nf, 0);
+  for (int b = 0; b < nb; ++b) { if (bq[b] >= tlen[bt[b]]) return false; char &c = seen_b[toff[bt[b]] + bq[b]]; if (c) return false; c = 1; }
+  for (int f = 0; f < nf; ++f) { if (fq[f] >= blen[fb[f]]) return false; char &c = seen_f[boff[fb[f]] + fq[f]]; if (c) return false; c = 1; }
+  for (int u = 0; u < H.n_hu; ++u) { if (hu[u] >= nt) return false; ++nhu[hu[u]]; }
+  for (int u = 0; u < H.n_su; ++u) { if (su[u] >= nt) return false; ++nsu[su[u]]; }
+  for (int g = 0; g < nt; ++g) if (nhu[g] < 1 || nsu[g] < 1) return false;
+  return true;
+}
+
+struct PlanDev {
+  uint8_t *base = nullptr;
+  uint8_t *bt, *bq, *hu, *su; uint16_t *fb, *fq;
+  size_t bytes = 0;
+};
+
+int plan_dev_alloc(const ImgHdr &H, cudaStream_t st, PlanDev &D)
+{
+  const size_t nb = H.n_b, nf = H.n_f, nhu = H.n_hu, nsu = H.n_su;
+  size_t o = 0;
+  const size_t o_fb = o; o += 2 * nf; const size_t o_fq = o; o += 2 * nf;
+  const size_t o_bt = o; o += nb; const size_t o_bq = o; o += nb; const size_t o_hu = o; o += nhu; const size_t o_su = o; o += nsu;
+  D.bytes = o;
+  CU(cudaMallocAsync((void **)&D.base, o, st));
+  D.fb = reinterpret_cast<uint16_t *>(D.base + o_fb); D.fq = reinterpret_cast<uint16_t *>(D.base + o_fq);
+  D.bt = D.base + o_bt; D.bq = D.base + o_bq; D.hu = D.base + o_hu; D.su = D.base + o_su;
+  return LGX_OK;
+}
+
+int plan_upload(const ImgHdr &H, const PlanDev &D, const uint8_t *bt, const uint8_t *bq, const uint16_t *fb, const uint16_t *fq,
+                const uint8_t *hu, const uint8_t *su, cudaStream_t st)
+{
+  CU(cudaMemcpyAsync(D.bt, bt, (size_t)H.n_b, cudaMemcpyHostToDevice, st));
+  CU(cudaMemcpyAsync(D.bq, bq, (size_t)H.n_b, cudaMemcpyHostToDevice, st));
+  CU(cudaMemcpyAsync(D.fb, fb, 2 * (size_t)H.n_f, cudaMemcpyHostToDevice, st));
+  CU(cudaMemcpyAsync(D.fq, fq, 2 * (size_t)H.n_f, cudaMemcpyHostToDevice, st));
+  CU(cudaMemcpyAsync(D.hu, hu, (size_t)H.n_hu, cudaMemcpyHostToDevice, st));
+  CU(cudaMemcpyAsync(D.su, su, (size_t)H.n_su, cudaMemcpyHostToDevice, st));
+  return LGX_OK;
+}
+
+int plan_download(const ImgHdr &H, const PlanDev &D, uint8_t *bt, uint8_t *bq, uint16_t *fb, uint16_t *fq, uint8_t *hu, uint8_t *su,
+                  cudaStream_t st)
+{
+  CU(cudaMemcpyAsync(bt, D.bt, (size_t)H.n_b, cudaMemcpyDeviceToHost, st));
+  CU(cudaMemcpyAsync(bq, D.bq, (size_t)H.n_b, cudaMemcpyDeviceToHost, st));
+  CU(cudaMemcpyAsync(fb, D.fb, 2 * (size_t)H.n_f, cudaMemcpyDeviceToHost, st));
+  CU(cudaMemcpyAsync(fq, D.fq, 2 * (size_t)H.n_f, cudaMemcpyDeviceToHost, st));
+  CU(cudaMemcpyAsync(hu, D.hu, (size_t)H.n_hu, cudaMemcpyDeviceToHost, st));
+  CU(cudaMemcpyAsync(su, D.su, (size_t)H.n_su, cudaMemcpyDeviceToHost, st));
+  return LGX_OK;
+}
+
+void mv_fill(const lgx_instance *I, MvParams &P, uint64_t seed, const PlanDev &D)
+{
+  P.H = I->hdr; P.M = I->mv; P.image = I->d_image; P.image_c = I->d_image_c;
+  uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+  for (int r = 0; r < 10; ++r) { P.rk[2 * r] = k0; P.rk[2 * r + 1] = k1; k0 += kPhiloxW0; k1 += kPhiloxW1; }
+  P.bp_tour = D.bt; P.bp_pos = D.bq; P.field_bp = D.fb; P.field_pos = D.fq; P.hu_tour = D.hu; P.su_tour = D.su;
+}
+
+}  // namespace
+
+extern "C" {
+
+int lgx_init_plan(const lgx_instance *I, uint8_t *h_bp_tour, uint8_t *h_bp_pos, uint16_t *h_field_bp, uint16_t *h_field_pos,
+                  uint8_t *h_hu_tour, uint8_t *h_su_tour, void *stream)
+{
+  if (!I || !h_bp_tour || !h_bp_pos || !h_field_bp || !h_field_pos || !h_hu_tour || !h_su_tour) return LGX_EINVAL;
+  cudaStream_t st = (cudaStream_t)stream;
+  const ImgHdr &H = I->hdr;
+  PlanDev D;
+  int rc = plan_dev_alloc(H, st, D);
+  if (rc != LGX_OK) return rc;
+  const size_t nb = H.n_b, nf = H.n_f;
+  const size_t scratch_bytes = 4 * (3 * nb + 1) + 2 * (nf + (nf & 1)) + 2 * nb + 16;
+  uint32_t *scratch = nullptr;
+  cudaError_t e = cudaMallocAsync((void **)&scratch, scratch_bytes, st);
+  if (e != cudaSuccess) { cudaFreeAsync(D.base, st); return cuda_fail(e, "cudaMallocAsync(init scratch)"); }
+  InitParams P{};
+  P.n_f = H.n_f; P.n_b = H.n_b; P.n_t = H.n_t; P.n_hu = H.n_hu; P.n_su = H.n_su;
+  P.xy = I->d_xy;
+  P.sq = reinterpret_cast<const uint32_t *>(I->d_image_c + H.offc_s);
+  P.dq = reinterpret_cast<const uint32_t *>(I->d_image + H.off_dq);
+  P.unit_of = I->d_image_c + H.offc_unit;
+  P.bp_tour = D.bt; P.bp_pos = D.bq; P.field_bp = D.fb; P.field_pos = D.fq; P.hu_tour = D.hu; P.su_tour = D.su;
+  P.scratch = scratch;
+  lgx_init_plan_k<<<1, 256, 0, st>>>(P);
+  I->launches.fetch_add(1);
+  e = cudaGetLastError();
+  if (e == cudaSuccess) rc = plan_download(H, D, h_bp_tour, h_bp_pos, h_field_bp, h_field_pos, h_hu_tour, h_su_tour, st);
+  if (e == cudaSuccess && rc == LGX_OK) e = cudaStreamSynchronize(st);
+  cudaFreeAsync(scratch, st); cudaFreeAsync(D.base, st);
+  if (e != cudaSuccess) return cuda_fail(e, "lgx_init_plan");
+  return rc;
+}
+
+int lgx_move_eval_batch(const lgx_instance *I,
+                        const uint8_t *h_bp_tour, const uint8_t *h_bp_pos, const uint16_t *h_field_bp, const uint16_t *h_field_pos,
+                        const uint8_t *h_hu_tour, const uint8_t *h_su_tour,
+                        uint64_t seed, uint64_t first_id, uint64_t n,
+                        double *d_cost, double *d_path_km, double *d_makespan_h, uint8_t *d_feasible, void *stream)
+{
+  if (!I || !h_bp_tour || !h_bp_pos || !h_field_bp || !h_field_pos || !h_hu_tour || !h_su_tour) return LGX_EINVAL;
+  const ImgHdr &H = I->hdr;
+  if (!plan_valid(H, h_bp_tour, h_bp_pos, h_field_bp, h_field_pos, h_hu_tour, h_su_tour)) return LGX_EINVAL;
+  if (I->threads_mv < 64) return LGX_ETOOBIG;
+  if (n == 0) return LGX_OK;
+  cudaStream_t st = (cudaStream_t)stream;
+  MvKernelFn kb, ks; pick_move_kernels(H, kb, ks);
+  if (!kb) return LGX_EINVAL;
+  PlanDev D;
+  int rc = plan_dev_alloc(H, st, D);
+  if (rc != LGX_OK) return rc;
+  rc = plan_upload(H, D, h_bp_tour, h_bp_pos, h_field_bp, h_field_pos, h_hu_tour, h_su_tour, st);
+  if (rc == LGX_OK) {
+    MvParams P{};
+    mv_fill(I, P, seed, D);
+    P.first_id = first_id; P.n = n;
+    P.cost = d_cost; P.path_km = d_path_km; P.makespan_h = d_makespan_h; P.feasible = d_feasible;
+    cudaError_t e = cudaFuncSetAttribute((const void *)kb, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)I->smem_mv);
+    if (e == cudaSuccess) {
+      const uint64_t blocks = (n + (uint64_t)I->threads_mv - 1) / (uint64_t)I->threads_mv;
+      const unsigned grid = (unsigned)std::min<uint64_t>((uint64_t)I->grid, blocks);
+      void *args[] = { (void *)&P };
+      e = cudaLaunchKernel((const void *)kb, dim3(grid), dim3((unsigned)I->threads_mv), args, I->smem_mv, st);
+      I->launches.fetch_add(1);
+    }
+    if (e != cudaSuccess) rc = cuda_fail(e, "lgx_move_eval_batch: launch");
+  }
+  cudaFreeAsync(D.base, st);
+  return rc;
+}
+
+int lgx_local_search(const lgx_instance *I,
+                     uint8_t *h_bp_tour, uint8_t *h_bp_pos, uint16_t *h_field_bp, uint16_t *h_field_pos,
+                     uint8_t *h_hu_tour, uint8_t *h_su_tour,
+                     uint64_t seed, uint32_t n_iters, uint32_t n_workers, uint32_t eps_thresh,
+                     double *h_best_cost, double *h_hist_cost, uint64_t *h_hist_id, void *stream)
+{
+  if (!I || !h_bp_tour || !h_bp_pos || !h_field_bp || !h_field_pos || !h_hu_tour || !h_su_tour || !h_best_cost) return LGX_EINVAL;
+  if (n_workers == 0) return LGX_EINVAL;
+  const ImgHdr &H = I->hdr;
+  if (!plan_valid(H, h_bp_tour, h_bp_pos, h_field_bp, h_field_pos, h_hu_tour, h_su_tour)) return LGX_EINVAL;
+  if (I->threads_mv < 64) return LGX_ETOOBIG;
+  cudaStream_t st = (cudaStream_t)stream;
+  MvKernelFn kb, ks; pick_move_kernels(H, kb, ks);
+  if (!ks) return LGX_EINVAL;
+  int coop = 0;
+  cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, I->device);
+  if (!coop) { g_cuda_msg = "device does not support cooperative launches"; return LGX_ECUDA; }
+  CU(cudaFuncSetAttribute((const void *)ks, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)I->smem_mv));
+  int per_sm = 0;
+  CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void *)ks, I->threads_mv, I->smem_mv));
+  if (per_sm < 1) return LGX_ETOOBIG;
+  // one block per SM, fewer when the workers of an iteration do not fill them
+  const uint64_t blocks = ((uint64_t)n_workers + (uint64_t)I->threads_mv - 1) / (uint64_t)I->threads_mv;
+  const unsigned grid = (unsigned)std::min<uint64_t>((uint64_t)I->sm_count, blocks);
+  PlanDev D;
+  int rc = plan_dev_alloc(H, st, D);
+  if (rc != LGX_OK) return rc;
+  uint8_t *ws = nullptr;
+  const size_t slots_bytes = 2ull * grid * I->mv.slot_words * 8ull;
+  const size_t hist_bytes = (size_t)n_iters * 8ull;
+  const size_t ws_bytes = slots_bytes + 2 * hist_bytes + 16;
+  cudaError_t e = cudaMallocAsync((void **)&ws, ws_bytes, st);
+  if (e != cudaSuccess) { cudaFreeAsync(D.base, st); return cuda_fail(e, "cudaMallocAsync(search workspace)"); }
+  rc = plan_upload(H, D, h_bp_tour, h_bp_pos, h_field_bp, h_field_pos, h_hu_tour, h_su_tour, st);
+  double best = 0.0;
+  if (rc == LGX_OK) {
+    MvParams P{};
+    mv_fill(I, P, seed, D);
+    P.n_iters = n_iters; P.n_workers = n_workers; P.eps_thresh = eps_thresh;
+    P.slots = reinterpret_cast<unsigned long long *>(ws);
+    P.hist_cost = reinterpret_cast<double *>(ws + slots_bytes);
+    P.hist_id = reinterpret_cast<unsigned long long *>(ws + slots_bytes + hist_bytes);
+    P.best_cost = reinterpret_cast<double *>(ws + slots_bytes + 2 * hist_bytes);
+    void *args[] = { (void *)&P };
+    e = cudaLaunchCooperativeKernel((const void *)ks, dim3(grid), dim3((unsigned)I->threads_mv), args, I->smem_mv, st);
+    I->launches.fetch_add(1);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&best, P.best_cost, 8, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && h_hist_cost && n_iters) e = cudaMemcpyAsync(h_hist_cost, P.hist_cost, hist_bytes, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && h_hist_id && n_iters) e = cudaMemcpyAsync(h_hist_id, P.hist_id, hist_bytes, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) rc = plan_download(H, D, h_bp_tour, h_bp_pos, h_field_bp, h_field_pos, h_hu_tour, h_su_tour, st);
+    if (e == cudaSuccess && rc == LGX_OK) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) rc = cuda_fail(e, "lgx_local_search");
+  }
+  cudaFreeAsync(ws, st); cudaFreeAsync(D.base, st);
+  if (rc == LGX_OK) *h_best_cost = best;
   return rc;
 }
 

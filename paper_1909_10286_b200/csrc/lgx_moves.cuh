@@ -1,0 +1,742 @@
+// lgx_moves.cuh — the paper's own search loop as CUDA for sm_100a:
+//   lgx_init_plan_k      Algorithm 1 steps 1-3: nearest-neighbour initialisation
+//   lgx_move_eval_k      step 8 + cost for a batch of workers (L158-165, L184): every worker applies ONE
+//                        remove/reinsert move to the broadcast incumbent x and scores the result
+//   lgx_local_search_k   steps 4-16 (L133-169) with the exploration rule eq. (5) (L177): ONE persistent
+//                        cooperative kernel runs all N_iters iterations; nothing returns to the host in between
+// Product code (CUDA path); shares nothing with oracle/.
+//
+// Design (B200-first, not the paper's host loop).  The paper broadcasts x, collects every C_i on the host,
+// takes the argmin there and rebuilds x_{i*} by replaying the random stream (L163-169, L233).  Here the
+// incumbent lives in the shared memory of every SM as a FLAT SEQUENCE: the fields in plan order (tour 0's
+// first BP's fields, ...), each entry carrying its BP.  A move (one field, or one BP with all its fields,
+// L184) is a rotation of one block of that sequence, so a worker never materialises x_i: it walks positions
+// s = 0..N_F-1 and maps s to an index of the incumbent's sequence with a handful of integer operations.
+// All workers of a warp therefore read (nearly) the same shared-memory words — broadcast, conflict-free —
+// and hit the BP / tour boundaries at (nearly) the same step, unlike the independently sampled plans of
+// lgx_decode_walk.  After the block/grid reduction of (cost bits, id) every block rebuilds x_{i*} ITSELF
+// from the winning id ("identical random process control", L233, taken one step further): the only
+// inter-SM traffic per iteration is one slot of (cost, id, SU sets) per block and one grid barrier.
+//
+// FP64 arithmetic follows DESIGN.md S4-S7 operation by operation (compiled with -fmad=false), in the
+// oracle's summation order, so costs are bit-equal.
+#pragma once
+#include <cooperative_groups.h>
+#include "lgx_kernels.cuh"
+
+namespace lgx {
+namespace cg = cooperative_groups;
+
+constexpr int      kMvThreads = 512;            // __launch_bounds__ of the move kernels
+constexpr uint32_t kNone      = 0xFFFFFFFFu;
+
+// Shared-memory layout of the move kernels (byte offsets from the start of dynamic shared memory):
+//   image AB | tail of image C (from offc_s) | incumbent tables | plan store | per-thread state rows
+struct MvHdr {
+  uint32_t off_c;       // tail of image C: byte x of image C (x >= offc_s) sits at off_c + x - offc_s
+  uint32_t off_seq;     // u32 [n_f]      f | b << 16 in plan order
+  uint32_t off_posf;    // u16 [n_f]      position of field f in seq
+  uint32_t off_bp;      // u32x2 [n_b]    x = start | len << 16;  y = plan index | tour << 8 | pos << 16
+  uint32_t off_pre;     // u16 [n_b + 1]  start of the BP at plan index j; pre[n_b] = n_f
+  uint32_t off_bpat;    // u8 [n_b]       BP at plan index j
+  uint32_t off_cnt;     // u32 [n_b]      scratch: fields per BP
+  uint32_t off_tpl;     // u32 [n_t]      first plan index | BPs on the tour << 8
+  uint32_t off_thu;     // u32x2 [n_t]    n_HU(g), R_g (fixed during a search: R20)
+  uint32_t off_ts;      // u32 [n_t]      S_g = capacity quanta of the tour's SUs
+  uint32_t off_tmask;   // u64 [n_t*MW]   SU membership by capacity rank
+  uint32_t off_misc;    // u32 [16]       [0] empty BPs with positive demand; [4..9] the move being applied
+  uint32_t off_plans;   // 3 plans (x*, x_old, scratch); the batch kernel uses the first
+  uint32_t plan_bytes;  // one plan: bp_tour u8[n_b] | bp_pos u8[n_b] | field_bp u16[n_f] | field_pos u16[n_f] | masks u64[n_t*MW]
+  uint32_t pl_bpos, pl_fbp, pl_fpos, pl_mask;
+  uint32_t off_state;   // per-thread rows (64-bit region, then 32-bit region)
+  uint32_t m64_lt, m64_e, m64_w, m64_mask, m64_bmask, m64_rows;
+  uint32_t m32_hq, m32_s, m32_ng, m32_magic, m32_rows;
+  uint32_t slot_words;  // 64-bit words per block slot: cost bits, id, masks
+  uint32_t pad_[2];
+};
+
+struct MvParams {
+  ImgHdr          H;
+  MvHdr           M;
+  const uint8_t  *image, *image_c;
+  uint32_t        rk[20];               // Philox round keys of the seed
+  // the plan x (device arrays; in for the batch kernel, in/out for the search)
+  uint8_t *bp_tour, *bp_pos; uint16_t *field_bp, *field_pos; uint8_t *hu_tour, *su_tour;
+  // batch: workers first_id .. first_id + n - 1
+  uint64_t first_id, n;
+  double *cost, *path_km, *makespan_h; uint8_t *feasible;
+  // search
+  uint32_t n_iters, n_workers, eps_thresh;
+  unsigned long long *slots;            // [2][gridDim.x][slot_words]
+  double *hist_cost; unsigned long long *hist_id;   // [n_iters] or nullptr
+  double *best_cost;
+};
+
+#define MV_TAB(type, off) (reinterpret_cast<type *>(sm + (off)))
+#define MV_CTAB(type, offc) (reinterpret_cast<const type *>(sm + (P.M.off_c + ((offc) - P.H.offc_s))))
+
+// ------------------------------------------------------------------ plan -> shared memory
+
+// Copy the plan arrays from global memory into a plan slot; SU sets become masks over capacity ranks.
+// Also fills the per-tour HU table (n_HU(g), R_g = sum of rate quanta, L69; R7).
+template <int MASKW>
+__device__ void mv_load_plan(const MvParams &P, uint8_t *sm, uint8_t *plan, uint32_t tid, uint32_t T)
+{
+  const ImgHdr &H = P.H; const MvHdr &M = P.M;
+  const uint32_t n_f = H.n_f, n_b = H.n_b, n_t = H.n_t;
+  for (uint32_t b = tid; b < n_b; b += T) { plan[b] = P.bp_tour[b]; plan[M.pl_bpos + b] = P.bp_pos[b]; }
+  uint16_t *fb = reinterpret_cast<uint16_t *>(plan + M.pl_fbp), *fp = reinterpret_cast<uint16_t *>(plan + M.pl_fpos);
+  for (uint32_t f = tid; f < n_f; f += T) { fb[f] = P.field_bp[f]; fp[f] = P.field_pos[f]; }
+  if (tid == 0) {
+    uint64_t *mk = reinterpret_cast<uint64_t *>(plan + M.pl_mask);
+    const uint8_t *rank_of = MV_CTAB(uint8_t, H.offc_rank);
+    const uint32_t *rq = MV_CTAB(uint32_t, H.offc_rq);
+    uint2 *thu = MV_TAB(uint2, M.off_thu);
+    for (uint32_t i = 0; i < n_t * MASKW; ++i) mk[i] = 0ull;
+    for (uint32_t g = 0; g < n_t; ++g) thu[g] = make_uint2(0u, 0u);
+    for (uint32_t u = 0; u < (uint32_t)H.n_su; ++u) { const uint32_t r = rank_of[u]; mk[P.su_tour[u] * MASKW + (r >> 6)] |= 1ull << (r & 63u); }
+    for (uint32_t u = 0; u < (uint32_t)H.n_hu; ++u) { uint2 &t = thu[P.hu_tour[u]]; t.x += 1u; t.y += rq[u]; }
+  }
+  __syncthreads();
+}
+
+// Incumbent tables from a plan slot (block-wide; ends with a barrier).
+template <int MASKW>
+__device__ void mv_encode(const MvParams &P, uint8_t *sm, const uint8_t *plan, uint32_t tid, uint32_t T)
+{
+  const ImgHdr &H = P.H; const MvHdr &M = P.M;
+  const uint32_t n_f = H.n_f, n_b = H.n_b, n_t = H.n_t;
+  const uint8_t *p_bt = plan, *p_bp = plan + M.pl_bpos;
+  const uint16_t *p_fb = reinterpret_cast<const uint16_t *>(plan + M.pl_fbp), *p_fp = reinterpret_cast<const uint16_t *>(plan + M.pl_fpos);
+  const uint64_t *p_mk = reinterpret_cast<const uint64_t *>(plan + M.pl_mask);
+  uint32_t *cnt = MV_TAB(uint32_t, M.off_cnt);
+  uint2 *bp = MV_TAB(uint2, M.off_bp);
+  for (uint32_t b = tid; b < n_b; b += T) cnt[b] = 0u;
+  __syncthreads();
+  for (uint32_t f = tid; f < n_f; f += T) atomicAdd(&cnt[p_fb[f]], 1u);
+  __syncthreads();
+  if (tid == 0) {
+    uint32_t *tpl = MV_TAB(uint32_t, M.off_tpl);
+    uint16_t *pre = MV_TAB(uint16_t, M.off_pre);
+    uint8_t *bpat = MV_TAB(uint8_t, M.off_bpat);
+    const uint32_t *dq = MV_TAB(const uint32_t, H.off_dq);
+    for (uint32_t g = 0; g < n_t; ++g) tpl[g] = 0u;
+    for (uint32_t b = 0; b < n_b; ++b) tpl[p_bt[b]] += 0x100u;
+    uint32_t acc = 0;
+    for (uint32_t g = 0; g < n_t; ++g) { const uint32_t len = tpl[g] >> 8; tpl[g] = acc | (len << 8); acc += len; }
+    for (uint32_t b = 0; b < n_b; ++b) bpat[(tpl[p_bt[b]] & 0xFFu) + p_bp[b]] = (uint8_t)b;
+    acc = 0; uint32_t n_bad = 0;
+    for (uint32_t j = 0; j < n_b; ++j) {
+      const uint32_t b = bpat[j], len = cnt[b];
+      pre[j] = (uint16_t)acc;
+      bp[b] = make_uint2(acc | (len << 16), j | ((uint32_t)p_bt[b] << 8) | ((uint32_t)p_bp[b] << 16));
+      acc += len;
+      if (len == 0u && dq[b] > 0u) ++n_bad;                    // a BP without fields fails eq. (2) unless it needs nothing
+    }
+    pre[n_b] = (uint16_t)acc;
+    MV_TAB(uint32_t, M.off_misc)[0] = n_bad;
+  }
+  if (tid >= 32u) {
+    const uint32_t *cs = MV_CTAB(uint32_t, H.offc_cs);
+    uint64_t *tmask = MV_TAB(uint64_t, M.off_tmask);
+    uint32_t *ts = MV_TAB(uint32_t, M.off_ts);
+    for (uint32_t g = tid - 32u; g < n_t; g += T - 32u) {
+      uint32_t S = 0;
+#pragma unroll
+      for (int i = 0; i < MASKW; ++i) {
+        uint64_t w = p_mk[g * MASKW + i];
+        tmask[g * MASKW + i] = w;
+        while (w) { const int r = __ffsll((long long)w) - 1; w &= w - 1; S += cs[64 * i + r]; }
+      }
+      ts[g] = S;
+    }
+  }
+  __syncthreads();
+  uint32_t *seq = MV_TAB(uint32_t, M.off_seq);
+  uint16_t *posf = MV_TAB(uint16_t, M.off_posf);
+  for (uint32_t f = tid; f < n_f; f += T) {
+    const uint32_t b = p_fb[f], pos = (bp[b].x & 0xFFFFu) + p_fp[f];
+    seq[pos] = f | (b << 16); posf[f] = (uint16_t)pos;
+  }
+  __syncthreads();
+}
+
+// ------------------------------------------------------------------ step 8: one remove/reinsert move
+
+// The moved block [a, a+len) of the incumbent's sequence reappears at position c of the worker's sequence.
+struct Move {
+  uint32_t a, len, c;
+  uint32_t fld_b;     // field move: the BP the moved field now belongs to; else kNone
+  uint32_t mv_b;      // BP move: the BP whose tour changes (to mv_t); else kNone
+  uint32_t mv_t;
+  uint32_t bad;       // BPs without fields but with positive demand under this move
+};
+
+// PAPER.md:L158, L184; R35: v = below(w0, N_F+N_B) picks a field or a BP ("since N_F >> N_B it is
+// more likely to draw fields"), target = below(w1, N_B | N_T), position = below(w2, len+1), len = length of the
+// target list after the removal.  raw (optional) receives {kind, vertex, source list, source position, target, position}.
+__device__ __forceinline__ Move mv_derive(const MvParams &P, const uint8_t *sm, uint32_t w0, uint32_t w1, uint32_t w2, uint32_t *raw)
+{
+  const ImgHdr &H = P.H; const MvHdr &M = P.M;
+  const uint32_t n_f = H.n_f, n_b = H.n_b, n_t = H.n_t;
+  const uint2 *bp = MV_TAB(const uint2, M.off_bp);
+  const uint32_t *dq = MV_TAB(const uint32_t, H.off_dq);
+  const uint32_t n_bad = MV_TAB(const uint32_t, M.off_misc)[0];
+  const uint32_t v = __umulhi(w0, n_f + n_b);
+  Move m;
+  if (v < n_f) {
+    const uint32_t a = MV_TAB(const uint16_t, M.off_posf)[v];
+    const uint32_t A = MV_TAB(const uint32_t, M.off_seq)[a] >> 16;
+    const uint32_t t = __umulhi(w1, n_b);
+    const uint2 bt = bp[t], bA = bp[A];
+    const uint32_t len_t = bt.x >> 16, start_t = bt.x & 0xFFFFu, len_A = bA.x >> 16;
+    const uint32_t q = __umulhi(w2, len_t - (A == t ? 1u : 0u) + 1u);
+    m.a = a; m.len = 1u; m.c = start_t - (a < start_t ? 1u : 0u) + q;
+    m.fld_b = t; m.mv_b = kNone; m.mv_t = 0u;
+    m.bad = n_bad - ((len_t == 0u && dq[t] > 0u) ? 1u : 0u) + ((len_A == 1u && A != t && dq[A] > 0u) ? 1u : 0u);
+    if (raw) { raw[0] = 0u; raw[1] = v; raw[2] = A; raw[3] = a - (bA.x & 0xFFFFu); raw[4] = t; raw[5] = q; }
+  } else {
+    const uint32_t b = v - n_f;
+    const uint2 bb = bp[b];
+    const uint32_t j = bb.y & 0xFFu, g = (bb.y >> 8) & 0xFFu, len = bb.x >> 16;
+    const uint32_t t = __umulhi(w1, n_t);
+    const uint32_t tp = MV_TAB(const uint32_t, M.off_tpl)[t];
+    const uint32_t t_start = tp & 0xFFu, t_len = tp >> 8;
+    const uint32_t q = __umulhi(w2, t_len - (g == t ? 1u : 0u) + 1u);
+    const uint32_t jq = t_start - (j < t_start ? 1u : 0u) + q;       // plan index of b after the move
+    const uint16_t *pre = MV_TAB(const uint16_t, M.off_pre);
+    m.a = bb.x & 0xFFFFu; m.len = len;
+    m.c = (jq <= j) ? (uint32_t)pre[jq] : (uint32_t)pre[jq + 1u] - len;
+    m.fld_b = kNone; m.mv_b = b; m.mv_t = t;
+    m.bad = n_bad;
+    if (raw) { raw[0] = 1u; raw[1] = b; raw[2] = g; raw[3] = (bb.y >> 16) & 0xFFu; raw[4] = t; raw[5] = q; }
+  }
+  return m;
+}
+
+__device__ __forceinline__ Move mv_identity(const MvParams &P, const uint8_t *sm)
+{
+  Move m; m.a = m.len = m.c = 0u; m.fld_b = m.mv_b = kNone; m.mv_t = 0u;
+  m.bad = MV_TAB(const uint32_t, P.M.off_misc)[0];
+  return m;
+}
+
+// ------------------------------------------------------------------ cost of move(x) (S4-S7)
+
+struct EvalOut { bool feasible; double cost, path, makespan; };
+
+template <int DM, int MASKW>
+__device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm, const St &s, const Move &mv)
+{
+  constexpr bool COORDS_H = (DM != 0), COORDS_B = (DM == 1);
+  const ImgHdr &H = P.H; const MvHdr &M = P.M;
+  const uint32_t n_f = H.n_f, n_b = H.n_b, n_t = H.n_t, n_su = H.n_su;
+  const uint32_t *seq  = MV_TAB(const uint32_t, M.off_seq);
+  const uint2    *bp   = MV_TAB(const uint2, M.off_bp);
+  const uint2    *thu  = MV_TAB(const uint2, M.off_thu);
+  const uint32_t *dq   = MV_TAB(const uint32_t, H.off_dq);
+  const uint2    *sh   = MV_TAB(const uint2, H.off_sh);
+  const double   *dtri = MV_TAB(const double, H.off_dtri);
+  const double   *dfb  = MV_TAB(const double, H.off_dfb);
+  const double2  *xy   = MV_TAB(const double2, H.off_xy);
+  const uint32_t *cs   = MV_CTAB(uint32_t, H.offc_cs);
+  const double   *rcp  = MV_CTAB(double, H.offc_rcp);
+  const double inf = __longlong_as_double(0x7FF0000000000000ll);
+  EvalOut out; out.feasible = false; out.cost = out.path = out.makespan = inf;
+
+  // position s of the worker's sequence -> index into the incumbent's sequence
+  const uint32_t lo = min(mv.a, mv.c), span = max(mv.a, mv.c) + mv.len - lo;
+  const uint32_t shift = (mv.c <= mv.a) ? (0u - mv.len) : mv.len;
+  const bool fld = (mv.fld_b != kNone);
+
+  // ---- S4 pass 1 (L69, L106, L213): route, area, supplies, sum over BPs of the mean field->BP leg
+  for (uint32_t g = 0; g < n_t; ++g) { s.d(M.m64_lt + g) = 0.0; s.d(M.m64_e + g) = 0.0; s.w(M.m32_hq + g) = 0u; s.w(M.m32_ng + g) = 0u; }
+  bool feas = (mv.bad == 0u);
+  {
+    uint32_t b_cur = kNone, g_cur = 0, Sq = 0, Hq = 0, k = 0, m = 0, prev = 0 /* HQ */;
+    double Lt = 0.0, sd = 0.0, sumE = 0.0;
+    for (uint32_t p = 0; p < n_f; ++p) {
+      uint32_t idx = p; bool inb = false;
+      if (p - lo < span) { const uint32_t o = p - mv.c; inb = o < mv.len; idx = inb ? mv.a + o : p + shift; }
+      const uint32_t en = seq[idx];
+      const uint32_t f = en & 0xFFFFu;
+      uint32_t b = en >> 16;
+      if (inb && fld) b = mv.fld_b;
+      if (b != b_cur) {
+        const uint32_t g = (b == mv.mv_b) ? mv.mv_t : ((bp[b].y >> 8) & 0xFFu);
+        if (b_cur != kNone) {
+          feas = feas && (Sq >= dq[b_cur]);                                  // eq. (2)
+          sumE = __dadd_rn(sumE, div_small(sd, k, rcp)); ++m;                // R10: only BPs with fields
+          if (g != g_cur) {                                                  // the tour is complete: back to HQ (L21; R2)
+            const double leg = COORDS_H ? edge_from_xy(xy, prev + n_b, 0u) : dtri[(prev * (prev - 1u)) >> 1];
+            s.d(M.m64_lt + g_cur) = __dadd_rn(Lt, leg); s.w(M.m32_hq + g_cur) = Hq;
+            s.d(M.m64_e + g_cur) = sumE; s.w(M.m32_ng + g_cur) = m;
+            Lt = 0.0; Hq = 0u; sumE = 0.0; m = 0u; prev = 0u;
+          }
+        }
+        g_cur = g; b_cur = b; sd = 0.0; Sq = 0u; k = 0u;
+      }
+      const uint2 qf = sh[f];
+      const uint32_t cur = f + 1u;
+      double leg_h, leg_b;
+      if (COORDS_H) leg_h = edge_from_xy(xy, prev ? prev + n_b : 0u, cur + n_b);
+      else { const uint32_t hi = max(prev, cur), lw = min(prev, cur); leg_h = dtri[((hi * (hi - 1u)) >> 1) + lw]; }
+      if (COORDS_B) leg_b = edge_from_xy(xy, cur + n_b, 1u + b);
+      else leg_b = dfb[f * n_b + b];
+      Lt = __dadd_rn(Lt, leg_h);                                             // field to field (L69)
+      prev = cur;
+      Hq += qf.y; Sq += qf.x; ++k;
+      sd = __dadd_rn(sd, leg_b);
+    }
+    feas = feas && (Sq >= dq[b_cur]);
+    sumE = __dadd_rn(sumE, div_small(sd, k, rcp)); ++m;
+    const double leg = COORDS_H ? edge_from_xy(xy, prev + n_b, 0u) : dtri[(prev * (prev - 1u)) >> 1];
+    s.d(M.m64_lt + g_cur) = __dadd_rn(Lt, leg); s.w(M.m32_hq + g_cur) = Hq;
+    s.d(M.m64_e + g_cur) = sumE; s.w(M.m32_ng + g_cur) = m;
+  }
+  if (!feas) return out;                                                     // discarded (L186; R19)
+
+  // ---- E(g) = 2 (sumE/m) / v_SU (L199, L213; R9); T_wait(g) (eq. (6)); T(g) = L_tour/v_HU + H_q/R_g (L190; R6)
+  const uint64_t *tmask = MV_TAB(const uint64_t, M.off_tmask);
+  const uint32_t *ts = MV_TAB(const uint32_t, M.off_ts);
+  double makespan = 0.0;
+  for (uint32_t g = 0; g < n_t; ++g) {
+    const uint32_t mm = s.w(M.m32_ng + g);
+    double E = 0.0;
+    if (mm > 0u) E = __ddiv_rn(__dmul_rn(2.0, div_small(s.d(M.m64_e + g), mm, rcp)), H.v_su);
+    s.d(M.m64_e + g) = E;
+    Mask<MASKW> mk;
+#pragma unroll
+    for (int i = 0; i < MASKW; ++i) mk.w[i] = tmask[g * MASKW + i];
+    mask_store<MASKW>(s, M.m64_mask + MASKW * g, mk);
+    const uint32_t S = ts[g];
+    s.w(M.m32_s + g) = S;
+    const uint2 hu = thu[g];
+    s.d(M.m64_w + g) = wait_time(E, S, cs[mask_top(mk)], hu.x, H.kappa, rcp);
+    const double t_g = __dadd_rn(__ddiv_rn(s.d(M.m64_lt + g), H.v_hu), __ddiv_rn((double)s.w(M.m32_hq + g), (double)hu.y));
+    if (g == 0u || t_g > makespan) makespan = t_g;
+  }
+
+  // ---- S6: Algorithm 2 (L209-227), readings R11-R16 (same procedure as in lgx_finish)
+  if (n_t >= 2u) {
+    for (uint32_t iter = 0; iter < n_su; ++iter) {
+      uint32_t g_max = 0, g_2nd = kNone; double w_max = s.d(M.m64_w), w_2nd = 0.0;
+      for (uint32_t g = 1; g < n_t; ++g) {
+        const double w = s.d(M.m64_w + g);
+        if (w > w_max) { w_2nd = w_max; g_2nd = g_max; w_max = w; g_max = g; }
+        else if (g_2nd == kNone || w > w_2nd) { w_2nd = w; g_2nd = g; }
+      }
+      uint32_t g_min = kNone; double w_min = 0.0;
+      for (uint32_t g = 0; g < n_t; ++g) {
+        const double w = s.d(M.m64_w + g);
+        if (g != g_max && g != g_2nd && (g_min == kNone || w < w_min)) { w_min = w; g_min = g; }
+      }
+      const bool two = (g_min == kNone);
+      if (two) g_min = g_2nd;                                                // R12
+      Mask<MASKW> mk_min = mask_load<MASKW>(s, M.m64_mask + MASKW * g_min);
+      if (mask_count(mk_min) <= 1) break;                                    // R15
+      Mask<MASKW> mk_max = mask_load<MASKW>(s, M.m64_mask + MASKW * g_max);
+      const uint32_t S_max = s.w(M.m32_s + g_max), M_max = cs[mask_top(mk_max)];
+      const uint32_t hu_max = thu[g_max].x;
+      const double   E_max = s.d(M.m64_e + g_max);
+      // donor's units by rising fill time (L221): the first that brings T_wait(g_max) below T_wait(g_2nd),
+      // else the largest (L225; R13).  The test is monotone in the capacity: bisect over the ranks.
+      int r = mask_top(mk_min);
+      uint32_t cr = cs[r];
+      double w_new = wait_time(E_max, S_max + cr, max(M_max, cr), hu_max, H.kappa, rcp);
+      if (w_new < w_2nd) {
+        uint32_t lo2 = 0, hi2 = (uint32_t)r;
+        while (lo2 < hi2) {
+          const uint32_t mid = (lo2 + hi2) >> 1;
+          const uint32_t cm = cs[mid];
+          const double wm = wait_time(E_max, S_max + cm, max(M_max, cm), hu_max, H.kappa, rcp);
+          if (wm < w_2nd) hi2 = mid; else lo2 = mid + 1u;
+        }
+        Mask<MASKW> ge = mk_min;
+#pragma unroll
+        for (int i = 0; i < MASKW; ++i) {
+          const int sft = (int)lo2 - 64 * i;
+          if (sft >= 64) ge.w[i] = 0ull; else if (sft > 0) ge.w[i] &= ~0ull << sft;
+        }
+        r = mask_pop_lowest(ge);
+        cr = cs[r];
+        w_new = wait_time(E_max, S_max + cr, max(M_max, cr), hu_max, H.kappa, rcp);
+      }
+      mask_flip(mk_min, r);
+      const uint32_t S_min = s.w(M.m32_s + g_min) - cr;
+      const double w_don = wait_time(s.d(M.m64_e + g_min), S_min, cs[mask_top(mk_min)], thu[g_min].x, H.kappa, rcp);
+      double new_max = w_new > w_don ? w_new : w_don;                        // step 11 (L227; R14)
+      if (!two && w_2nd > new_max) new_max = w_2nd;
+      if (!(new_max < w_max)) break;
+      mask_flip(mk_max, r);
+      mask_store<MASKW>(s, M.m64_mask + MASKW * g_min, mk_min); s.w(M.m32_s + g_min) = S_min; s.d(M.m64_w + g_min) = w_don;
+      mask_store<MASKW>(s, M.m64_mask + MASKW * g_max, mk_max); s.w(M.m32_s + g_max) = S_max + cr; s.d(M.m64_w + g_max) = w_new;
+    }
+  }
+
+  // ---- S7 pass 2: shuttles per field, eq. (4) (L89) with the tour's mean capacity (R4)
+  for (uint32_t g = 0; g < n_t; ++g) {
+    s.w(M.m32_ng + g)    = (uint32_t)mask_count(mask_load<MASKW>(s, M.m64_mask + MASKW * g));
+    s.w(M.m32_magic + g) = 0xFFFFFFFFu / s.w(M.m32_s + g);
+    s.d(M.m64_w + g) = 0.0;                                                  // T_wait is dead: the row holds the shuttle sum
+  }
+  {
+    const uint32_t *sq = MV_CTAB(uint32_t, H.offc_s);
+    uint32_t b_cur = kNone, g_cur = 0, n_g = 0, C_g = 1, magic = 0;
+    double shut = 0.0;
+    for (uint32_t p = 0; p < n_f; ++p) {
+      uint32_t idx = p; bool inb = false;
+      if (p - lo < span) { const uint32_t o = p - mv.c; inb = o < mv.len; idx = inb ? mv.a + o : p + shift; }
+      const uint32_t en = seq[idx];
+      const uint32_t f = en & 0xFFFFu;
+      uint32_t b = en >> 16;
+      if (inb && fld) b = mv.fld_b;
+      if (b != b_cur) {
+        const uint32_t g = (b == mv.mv_b) ? mv.mv_t : ((bp[b].y >> 8) & 0xFFu);
+        if (b_cur == kNone || g != g_cur) {
+          if (b_cur != kNone) { s.d(M.m64_w + g_cur) = shut; shut = 0.0; }
+          n_g = s.w(M.m32_ng + g); C_g = s.w(M.m32_s + g); magic = s.w(M.m32_magic + g);
+          g_cur = g;
+        }
+        b_cur = b;
+      }
+      const uint32_t xq = sq[f] * n_g + (C_g - 1u);
+      uint32_t N = __umulhi(xq, magic);
+      uint32_t rem = xq - N * C_g;
+      if (rem >= C_g) { ++N; rem -= C_g; }
+      if (rem >= C_g) { ++N; }
+      const double leg = COORDS_B ? edge_from_xy(xy, 1u + n_b + f, 1u + b) : dfb[f * n_b + b];
+      shut = __dadd_rn(shut, __dmul_rn((double)N, leg));
+    }
+    s.d(M.m64_w + g_cur) = shut;
+  }
+  // ---- lengths (L106): N_HU(g), N_SU(g) multiply the tour distance, shuttles x2; cost (R1)
+  double path = 0.0;
+  for (uint32_t g = 0; g < n_t; ++g) {
+    const double lt = s.d(M.m64_lt + g), shut = s.d(M.m64_w + g);
+    const double l_hu  = __dmul_rn((double)thu[g].x, lt);
+    const double l_esu = __dadd_rn(__dmul_rn((double)s.w(M.m32_ng + g), lt), shut);
+    path = __dadd_rn(path, __dadd_rn(__dadd_rn(l_hu, l_esu), shut));
+  }
+  out.feasible = true; out.path = path; out.makespan = makespan;
+  out.cost = __dadd_rn(__dmul_rn(H.w_path, path), __dmul_rn(H.w_time, makespan));
+  return out;
+}
+
+// ------------------------------------------------------------------ common prologue
+
+template <int MASKW>
+__device__ __forceinline__ void mv_prologue(const MvParams &P, uint8_t *sm, St &s, uint32_t tid, uint32_t T)
+{
+  const ImgHdr &H = P.H; const MvHdr &M = P.M;
+  {
+    const uint4 *src = reinterpret_cast<const uint4 *>(P.image);
+    uint4 *dst = reinterpret_cast<uint4 *>(sm);
+    for (uint32_t i = tid; i < H.image_bytes / 16u; i += T) dst[i] = src[i];
+    src = reinterpret_cast<const uint4 *>(P.image_c + H.offc_s);
+    dst = reinterpret_cast<uint4 *>(sm + M.off_c);
+    for (uint32_t i = tid; i < (H.imagec_bytes - H.offc_s) / 16u; i += T) dst[i] = src[i];
+  }
+  s.T4 = 4u * T; s.T8 = 8u * T;
+  s.b64 = sm + M.off_state + 8u * tid;
+  s.b32 = sm + M.off_state + M.m64_rows * s.T8 + 4u * tid;
+  __syncthreads();
+}
+
+// ================================================================== batch kernel (L163-165)
+
+template <int DM, int MASKW>
+__global__ void __launch_bounds__(kMvThreads, 1) lgx_move_eval_k(const __grid_constant__ MvParams P)
+{
+  extern __shared__ __align__(16) uint8_t smem[];
+  uint8_t *sm = smem;
+  const uint32_t tid = threadIdx.x, T = blockDim.x;
+  St s;
+  mv_prologue<MASKW>(P, sm, s, tid, T);
+  uint8_t *plan = sm + P.M.off_plans;
+  mv_load_plan<MASKW>(P, sm, plan, tid, T);
+  mv_encode<MASKW>(P, sm, plan, tid, T);
+  const uint64_t stride = (uint64_t)gridDim.x * T;
+  for (uint64_t i = (uint64_t)blockIdx.x * T + tid; i < P.n; i += stride) {
+    const uint64_t id = P.first_id + i;
+    uint32_t w[4];
+    philox_block(P, (uint32_t)id, (uint32_t)(id >> 32), 5u, 0u, w);
+    const Move mv = mv_derive(P, sm, w[0], w[1], w[2], nullptr);
+    const EvalOut r = mv_eval<DM, MASKW>(P, sm, s, mv);
+    if (P.cost)       P.cost[i] = r.cost;
+    if (P.path_km)    P.path_km[i] = r.path;
+    if (P.makespan_h) P.makespan_h[i] = r.makespan;
+    if (P.feasible)   P.feasible[i] = r.feasible ? 1 : 0;
+  }
+}
+
+// ================================================================== Algorithm 1 steps 4-16, persistent
+
+template <int DM, int MASKW>
+__global__ void __launch_bounds__(kMvThreads, 1) lgx_local_search_k(const __grid_constant__ MvParams P)
+{
+  extern __shared__ __align__(16) uint8_t smem[];
+  uint8_t *sm = smem;
+  cg::grid_group grid = cg::this_grid();
+  const ImgHdr &H = P.H; const MvHdr &M = P.M;
+  const uint32_t tid = threadIdx.x, T = blockDim.x;
+  const uint32_t n_f = H.n_f, n_b = H.n_b, n_t = H.n_t;
+  __shared__ unsigned long long s_bits[kMvThreads / 32], s_id[kMvThreads / 32];
+  __shared__ unsigned long long s_win[3];      // global winner of the iteration: cost bits, id, block
+  __shared__ unsigned long long s_cstar;       // cost bits of x*
+  St s;
+  mv_prologue<MASKW>(P, sm, s, tid, T);
+  uint8_t *x_best = sm + M.off_plans, *x_old = x_best + M.plan_bytes, *x_tmp = x_old + M.plan_bytes;
+  uint32_t *misc = MV_TAB(uint32_t, M.off_misc);
+  auto copy_plan = [&](uint8_t *dst, const uint8_t *src) {
+    for (uint32_t i = tid; i < M.plan_bytes / 8u; i += T) reinterpret_cast<uint64_t *>(dst)[i] = reinterpret_cast<const uint64_t *>(src)[i];
+  };
+
+  // ---- step 4 (L133): x* = x_0 with its cost; x_0 takes the SU sets Algorithm 2 leaves it with (R37)
+  mv_load_plan<MASKW>(P, sm, x_best, tid, T);
+  mv_encode<MASKW>(P, sm, x_best, tid, T);
+  if (tid == 0) {
+    const EvalOut r = mv_eval<DM, MASKW>(P, sm, s, mv_identity(P, sm));
+    s_cstar = (unsigned long long)__double_as_longlong(r.cost);
+    if (r.feasible) {
+      uint64_t *mk = reinterpret_cast<uint64_t *>(x_best + M.pl_mask);
+      for (uint32_t i = 0; i < n_t * MASKW; ++i) mk[i] = s.q(M.m64_mask + i);
+    }
+  }
+  __syncthreads();
+  copy_plan(x_old, x_best);
+  __syncthreads();
+
+  const uint32_t SW = M.slot_words;
+  for (uint32_t k = 0; k < P.n_iters; ++k) {
+    // ---- step 6, eq. (5) (L177): x = x* with probability eps, else the previous iteration's winner
+    uint32_t uw[4];
+    philox_block(P, k, 0u, 6u, 0u, uw);
+    const uint8_t *x_cur = (uw[0] < P.eps_thresh) ? x_best : x_old;
+    mv_encode<MASKW>(P, sm, x_cur, tid, T);
+
+    // ---- steps 7-12: every worker moves x once and scores it; running (cost, id) minimum per thread
+    unsigned long long best_bits = ~0ull, best_id = ~0ull;
+    const uint64_t id0 = (uint64_t)k * P.n_workers;
+    for (uint64_t i = (uint64_t)blockIdx.x * T + tid; i < P.n_workers; i += (uint64_t)gridDim.x * T) {
+      const uint64_t id = id0 + i;
+      uint32_t w[4];
+      philox_block(P, (uint32_t)id, (uint32_t)(id >> 32), 5u, 0u, w);
+      const Move mv = mv_derive(P, sm, w[0], w[1], w[2], nullptr);
+      const EvalOut r = mv_eval<DM, MASKW>(P, sm, s, mv);
+      const unsigned long long bits = (unsigned long long)__double_as_longlong(r.cost);
+      if (bits < best_bits || (bits == best_bits && id < best_id)) {
+        best_bits = bits; best_id = id;
+        if (r.feasible) for (uint32_t q = 0; q < n_t * MASKW; ++q) s.q(M.m64_bmask + q) = s.q(M.m64_mask + q);
+      }
+    }
+    // ---- step 13 (L167): i* = arg min C_i.  warp -> block -> one slot per block -> grid barrier -> every block folds
+    unsigned long long bb = best_bits, bi = best_id;
+#pragma unroll
+    for (int off = 16; off >= 1; off >>= 1) {
+      const unsigned long long ob = __shfl_down_sync(0xFFFFFFFFu, bb, off), oi = __shfl_down_sync(0xFFFFFFFFu, bi, off);
+      take_min(bb, bi, ob, oi);
+    }
+    if ((tid & 31u) == 0u) { s_bits[tid >> 5] = bb; s_id[tid >> 5] = bi; }
+    __syncthreads();
+    if (tid < 32u) {
+      const uint32_t nw = (T + 31u) >> 5;
+      bb = tid < nw ? s_bits[tid] : ~0ull; bi = tid < nw ? s_id[tid] : ~0ull;
+#pragma unroll
+      for (int off = 16; off >= 1; off >>= 1) {
+        const unsigned long long ob = __shfl_down_sync(0xFFFFFFFFu, bb, off), oi = __shfl_down_sync(0xFFFFFFFFu, bi, off);
+        take_min(bb, bi, ob, oi);
+      }
+      if (tid == 0u) { s_win[0] = bb; s_win[1] = bi; }
+    }
+    __syncthreads();
+    unsigned long long *slot = P.slots + ((size_t)(k & 1u) * gridDim.x + blockIdx.x) * SW;
+    if (tid == 0u) { slot[0] = s_win[0]; slot[1] = s_win[1]; }
+    if (best_id == s_win[1] && best_id != ~0ull)                             // the block's winner publishes its SU sets
+      for (uint32_t q = 0; q < n_t * MASKW; ++q) slot[2 + q] = s.q(M.m64_bmask + q);
+    grid.sync();
+    if (tid < 32u) {
+      const unsigned long long *all = P.slots + (size_t)(k & 1u) * gridDim.x * SW;
+      bb = ~0ull; bi = ~0ull; unsigned long long bw = 0;
+      for (uint32_t blk = tid; blk < gridDim.x; blk += 32u) {
+        const unsigned long long ob = __ldcg(all + (size_t)blk * SW), oi = __ldcg(all + (size_t)blk * SW + 1);
+        if (ob < bb || (ob == bb && oi < bi)) { bb = ob; bi = oi; bw = blk; }
+      }
+#pragma unroll
+      for (int off = 16; off >= 1; off >>= 1) {
+        const unsigned long long ob = __shfl_down_sync(0xFFFFFFFFu, bb, off), oi = __shfl_down_sync(0xFFFFFFFFu, bi, off);
+        const unsigned long long ow = __shfl_down_sync(0xFFFFFFFFu, bw, off);
+        if (ob < bb || (ob == bb && oi < bi)) { bb = ob; bi = oi; bw = ow; }
+      }
+      if (tid == 0u) {
+        s_win[0] = bb; s_win[1] = bi; s_win[2] = bw;
+        if (blockIdx.x == 0u) {
+          if (P.hist_cost) P.hist_cost[k] = __longlong_as_double((long long)bb);
+          if (P.hist_id)   P.hist_id[k] = bi;
+        }
+        // the winning move, replayed from its id (L233), for the block-wide update below
+        uint32_t w[4];
+        philox_block(P, (uint32_t)bi, (uint32_t)(bi >> 32), 5u, 0u, w);
+        (void)mv_derive(P, sm, w[0], w[1], w[2], misc + 4);
+      }
+    }
+    __syncthreads();
+    // ---- steps 14-15 (L169): x_old <- x_{i*}; x* <- x_{i*} if it improves C*.  All workers infeasible: keep x_old (R37)
+    const unsigned long long win_bits = s_win[0];
+    if (win_bits < 0x7FF0000000000000ull) {
+      if (x_cur != x_tmp) copy_plan(x_tmp, x_cur);
+      __syncthreads();
+      const uint32_t kind = misc[4], vx = misc[5], src = misc[6], sp = misc[7], dst = misc[8], dp = misc[9];
+      if (kind == 0u) {
+        uint16_t *fb = reinterpret_cast<uint16_t *>(x_tmp + M.pl_fbp), *fp = reinterpret_cast<uint16_t *>(x_tmp + M.pl_fpos);
+        for (uint32_t f = tid; f < n_f; f += T) {
+          if (f == vx) { fb[f] = (uint16_t)dst; fp[f] = (uint16_t)dp; continue; }
+          const uint32_t b = fb[f]; uint32_t q = fp[f];
+          if (b == src && q > sp) --q;
+          if (b == dst && q >= dp) ++q;
+          fp[f] = (uint16_t)q;
+        }
+      } else {
+        uint8_t *bt = x_tmp, *bq = x_tmp + M.pl_bpos;
+        for (uint32_t b = tid; b < n_b; b += T) {
+          if (b == vx) { bt[b] = (uint8_t)dst; bq[b] = (uint8_t)dp; continue; }
+          const uint32_t g = bt[b]; uint32_t q = bq[b];
+          if (g == src && q > sp) --q;
+          if (g == dst && q >= dp) ++q;
+          bq[b] = (uint8_t)q;
+        }
+      }
+      {
+        const unsigned long long *wm = P.slots + ((size_t)(k & 1u) * gridDim.x + (size_t)s_win[2]) * SW + 2;
+        uint64_t *mk = reinterpret_cast<uint64_t *>(x_tmp + M.pl_mask);
+        for (uint32_t q = tid; q < n_t * MASKW; q += T) mk[q] = __ldcg(wm + q);
+      }
+      __syncthreads();
+      const bool improves = win_bits < s_cstar;
+      __syncthreads();
+      if (improves) { copy_plan(x_best, x_tmp); if (tid == 0u) s_cstar = win_bits; }
+      copy_plan(x_old, x_tmp);
+      __syncthreads();
+    }
+  }
+
+  // ---- x* and C* back to the caller's arrays
+  if (blockIdx.x == 0u) {
+    for (uint32_t b = tid; b < n_b; b += T) { P.bp_tour[b] = x_best[b]; P.bp_pos[b] = x_best[M.pl_bpos + b]; }
+    const uint16_t *fb = reinterpret_cast<const uint16_t *>(x_best + M.pl_fbp), *fp = reinterpret_cast<const uint16_t *>(x_best + M.pl_fpos);
+    for (uint32_t f = tid; f < n_f; f += T) { P.field_bp[f] = fb[f]; P.field_pos[f] = fp[f]; }
+    if (tid == 0u) {
+      const uint64_t *mk = reinterpret_cast<const uint64_t *>(x_best + M.pl_mask);
+      const uint8_t *unit_of = MV_CTAB(uint8_t, H.offc_unit);
+      for (uint32_t g = 0; g < n_t; ++g)
+        for (int i = 0; i < MASKW; ++i) {
+          uint64_t w = mk[g * MASKW + i];
+          while (w) { const int r = __ffsll((long long)w) - 1; w &= w - 1; P.su_tour[unit_of[64 * i + r]] = (uint8_t)g; }
+        }
+      *P.best_cost = __longlong_as_double((long long)s_cstar);
+    }
+  }
+}
+
+// ================================================================== Algorithm 1 steps 1-3
+
+struct InitParams {
+  int32_t n_f, n_b, n_t, n_hu, n_su;
+  const double2  *xy;        // [1 + n_b + n_f] vertex coordinates: HQ, BPs, fields
+  const uint32_t *sq, *dq;   // supply / demand quanta
+  const uint8_t  *unit_of;   // SU of capacity rank r (ascending (capacity, unit))
+  uint8_t *bp_tour, *bp_pos; uint16_t *field_bp, *field_pos; uint8_t *hu_tour, *su_tour;
+  uint32_t *scratch;         // [n_b] supplies | [n_b + 1] list offsets | [n_b] cursors | u16 [n_f] lists | u8 [n_b] chain, flags
+};
+
+// lexicographic (distance, index) minimum over a warp: "closest", lowest index on ties
+__device__ __forceinline__ void warp_argmin(double &d, uint32_t &i)
+{
+#pragma unroll
+  for (int off = 16; off >= 1; off >>= 1) {
+    const double od = __shfl_xor_sync(0xFFFFFFFFu, d, off);
+    const uint32_t oi = __shfl_xor_sync(0xFFFFFFFFu, i, off);
+    if (oi != kNone && (i == kNone || od < d || (od == d && oi < i))) { d = od; i = oi; }
+  }
+}
+
+// One block.  Step 1 (L122): HUs in index order, floor(N_HU/N_T) per tour, the residual on the last tour (R25);
+// SUs dealt round-robin over the capacity order (Case 1: the same number of each class per tour, L273; R31);
+// nearest-neighbour chain over the BPs from HQ, cut into N_T consecutive runs (R32).  Step 2 (L124): fields in
+// identification order (L173) to their closest BP not yet supplied, else to their closest BP.  Step 3 (L126,
+// L171): per BP a nearest-neighbour order starting from HQ.
+__global__ void __launch_bounds__(256, 1) lgx_init_plan_k(const InitParams P)
+{
+  const uint32_t tid = threadIdx.x, T = blockDim.x, lane = tid & 31u, warp = tid >> 5, n_warps = T >> 5;
+  const uint32_t n_f = P.n_f, n_b = P.n_b, n_t = P.n_t;
+  uint32_t *Sq = P.scratch, *off = Sq + n_b, *cur_w = off + n_b + 1u;
+  uint16_t *lst = reinterpret_cast<uint16_t *>(cur_w + n_b);
+  uint8_t *chain = reinterpret_cast<uint8_t *>(lst + n_f + (n_f & 1u)), *used = chain + n_b;
+  for (uint32_t b = tid; b < n_b; b += T) { Sq[b] = 0u; used[b] = 0; }
+  { const uint32_t per = (uint32_t)P.n_hu / n_t;
+    for (uint32_t u = tid; u < (uint32_t)P.n_hu; u += T) { const uint32_t g = u / per; P.hu_tour[u] = (uint8_t)(g < n_t ? g : n_t - 1u); } }
+  for (uint32_t r = tid; r < (uint32_t)P.n_su; r += T) P.su_tour[P.unit_of[r]] = (uint8_t)(r % n_t);
+  __syncthreads();
+  if (warp == 0u) {
+    // step 1 (ii): BP chain
+    uint32_t cur = 0;
+    for (uint32_t k = 0; k < n_b; ++k) {
+      double bd = 0.0; uint32_t best = kNone;
+      for (uint32_t b = lane; b < n_b; b += 32u) if (!used[b]) { const double d = edge_from_xy(P.xy, cur, 1u + b); if (best == kNone || d < bd) { best = b; bd = d; } }
+      warp_argmin(bd, best);
+      if (lane == 0u) { used[best] = 1; chain[k] = (uint8_t)best; }
+      __syncwarp();
+      cur = 1u + best;
+    }
+    for (uint32_t g = 0; g < n_t; ++g) {
+      const uint32_t lo = (g * n_b) / n_t, hi = ((g + 1u) * n_b) / n_t;
+      for (uint32_t k = lo + lane; k < hi; k += 32u) { P.bp_tour[chain[k]] = (uint8_t)g; P.bp_pos[chain[k]] = (uint8_t)(k - lo); }
+    }
+    // step 2: fields -> BPs, serial over the fields (the supplies change), the BP scan across the lanes
+    for (uint32_t f = 0; f < n_f; ++f) {
+      double bd = 0.0, ad = 0.0; uint32_t best = kNone, any = kNone;
+      for (uint32_t b = lane; b < n_b; b += 32u) {
+        const double d = edge_from_xy(P.xy, 1u + n_b + f, 1u + b);
+        if (any == kNone || d < ad) { any = b; ad = d; }
+        if (Sq[b] < P.dq[b] && (best == kNone || d < bd)) { best = b; bd = d; }
+      }
+      warp_argmin(bd, best);
+      if (best == kNone) { warp_argmin(ad, any); best = any; }
+      if (lane == 0u) { P.field_bp[f] = (uint16_t)best; Sq[best] += P.sq[f]; }
+      __syncwarp();
+    }
+  }
+  __syncthreads();
+  // per-BP field lists
+  for (uint32_t b = tid; b <= n_b; b += T) off[b] = 0u;
+  __syncthreads();
+  for (uint32_t f = tid; f < n_f; f += T) atomicAdd(&off[P.field_bp[f] + 1u], 1u);
+  __syncthreads();
+  if (tid == 0u) for (uint32_t b = 0; b < n_b; ++b) { off[b + 1u] += off[b]; cur_w[b] = off[b]; }
+  __syncthreads();
+  for (uint32_t f = tid; f < n_f; f += T) lst[atomicAdd(&cur_w[P.field_bp[f]], 1u)] = (uint16_t)f;
+  __syncthreads();
+  // step 3: one warp per BP, nearest neighbour from HQ; a visited list entry becomes 0xFFFF
+  for (uint32_t b = warp; b < n_b; b += n_warps) {
+    uint32_t cur = 0;
+    const uint32_t lo = off[b], hi = off[b + 1u];
+    for (uint32_t k = 0; k < hi - lo; ++k) {
+      double bd = 0.0; uint32_t best = kNone, slot = 0;
+      for (uint32_t e = lo + lane; e < hi; e += 32u) {
+        const uint32_t f = lst[e];
+        if (f != 0xFFFFu) { const double d = edge_from_xy(P.xy, cur, 1u + n_b + f); if (best == kNone || d < bd || (d == bd && f < best)) { best = f; bd = d; slot = e; } }
+      }
+      // the warp minimum over (distance, field); its owner clears the entry
+      double wd = bd; uint32_t wf = best;
+      warp_argmin(wd, wf);
+      if (best == wf && best != kNone) { lst[slot] = 0xFFFFu; P.field_pos[wf] = (uint16_t)k; }
+      __syncwarp();
+      cur = 1u + n_b + wf;
+    }
+  }
+}
+
+#undef MV_TAB
+#undef MV_CTAB
+
+}  // namespace lgx
