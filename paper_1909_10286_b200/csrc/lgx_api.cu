@@ -344,9 +344,12 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   // ---- move kernels: shared-memory layout (lgx_moves.cuh) and vertex coordinates for lgx_init_plan
   {
     MvHdr &M = I->mv;
-    uint32_t o = H.image_bytes;
-    M.off_c = o;     o = align16(o + (H.imagec_bytes - H.offc_s));
-    M.off_seq = o;   o = align16(o + 4u * (uint32_t)nf);
+    uint32_t o = 0;
+    M.off_xy = o;    o = align16(o + 16u * (uint32_t)(1 + nb + nf));
+    M.off_dq = o;    o = align16(o + 4u * (uint32_t)nb);
+    M.off_c = o;     o = align16(o + (H.imagec_bytes - H.offc_cs));
+    M.off_pos4 = o;  o = align16(o + 16u * (uint32_t)nf);
+    M.off_leg2 = o;  o = align16(o + 16u * (uint32_t)nf);
     M.off_posf = o;  o = align16(o + 2u * (uint32_t)nf);
     M.off_bp = o;    o = align16(o + 8u * (uint32_t)nb);
     M.off_pre = o;   o = align16(o + 2u * ((uint32_t)nb + 1u));
@@ -624,11 +627,9 @@ using MvKernelFn = void (*)(const MvParams);
 
 void pick_move_kernels(const ImgHdr &h, MvKernelFn &kb, MvKernelFn &ks)
 {
-  const int dm = h.coords, mw = (int)h.mask_words;
   kb = ks = nullptr;
-#define LGX_PICK(D, M) if (dm == D && mw == M) { kb = lgx_move_eval_k<D, M>; ks = lgx_local_search_k<D, M>; }
-  LGX_PICK(0, 1) LGX_PICK(0, 2) LGX_PICK(1, 1) LGX_PICK(1, 2) LGX_PICK(2, 1) LGX_PICK(2, 2)
-#undef LGX_PICK
+  if (h.mask_words == 1u) { kb = lgx_move_eval_k<1>; ks = lgx_local_search_k<1>; }
+  if (h.mask_words == 2u) { kb = lgx_move_eval_k<2>; ks = lgx_local_search_k<2>; }
 }
 
 // A plan is valid when every BP sits on exactly one tour at a unique position 0..len-1, every field on exactly
@@ -697,7 +698,7 @@ int plan_download(const ImgHdr &H, const PlanDev &D, uint8_t *bt, uint8_t *bq, u
 
 void mv_fill(const lgx_instance *I, MvParams &P, uint64_t seed, const PlanDev &D)
 {
-  P.H = I->hdr; P.M = I->mv; P.image = I->d_image; P.image_c = I->d_image_c;
+  P.H = I->hdr; P.M = I->mv; P.image = I->d_image; P.image_c = I->d_image_c; P.xy = I->d_xy;
   uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
   for (int r = 0; r < 10; ++r) { P.rk[2 * r] = k0; P.rk[2 * r + 1] = k1; k0 += kPhiloxW0; k1 += kPhiloxW1; }
   P.bp_tour = D.bt; P.bp_pos = D.bq; P.field_bp = D.fb; P.field_pos = D.fq; P.hu_tour = D.hu; P.su_tour = D.su;

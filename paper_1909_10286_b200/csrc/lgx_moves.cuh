@@ -18,6 +18,13 @@
 // from the winning id ("identical random process control", L233, taken one step further): the only
 // inter-SM traffic per iteration is one slot of (cost, id, SU sets) per block and one grid barrier.
 //
+// Because every worker walks the SAME sequence except around its one moved block, the two distances each
+// field contributes — the HU leg from its predecessor and the shuttle leg to its BP — are computed ONCE per
+// iteration per SM while the incumbent is encoded (leg2[p]) and merely read by the workers; a worker computes
+// a distance itself (from the vertex coordinates, same formula, same bits) only at the <= 3 positions where its
+// predecessor differs and for the moved field's new BP.  The per-field work of a worker is then two
+// shared-memory loads, two FP64 additions and the integer bookkeeping, whatever N_F is.
+//
 // FP64 arithmetic follows DESIGN.md S4-S7 operation by operation (compiled with -fmad=false), in the
 // oracle's summation order, so costs are bit-equal.
 #pragma once
@@ -31,11 +38,14 @@ constexpr int      kMvThreads = 512;            // __launch_bounds__ of the move
 constexpr uint32_t kNone      = 0xFFFFFFFFu;
 
 // Shared-memory layout of the move kernels (byte offsets from the start of dynamic shared memory):
-//   image AB | tail of image C (from offc_s) | incumbent tables | plan store | per-thread state rows
+//   vertex coordinates | demand quanta | tail of image C (from offc_cs) | incumbent tables | plan store | per-thread state rows
 struct MvHdr {
-  uint32_t off_c;       // tail of image C: byte x of image C (x >= offc_s) sits at off_c + x - offc_s
-  uint32_t off_seq;     // u32 [n_f]      f | b << 16 in plan order
-  uint32_t off_posf;    // u16 [n_f]      position of field f in seq
+  uint32_t off_xy;      // f64x2 [1 + n_b + n_f]  vertex coordinates: HQ, BPs, fields
+  uint32_t off_dq;      // u32 [n_b]      demand quanta
+  uint32_t off_c;       // tail of image C: byte x of image C (x >= offc_cs) sits at off_c + x - offc_cs
+  uint32_t off_pos4;    // u32x4 [n_f]    plan order: f | b << 16, s_q[f], h_q[f], tour of b
+  uint32_t off_leg2;    // f64x2 [n_f]    plan order: D(predecessor on the tour or HQ, f), D(f, b)
+  uint32_t off_posf;    // u16 [n_f]      position of field f in plan order
   uint32_t off_bp;      // u32x2 [n_b]    x = start | len << 16;  y = plan index | tour << 8 | pos << 16
   uint32_t off_pre;     // u16 [n_b + 1]  start of the BP at plan index j; pre[n_b] = n_f
   uint32_t off_bpat;    // u8 [n_b]       BP at plan index j
@@ -52,13 +62,14 @@ struct MvHdr {
   uint32_t m64_lt, m64_e, m64_w, m64_mask, m64_bmask, m64_rows;
   uint32_t m32_hq, m32_s, m32_ng, m32_magic, m32_rows;
   uint32_t slot_words;  // 64-bit words per block slot: cost bits, id, masks
-  uint32_t pad_[2];
+  uint32_t pad_[3];
 };
 
 struct MvParams {
   ImgHdr          H;
   MvHdr           M;
-  const uint8_t  *image, *image_c;
+  const uint8_t  *image, *image_c;      // device copies of the instance images (global memory)
+  const double2  *xy;                   // vertex coordinates (global memory)
   uint32_t        rk[20];               // Philox round keys of the seed
   // the plan x (device arrays; in for the batch kernel, in/out for the search)
   uint8_t *bp_tour, *bp_pos; uint16_t *field_bp, *field_pos; uint8_t *hu_tour, *su_tour;
@@ -73,7 +84,7 @@ struct MvParams {
 };
 
 #define MV_TAB(type, off) (reinterpret_cast<type *>(sm + (off)))
-#define MV_CTAB(type, offc) (reinterpret_cast<const type *>(sm + (P.M.off_c + ((offc) - P.H.offc_s))))
+#define MV_CTAB(type, offc) (reinterpret_cast<const type *>(sm + (P.M.off_c + ((offc) - P.H.offc_cs))))
 
 // ------------------------------------------------------------------ plan -> shared memory
 
@@ -119,7 +130,7 @@ __device__ void mv_encode(const MvParams &P, uint8_t *sm, const uint8_t *plan, u
     uint32_t *tpl = MV_TAB(uint32_t, M.off_tpl);
     uint16_t *pre = MV_TAB(uint16_t, M.off_pre);
     uint8_t *bpat = MV_TAB(uint8_t, M.off_bpat);
-    const uint32_t *dq = MV_TAB(const uint32_t, H.off_dq);
+    const uint32_t *dq = MV_TAB(const uint32_t, M.off_dq);
     for (uint32_t g = 0; g < n_t; ++g) tpl[g] = 0u;
     for (uint32_t b = 0; b < n_b; ++b) tpl[p_bt[b]] += 0x100u;
     uint32_t acc = 0;
@@ -152,11 +163,27 @@ __device__ void mv_encode(const MvParams &P, uint8_t *sm, const uint8_t *plan, u
     }
   }
   __syncthreads();
-  uint32_t *seq = MV_TAB(uint32_t, M.off_seq);
+  uint4 *pos4 = MV_TAB(uint4, M.off_pos4);
   uint16_t *posf = MV_TAB(uint16_t, M.off_posf);
+  const uint2 *sh = reinterpret_cast<const uint2 *>(P.image + H.off_sh);     // {s_q, h_q} per field (global, L2-resident)
   for (uint32_t f = tid; f < n_f; f += T) {
-    const uint32_t b = p_fb[f], pos = (bp[b].x & 0xFFFFu) + p_fp[f];
-    seq[pos] = f | (b << 16); posf[f] = (uint16_t)pos;
+    const uint32_t b = p_fb[f];
+    const uint2 bb = bp[b];
+    const uint32_t pos = (bb.x & 0xFFFFu) + p_fp[f];
+    const uint2 q = sh[f];
+    pos4[pos] = make_uint4(f | (b << 16), q.x, q.y, (bb.y >> 8) & 0xFFu);
+    posf[f] = (uint16_t)pos;
+  }
+  __syncthreads();
+  // the two legs of every position of the incumbent (S0: one rounding per operation)
+  const double2 *xy = MV_TAB(const double2, M.off_xy);
+  double2 *leg2 = MV_TAB(double2, M.off_leg2);
+  for (uint32_t p = tid; p < n_f; p += T) {
+    const uint4 e = pos4[p];
+    const uint32_t f = e.x & 0xFFFFu, b = e.x >> 16;
+    uint32_t pred = 0u;                                                        // HQ: first field of its tour (L21)
+    if (p > 0u) { const uint4 ep = pos4[p - 1u]; if (ep.w == e.w) pred = 1u + n_b + (ep.x & 0xFFFFu); }
+    leg2[p] = make_double2(edge_from_xy(xy, pred, 1u + n_b + f), edge_from_xy(xy, 1u + n_b + f, 1u + b));
   }
   __syncthreads();
 }
@@ -166,7 +193,8 @@ __device__ void mv_encode(const MvParams &P, uint8_t *sm, const uint8_t *plan, u
 // The moved block [a, a+len) of the incumbent's sequence reappears at position c of the worker's sequence.
 struct Move {
   uint32_t a, len, c;
-  uint32_t fld_b;     // field move: the BP the moved field now belongs to; else kNone
+  uint32_t fld_b;     // field move: the BP the moved field now belongs to (on tour fld_g); else kNone
+  uint32_t fld_g;
   uint32_t mv_b;      // BP move: the BP whose tour changes (to mv_t); else kNone
   uint32_t mv_t;
   uint32_t bad;       // BPs without fields but with positive demand under this move
@@ -180,19 +208,19 @@ __device__ __forceinline__ Move mv_derive(const MvParams &P, const uint8_t *sm, 
   const ImgHdr &H = P.H; const MvHdr &M = P.M;
   const uint32_t n_f = H.n_f, n_b = H.n_b, n_t = H.n_t;
   const uint2 *bp = MV_TAB(const uint2, M.off_bp);
-  const uint32_t *dq = MV_TAB(const uint32_t, H.off_dq);
+  const uint32_t *dq = MV_TAB(const uint32_t, M.off_dq);
   const uint32_t n_bad = MV_TAB(const uint32_t, M.off_misc)[0];
   const uint32_t v = __umulhi(w0, n_f + n_b);
   Move m;
   if (v < n_f) {
     const uint32_t a = MV_TAB(const uint16_t, M.off_posf)[v];
-    const uint32_t A = MV_TAB(const uint32_t, M.off_seq)[a] >> 16;
+    const uint32_t A = MV_TAB(const uint4, M.off_pos4)[a].x >> 16;
     const uint32_t t = __umulhi(w1, n_b);
     const uint2 bt = bp[t], bA = bp[A];
     const uint32_t len_t = bt.x >> 16, start_t = bt.x & 0xFFFFu, len_A = bA.x >> 16;
     const uint32_t q = __umulhi(w2, len_t - (A == t ? 1u : 0u) + 1u);
     m.a = a; m.len = 1u; m.c = start_t - (a < start_t ? 1u : 0u) + q;
-    m.fld_b = t; m.mv_b = kNone; m.mv_t = 0u;
+    m.fld_b = t; m.fld_g = (bt.y >> 8) & 0xFFu; m.mv_b = kNone; m.mv_t = 0u;
     m.bad = n_bad - ((len_t == 0u && dq[t] > 0u) ? 1u : 0u) + ((len_A == 1u && A != t && dq[A] > 0u) ? 1u : 0u);
     if (raw) { raw[0] = 0u; raw[1] = v; raw[2] = A; raw[3] = a - (bA.x & 0xFFFFu); raw[4] = t; raw[5] = q; }
   } else {
@@ -207,7 +235,7 @@ __device__ __forceinline__ Move mv_derive(const MvParams &P, const uint8_t *sm, 
     const uint16_t *pre = MV_TAB(const uint16_t, M.off_pre);
     m.a = bb.x & 0xFFFFu; m.len = len;
     m.c = (jq <= j) ? (uint32_t)pre[jq] : (uint32_t)pre[jq + 1u] - len;
-    m.fld_b = kNone; m.mv_b = b; m.mv_t = t;
+    m.fld_b = kNone; m.fld_g = 0u; m.mv_b = b; m.mv_t = t;
     m.bad = n_bad;
     if (raw) { raw[0] = 1u; raw[1] = b; raw[2] = g; raw[3] = (bb.y >> 16) & 0xFFu; raw[4] = t; raw[5] = q; }
   }
@@ -216,7 +244,7 @@ __device__ __forceinline__ Move mv_derive(const MvParams &P, const uint8_t *sm, 
 
 __device__ __forceinline__ Move mv_identity(const MvParams &P, const uint8_t *sm)
 {
-  Move m; m.a = m.len = m.c = 0u; m.fld_b = m.mv_b = kNone; m.mv_t = 0u;
+  Move m; m.a = m.len = m.c = 0u; m.fld_b = m.mv_b = kNone; m.fld_g = m.mv_t = 0u;
   m.bad = MV_TAB(const uint32_t, P.M.off_misc)[0];
   return m;
 }
@@ -225,73 +253,70 @@ __device__ __forceinline__ Move mv_identity(const MvParams &P, const uint8_t *sm
 
 struct EvalOut { bool feasible; double cost, path, makespan; };
 
-template <int DM, int MASKW>
+template <int MASKW>
 __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm, const St &s, const Move &mv)
 {
-  constexpr bool COORDS_H = (DM != 0), COORDS_B = (DM == 1);
   const ImgHdr &H = P.H; const MvHdr &M = P.M;
   const uint32_t n_f = H.n_f, n_b = H.n_b, n_t = H.n_t, n_su = H.n_su;
-  const uint32_t *seq  = MV_TAB(const uint32_t, M.off_seq);
-  const uint2    *bp   = MV_TAB(const uint2, M.off_bp);
+  const uint4    *pos4 = MV_TAB(const uint4, M.off_pos4);
+  const double2  *leg2 = MV_TAB(const double2, M.off_leg2);
   const uint2    *thu  = MV_TAB(const uint2, M.off_thu);
-  const uint32_t *dq   = MV_TAB(const uint32_t, H.off_dq);
-  const uint2    *sh   = MV_TAB(const uint2, H.off_sh);
-  const double   *dtri = MV_TAB(const double, H.off_dtri);
-  const double   *dfb  = MV_TAB(const double, H.off_dfb);
-  const double2  *xy   = MV_TAB(const double2, H.off_xy);
+  const uint32_t *dq   = MV_TAB(const uint32_t, M.off_dq);
+  const double2  *xy   = MV_TAB(const double2, M.off_xy);
   const uint32_t *cs   = MV_CTAB(uint32_t, H.offc_cs);
   const double   *rcp  = MV_CTAB(double, H.offc_rcp);
   const double inf = __longlong_as_double(0x7FF0000000000000ll);
   EvalOut out; out.feasible = false; out.cost = out.path = out.makespan = inf;
 
-  // position s of the worker's sequence -> index into the incumbent's sequence
+  // position p of the worker's sequence -> index into the incumbent's sequence
   const uint32_t lo = min(mv.a, mv.c), span = max(mv.a, mv.c) + mv.len - lo;
   const uint32_t shift = (mv.c <= mv.a) ? (0u - mv.len) : mv.len;
+  const uint32_t c_end = mv.c + mv.len;
   const bool fld = (mv.fld_b != kNone);
 
-  // ---- S4 pass 1 (L69, L106, L213): route, area, supplies, sum over BPs of the mean field->BP leg
+  // ---- S4 pass 1 (L69, L106, L213): route, area, supplies, sum over BPs of the mean field->BP leg.
+  // The HU leg of position p comes from the incumbent's table unless the worker's predecessor differs:
+  // at the moved block's first position, right after it, and right after the gap it left.
   for (uint32_t g = 0; g < n_t; ++g) { s.d(M.m64_lt + g) = 0.0; s.d(M.m64_e + g) = 0.0; s.w(M.m32_hq + g) = 0u; s.w(M.m32_ng + g) = 0u; }
   bool feas = (mv.bad == 0u);
   {
-    uint32_t b_cur = kNone, g_cur = 0, Sq = 0, Hq = 0, k = 0, m = 0, prev = 0 /* HQ */;
+    uint32_t b_cur = kNone, g_cur = 0, Sq = 0, Hq = 0, k = 0, m = 0, prev = 0 /* HQ */, idx_prev = kNone;
     double Lt = 0.0, sd = 0.0, sumE = 0.0;
     for (uint32_t p = 0; p < n_f; ++p) {
       uint32_t idx = p; bool inb = false;
       if (p - lo < span) { const uint32_t o = p - mv.c; inb = o < mv.len; idx = inb ? mv.a + o : p + shift; }
-      const uint32_t en = seq[idx];
-      const uint32_t f = en & 0xFFFFu;
-      uint32_t b = en >> 16;
-      if (inb && fld) b = mv.fld_b;
+      const uint4 en = pos4[idx];
+      const double2 lg = leg2[idx];
+      const uint32_t f = en.x & 0xFFFFu;
+      uint32_t b = en.x >> 16;
+      const bool moved_f = inb && fld;
+      if (moved_f) b = mv.fld_b;
       if (b != b_cur) {
-        const uint32_t g = (b == mv.mv_b) ? mv.mv_t : ((bp[b].y >> 8) & 0xFFu);
+        const uint32_t g = (b == mv.mv_b) ? mv.mv_t : (moved_f ? mv.fld_g : en.w);
         if (b_cur != kNone) {
           feas = feas && (Sq >= dq[b_cur]);                                  // eq. (2)
           sumE = __dadd_rn(sumE, div_small(sd, k, rcp)); ++m;                // R10: only BPs with fields
           if (g != g_cur) {                                                  // the tour is complete: back to HQ (L21; R2)
-            const double leg = COORDS_H ? edge_from_xy(xy, prev + n_b, 0u) : dtri[(prev * (prev - 1u)) >> 1];
-            s.d(M.m64_lt + g_cur) = __dadd_rn(Lt, leg); s.w(M.m32_hq + g_cur) = Hq;
+            s.d(M.m64_lt + g_cur) = __dadd_rn(Lt, edge_from_xy(xy, prev + n_b, 0u)); s.w(M.m32_hq + g_cur) = Hq;
             s.d(M.m64_e + g_cur) = sumE; s.w(M.m32_ng + g_cur) = m;
             Lt = 0.0; Hq = 0u; sumE = 0.0; m = 0u; prev = 0u;
           }
         }
         g_cur = g; b_cur = b; sd = 0.0; Sq = 0u; k = 0u;
       }
-      const uint2 qf = sh[f];
       const uint32_t cur = f + 1u;
-      double leg_h, leg_b;
-      if (COORDS_H) leg_h = edge_from_xy(xy, prev ? prev + n_b : 0u, cur + n_b);
-      else { const uint32_t hi = max(prev, cur), lw = min(prev, cur); leg_h = dtri[((hi * (hi - 1u)) >> 1) + lw]; }
-      if (COORDS_B) leg_b = edge_from_xy(xy, cur + n_b, 1u + b);
-      else leg_b = dfb[f * n_b + b];
+      double leg_h = lg.x, leg_b = lg.y;
+      if (p == mv.c || p == c_end || idx != idx_prev + 1u) leg_h = edge_from_xy(xy, prev ? prev + n_b : 0u, cur + n_b);
+      if (moved_f) leg_b = edge_from_xy(xy, cur + n_b, 1u + b);
+      idx_prev = idx;
       Lt = __dadd_rn(Lt, leg_h);                                             // field to field (L69)
       prev = cur;
-      Hq += qf.y; Sq += qf.x; ++k;
+      Hq += en.z; Sq += en.y; ++k;
       sd = __dadd_rn(sd, leg_b);
     }
     feas = feas && (Sq >= dq[b_cur]);
     sumE = __dadd_rn(sumE, div_small(sd, k, rcp)); ++m;
-    const double leg = COORDS_H ? edge_from_xy(xy, prev + n_b, 0u) : dtri[(prev * (prev - 1u)) >> 1];
-    s.d(M.m64_lt + g_cur) = __dadd_rn(Lt, leg); s.w(M.m32_hq + g_cur) = Hq;
+    s.d(M.m64_lt + g_cur) = __dadd_rn(Lt, edge_from_xy(xy, prev + n_b, 0u)); s.w(M.m32_hq + g_cur) = Hq;
     s.d(M.m64_e + g_cur) = sumE; s.w(M.m32_ng + g_cur) = m;
   }
   if (!feas) return out;                                                     // discarded (L186; R19)
@@ -381,18 +406,18 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
     s.d(M.m64_w + g) = 0.0;                                                  // T_wait is dead: the row holds the shuttle sum
   }
   {
-    const uint32_t *sq = MV_CTAB(uint32_t, H.offc_s);
     uint32_t b_cur = kNone, g_cur = 0, n_g = 0, C_g = 1, magic = 0;
     double shut = 0.0;
     for (uint32_t p = 0; p < n_f; ++p) {
       uint32_t idx = p; bool inb = false;
       if (p - lo < span) { const uint32_t o = p - mv.c; inb = o < mv.len; idx = inb ? mv.a + o : p + shift; }
-      const uint32_t en = seq[idx];
-      const uint32_t f = en & 0xFFFFu;
-      uint32_t b = en >> 16;
-      if (inb && fld) b = mv.fld_b;
+      const uint4 en = pos4[idx];
+      double leg = leg2[idx].y;
+      uint32_t b = en.x >> 16;
+      const bool moved_f = inb && fld;
+      if (moved_f) { b = mv.fld_b; leg = edge_from_xy(xy, 1u + n_b + (en.x & 0xFFFFu), 1u + b); }
       if (b != b_cur) {
-        const uint32_t g = (b == mv.mv_b) ? mv.mv_t : ((bp[b].y >> 8) & 0xFFu);
+        const uint32_t g = (b == mv.mv_b) ? mv.mv_t : (moved_f ? mv.fld_g : en.w);
         if (b_cur == kNone || g != g_cur) {
           if (b_cur != kNone) { s.d(M.m64_w + g_cur) = shut; shut = 0.0; }
           n_g = s.w(M.m32_ng + g); C_g = s.w(M.m32_s + g); magic = s.w(M.m32_magic + g);
@@ -400,12 +425,11 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
         }
         b_cur = b;
       }
-      const uint32_t xq = sq[f] * n_g + (C_g - 1u);
+      const uint32_t xq = en.y * n_g + (C_g - 1u);
       uint32_t N = __umulhi(xq, magic);
       uint32_t rem = xq - N * C_g;
       if (rem >= C_g) { ++N; rem -= C_g; }
       if (rem >= C_g) { ++N; }
-      const double leg = COORDS_B ? edge_from_xy(xy, 1u + n_b + f, 1u + b) : dfb[f * n_b + b];
       shut = __dadd_rn(shut, __dmul_rn((double)N, leg));
     }
     s.d(M.m64_w + g_cur) = shut;
@@ -430,12 +454,15 @@ __device__ __forceinline__ void mv_prologue(const MvParams &P, uint8_t *sm, St &
 {
   const ImgHdr &H = P.H; const MvHdr &M = P.M;
   {
-    const uint4 *src = reinterpret_cast<const uint4 *>(P.image);
-    uint4 *dst = reinterpret_cast<uint4 *>(sm);
-    for (uint32_t i = tid; i < H.image_bytes / 16u; i += T) dst[i] = src[i];
-    src = reinterpret_cast<const uint4 *>(P.image_c + H.offc_s);
+    const uint4 *src = reinterpret_cast<const uint4 *>(P.xy);
+    uint4 *dst = reinterpret_cast<uint4 *>(sm + M.off_xy);
+    for (uint32_t i = tid; i < 1u + (uint32_t)H.n_b + (uint32_t)H.n_f; i += T) dst[i] = src[i];
+    const uint32_t *dqg = reinterpret_cast<const uint32_t *>(P.image + H.off_dq);
+    uint32_t *dqs = reinterpret_cast<uint32_t *>(sm + M.off_dq);
+    for (uint32_t i = tid; i < (uint32_t)H.n_b; i += T) dqs[i] = dqg[i];
+    src = reinterpret_cast<const uint4 *>(P.image_c + H.offc_cs);
     dst = reinterpret_cast<uint4 *>(sm + M.off_c);
-    for (uint32_t i = tid; i < (H.imagec_bytes - H.offc_s) / 16u; i += T) dst[i] = src[i];
+    for (uint32_t i = tid; i < (H.imagec_bytes - H.offc_cs) / 16u; i += T) dst[i] = src[i];
   }
   s.T4 = 4u * T; s.T8 = 8u * T;
   s.b64 = sm + M.off_state + 8u * tid;
@@ -445,7 +472,7 @@ __device__ __forceinline__ void mv_prologue(const MvParams &P, uint8_t *sm, St &
 
 // ================================================================== batch kernel (L163-165)
 
-template <int DM, int MASKW>
+template <int MASKW>
 __global__ void __launch_bounds__(kMvThreads, 1) lgx_move_eval_k(const __grid_constant__ MvParams P)
 {
   extern __shared__ __align__(16) uint8_t smem[];
@@ -462,7 +489,7 @@ __global__ void __launch_bounds__(kMvThreads, 1) lgx_move_eval_k(const __grid_co
     uint32_t w[4];
     philox_block(P, (uint32_t)id, (uint32_t)(id >> 32), 5u, 0u, w);
     const Move mv = mv_derive(P, sm, w[0], w[1], w[2], nullptr);
-    const EvalOut r = mv_eval<DM, MASKW>(P, sm, s, mv);
+    const EvalOut r = mv_eval<MASKW>(P, sm, s, mv);
     if (P.cost)       P.cost[i] = r.cost;
     if (P.path_km)    P.path_km[i] = r.path;
     if (P.makespan_h) P.makespan_h[i] = r.makespan;
@@ -472,7 +499,7 @@ __global__ void __launch_bounds__(kMvThreads, 1) lgx_move_eval_k(const __grid_co
 
 // ================================================================== Algorithm 1 steps 4-16, persistent
 
-template <int DM, int MASKW>
+template <int MASKW>
 __global__ void __launch_bounds__(kMvThreads, 1) lgx_local_search_k(const __grid_constant__ MvParams P)
 {
   extern __shared__ __align__(16) uint8_t smem[];
@@ -496,7 +523,7 @@ __global__ void __launch_bounds__(kMvThreads, 1) lgx_local_search_k(const __grid
   mv_load_plan<MASKW>(P, sm, x_best, tid, T);
   mv_encode<MASKW>(P, sm, x_best, tid, T);
   if (tid == 0) {
-    const EvalOut r = mv_eval<DM, MASKW>(P, sm, s, mv_identity(P, sm));
+    const EvalOut r = mv_eval<MASKW>(P, sm, s, mv_identity(P, sm));
     s_cstar = (unsigned long long)__double_as_longlong(r.cost);
     if (r.feasible) {
       uint64_t *mk = reinterpret_cast<uint64_t *>(x_best + M.pl_mask);
@@ -523,7 +550,7 @@ __global__ void __launch_bounds__(kMvThreads, 1) lgx_local_search_k(const __grid
       uint32_t w[4];
       philox_block(P, (uint32_t)id, (uint32_t)(id >> 32), 5u, 0u, w);
       const Move mv = mv_derive(P, sm, w[0], w[1], w[2], nullptr);
-      const EvalOut r = mv_eval<DM, MASKW>(P, sm, s, mv);
+      const EvalOut r = mv_eval<MASKW>(P, sm, s, mv);
       const unsigned long long bits = (unsigned long long)__double_as_longlong(r.cost);
       if (bits < best_bits || (bits == best_bits && id < best_id)) {
         best_bits = bits; best_id = id;
