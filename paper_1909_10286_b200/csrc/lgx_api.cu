@@ -357,8 +357,11 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
     M.off_cnt = o;   o = align16(o + 4u * (uint32_t)nb);
     M.off_tpl = o;   o = align16(o + 4u * (uint32_t)nt);
     M.off_thu = o;   o = align16(o + 8u * (uint32_t)nt);
-    M.off_ts = o;    o = align16(o + 4u * (uint32_t)nt);
+    M.off_tsn = o;   o = align16(o + 8u * (uint32_t)nt);
     M.off_tmask = o; o = align16(o + 8u * (uint32_t)nt * MW);
+    M.off_trng = o;  o = align16(o + 8u * (uint32_t)nt);
+    M.off_tst = o;   o = align16(o + 40u * (uint32_t)nt);
+    M.off_tbad = o;  o = align16(o + 4u * (uint32_t)nt);
     M.off_misc = o;  o = align16(o + 64u);
     uint32_t q = 0;
     q += (uint32_t)nb; M.pl_bpos = q; q += (uint32_t)nb; q = (q + 1u) & ~1u;
@@ -368,16 +371,16 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
     M.off_plans = o; o += 3u * M.plan_bytes;
     M.off_state = o;
     uint32_t r = 0;
-    M.m64_lt = r; r += (uint32_t)nt; M.m64_e = r; r += (uint32_t)nt; M.m64_w = r; r += (uint32_t)nt;
+    M.m64_w = r; r += (uint32_t)nt;
     M.m64_mask = r; r += (uint32_t)nt * MW; M.m64_bmask = r; r += (uint32_t)nt * MW; M.m64_rows = r;
     r = 0;
-    M.m32_hq = r; r += (uint32_t)nt; M.m32_s = r; r += (uint32_t)nt; M.m32_ng = r; r += (uint32_t)nt;
-    M.m32_magic = r; r += (uint32_t)nt; M.m32_rows = r;
+    M.m32_s = r; r += (uint32_t)nt; M.m32_rows = r;
     M.slot_words = 2u + (uint32_t)nt * MW;
     const int64_t mv_state = 8ll * M.m64_rows + 4ll * M.m32_rows;
     int64_t tm = (budget - 256 - (int64_t)M.off_state) / mv_state;      // static smem of the reductions
     tm = std::min<int64_t>(tm, kMvThreads) / 32 * 32;
     if (const char *ev = std::getenv("LGX_THREADS_MV")) { const int v = std::atoi(ev); if (v >= 64 && v <= tm) tm = v / 32 * 32; }
+    if (nt > 64) tm = 0;                                                  // the workers keep a 64-bit set of tours
     I->threads_mv = tm >= 64 ? (int)tm : 0;                               // 0: the move kernels do not fit (LGX_ETOOBIG there)
     I->smem_mv = (size_t)M.off_state + (size_t)mv_state * (size_t)std::max<int64_t>(tm, 0);
     std::vector<double> xy(2 * (size_t)(1 + nb + nf));

@@ -43,7 +43,7 @@ struct MvHdr {
   uint32_t off_xy;      // f64x2 [1 + n_b + n_f]  vertex coordinates: HQ, BPs, fields
   uint32_t off_dq;      // u32 [n_b]      demand quanta
   uint32_t off_c;       // tail of image C: byte x of image C (x >= offc_cs) sits at off_c + x - offc_cs
-  uint32_t off_pos4;    // u32x4 [n_f]    plan order: f | b << 16, s_q[f], h_q[f], tour of b
+  uint32_t off_pos4;    // u32x4 [n_f]    plan order: f | b << 16, s_q[f], h_q[f], shuttle count N under the incumbent's SU sets
   uint32_t off_leg2;    // f64x2 [n_f]    plan order: D(predecessor on the tour or HQ, f), D(f, b)
   uint32_t off_posf;    // u16 [n_f]      position of field f in plan order
   uint32_t off_bp;      // u32x2 [n_b]    x = start | len << 16;  y = plan index | tour << 8 | pos << 16
@@ -52,15 +52,18 @@ struct MvHdr {
   uint32_t off_cnt;     // u32 [n_b]      scratch: fields per BP
   uint32_t off_tpl;     // u32 [n_t]      first plan index | BPs on the tour << 8
   uint32_t off_thu;     // u32x2 [n_t]    n_HU(g), R_g (fixed during a search: R20)
-  uint32_t off_ts;      // u32 [n_t]      S_g = capacity quanta of the tour's SUs
+  uint32_t off_tsn;     // u32x2 [n_t]    S_g = capacity quanta of the tour's SUs, n_g = their number
   uint32_t off_tmask;   // u64 [n_t*MW]   SU membership by capacity rank
-  uint32_t off_misc;    // u32 [16]       [0] empty BPs with positive demand; [4..9] the move being applied
+  uint32_t off_trng;    // u32x2 [n_t]    the tour's positions [begin, end) in plan order
+  uint32_t off_tst;     // f64 [5][n_t]   the incumbent's L_tour(g), E(g), T(g), T_wait(g), shuttle sum(g)
+  uint32_t off_tbad;    // u32 [n_t]      BPs of the tour that have fields but miss their demand
+  uint32_t off_misc;    // u32 [16]       [0] BPs without fields but with demand; [1] sum of tbad; [4..9] the move being applied
   uint32_t off_plans;   // 3 plans (x*, x_old, scratch); the batch kernel uses the first
   uint32_t plan_bytes;  // one plan: bp_tour u8[n_b] | bp_pos u8[n_b] | field_bp u16[n_f] | field_pos u16[n_f] | masks u64[n_t*MW]
   uint32_t pl_bpos, pl_fbp, pl_fpos, pl_mask;
   uint32_t off_state;   // per-thread rows (64-bit region, then 32-bit region)
-  uint32_t m64_lt, m64_e, m64_w, m64_mask, m64_bmask, m64_rows;
-  uint32_t m32_hq, m32_s, m32_ng, m32_magic, m32_rows;
+  uint32_t m64_w, m64_mask, m64_bmask, m64_rows;
+  uint32_t m32_s, m32_rows;
   uint32_t slot_words;  // 64-bit words per block slot: cost bits, id, masks
   uint32_t pad_[3];
 };
@@ -85,6 +88,18 @@ struct MvParams {
 
 #define MV_TAB(type, off) (reinterpret_cast<type *>(sm + (off)))
 #define MV_CTAB(type, offc) (reinterpret_cast<const type *>(sm + (P.M.off_c + ((offc) - P.H.offc_cs))))
+
+// eq. (4) (L89) with the tour's mean capacity (R4): N = ceil(s_q n_g / C_g) = floor(x'/C_g), x' = s_q n_g + C_g - 1 < 2^32;
+// q = mulhi(x', floor((2^32-1)/C_g)) is at most 2 below; two conditional increments fix it.
+__device__ __forceinline__ uint32_t shuttle_count(uint32_t s_q, uint32_t n_g, uint32_t C_g, uint32_t magic)
+{
+  const uint32_t xq = s_q * n_g + (C_g - 1u);
+  uint32_t N = __umulhi(xq, magic);
+  uint32_t rem = xq - N * C_g;
+  if (rem >= C_g) { ++N; rem -= C_g; }
+  if (rem >= C_g) { ++N; }
+  return N;
+}
 
 // ------------------------------------------------------------------ plan -> shared memory
 
@@ -111,7 +126,8 @@ __device__ void mv_load_plan(const MvParams &P, uint8_t *sm, uint8_t *plan, uint
   __syncthreads();
 }
 
-// Incumbent tables from a plan slot (block-wide; ends with a barrier).
+// Incumbent tables from a plan slot (block-wide; ends with a barrier): the flat sequence with its legs and
+// shuttle counts, and per tour everything a worker needs of the tours its move does not touch.
 template <int MASKW>
 __device__ void mv_encode(const MvParams &P, uint8_t *sm, const uint8_t *plan, uint32_t tid, uint32_t T)
 {
@@ -120,8 +136,15 @@ __device__ void mv_encode(const MvParams &P, uint8_t *sm, const uint8_t *plan, u
   const uint8_t *p_bt = plan, *p_bp = plan + M.pl_bpos;
   const uint16_t *p_fb = reinterpret_cast<const uint16_t *>(plan + M.pl_fbp), *p_fp = reinterpret_cast<const uint16_t *>(plan + M.pl_fpos);
   const uint64_t *p_mk = reinterpret_cast<const uint64_t *>(plan + M.pl_mask);
+  const uint32_t *dq = MV_TAB(const uint32_t, M.off_dq);
+  const uint32_t *cs = MV_CTAB(uint32_t, H.offc_cs);
+  const double   *rcp = MV_CTAB(double, H.offc_rcp);
   uint32_t *cnt = MV_TAB(uint32_t, M.off_cnt);
   uint2 *bp = MV_TAB(uint2, M.off_bp);
+  uint2 *trng = MV_TAB(uint2, M.off_trng);
+  uint2 *tsn = MV_TAB(uint2, M.off_tsn);
+  uint64_t *tmask = MV_TAB(uint64_t, M.off_tmask);
+  uint32_t *misc = MV_TAB(uint32_t, M.off_misc);
   for (uint32_t b = tid; b < n_b; b += T) cnt[b] = 0u;
   __syncthreads();
   for (uint32_t f = tid; f < n_f; f += T) atomicAdd(&cnt[p_fb[f]], 1u);
@@ -130,7 +153,6 @@ __device__ void mv_encode(const MvParams &P, uint8_t *sm, const uint8_t *plan, u
     uint32_t *tpl = MV_TAB(uint32_t, M.off_tpl);
     uint16_t *pre = MV_TAB(uint16_t, M.off_pre);
     uint8_t *bpat = MV_TAB(uint8_t, M.off_bpat);
-    const uint32_t *dq = MV_TAB(const uint32_t, M.off_dq);
     for (uint32_t g = 0; g < n_t; ++g) tpl[g] = 0u;
     for (uint32_t b = 0; b < n_b; ++b) tpl[p_bt[b]] += 0x100u;
     uint32_t acc = 0;
@@ -145,21 +167,20 @@ __device__ void mv_encode(const MvParams &P, uint8_t *sm, const uint8_t *plan, u
       if (len == 0u && dq[b] > 0u) ++n_bad;                    // a BP without fields fails eq. (2) unless it needs nothing
     }
     pre[n_b] = (uint16_t)acc;
-    MV_TAB(uint32_t, M.off_misc)[0] = n_bad;
+    misc[0] = n_bad;
+    for (uint32_t g = 0; g < n_t; ++g) { const uint32_t j0 = tpl[g] & 0xFFu, j1 = j0 + (tpl[g] >> 8); trng[g] = make_uint2(pre[j0], pre[j1]); }
   }
   if (tid >= 32u) {
-    const uint32_t *cs = MV_CTAB(uint32_t, H.offc_cs);
-    uint64_t *tmask = MV_TAB(uint64_t, M.off_tmask);
-    uint32_t *ts = MV_TAB(uint32_t, M.off_ts);
     for (uint32_t g = tid - 32u; g < n_t; g += T - 32u) {
-      uint32_t S = 0;
+      uint32_t S = 0, n = 0;
 #pragma unroll
       for (int i = 0; i < MASKW; ++i) {
         uint64_t w = p_mk[g * MASKW + i];
         tmask[g * MASKW + i] = w;
+        n += (uint32_t)__popcll(w);
         while (w) { const int r = __ffsll((long long)w) - 1; w &= w - 1; S += cs[64 * i + r]; }
       }
-      ts[g] = S;
+      tsn[g] = make_uint2(S, n);
     }
   }
   __syncthreads();
@@ -171,7 +192,8 @@ __device__ void mv_encode(const MvParams &P, uint8_t *sm, const uint8_t *plan, u
     const uint2 bb = bp[b];
     const uint32_t pos = (bb.x & 0xFFFFu) + p_fp[f];
     const uint2 q = sh[f];
-    pos4[pos] = make_uint4(f | (b << 16), q.x, q.y, (bb.y >> 8) & 0xFFu);
+    const uint2 sn = tsn[(bb.y >> 8) & 0xFFu];
+    pos4[pos] = make_uint4(f | (b << 16), q.x, q.y, shuttle_count(q.x, sn.y, sn.x, 0xFFFFFFFFu / sn.x));
     posf[f] = (uint16_t)pos;
   }
   __syncthreads();
@@ -182,9 +204,51 @@ __device__ void mv_encode(const MvParams &P, uint8_t *sm, const uint8_t *plan, u
     const uint4 e = pos4[p];
     const uint32_t f = e.x & 0xFFFFu, b = e.x >> 16;
     uint32_t pred = 0u;                                                        // HQ: first field of its tour (L21)
-    if (p > 0u) { const uint4 ep = pos4[p - 1u]; if (ep.w == e.w) pred = 1u + n_b + (ep.x & 0xFFFFu); }
+    if (p > 0u) { const uint4 ep = pos4[p - 1u]; if (((bp[ep.x >> 16].y ^ bp[b].y) & 0xFF00u) == 0u) pred = 1u + n_b + (ep.x & 0xFFFFu); }
     leg2[p] = make_double2(edge_from_xy(xy, pred, 1u + n_b + f), edge_from_xy(xy, 1u + n_b + f, 1u + b));
   }
+  __syncthreads();
+  // per tour, one lane each: the walk of DESIGN.md S4 / S7 over the tour's positions, in order
+  {
+    const uint2 *thu = MV_TAB(const uint2, M.off_thu);
+    double *tst = MV_TAB(double, M.off_tst);
+    uint32_t *tbad = MV_TAB(uint32_t, M.off_tbad);
+    const uint32_t n_warps = T >> 5;
+    if ((tid & 31u) == 0u)
+      for (uint32_t g = tid >> 5; g < n_t; g += n_warps) {
+        const uint2 r = trng[g];
+        double Lt = 0.0, sd = 0.0, sumE = 0.0, shut = 0.0;
+        uint32_t Hq = 0, Sq = 0, k = 0, m = 0, bad = 0, b_cur = kNone, f_last = 0;
+        for (uint32_t p = r.x; p < r.y; ++p) {
+          const uint4 e = pos4[p]; const double2 lg = leg2[p];
+          const uint32_t b = e.x >> 16;
+          if (b != b_cur) {
+            if (b_cur != kNone) { bad += (Sq < dq[b_cur]) ? 1u : 0u; sumE = __dadd_rn(sumE, div_small(sd, k, rcp)); ++m; }
+            b_cur = b; sd = 0.0; Sq = 0u; k = 0u;
+          }
+          Lt = __dadd_rn(Lt, lg.x); sd = __dadd_rn(sd, lg.y); Hq += e.z; Sq += e.y; ++k;
+          shut = __dadd_rn(shut, __dmul_rn((double)e.w, lg.y));
+          f_last = e.x & 0xFFFFu;
+        }
+        double E = 0.0;
+        if (b_cur != kNone) {
+          bad += (Sq < dq[b_cur]) ? 1u : 0u; sumE = __dadd_rn(sumE, div_small(sd, k, rcp)); ++m;
+          Lt = __dadd_rn(Lt, edge_from_xy(xy, 1u + n_b + f_last, 0u));
+          E = __ddiv_rn(__dmul_rn(2.0, div_small(sumE, m, rcp)), H.v_su);
+        }
+        const uint2 hu = thu[g]; const uint2 sn = tsn[g];
+        Mask<MASKW> mk;
+#pragma unroll
+        for (int i = 0; i < MASKW; ++i) mk.w[i] = tmask[g * MASKW + i];
+        tst[g] = Lt; tst[n_t + g] = E;
+        tst[2u * n_t + g] = __dadd_rn(__ddiv_rn(Lt, H.v_hu), __ddiv_rn((double)Hq, (double)hu.y));
+        tst[3u * n_t + g] = wait_time(E, sn.x, cs[mask_top(mk)], hu.x, H.kappa, rcp);
+        tst[4u * n_t + g] = shut;
+        tbad[g] = bad;
+      }
+  }
+  __syncthreads();
+  if (tid == 0) { const uint32_t *tbad = MV_TAB(const uint32_t, M.off_tbad); uint32_t a = 0; for (uint32_t g = 0; g < n_t; ++g) a += tbad[g]; misc[1] = a; }
   __syncthreads();
 }
 
@@ -193,10 +257,8 @@ __device__ void mv_encode(const MvParams &P, uint8_t *sm, const uint8_t *plan, u
 // The moved block [a, a+len) of the incumbent's sequence reappears at position c of the worker's sequence.
 struct Move {
   uint32_t a, len, c;
-  uint32_t fld_b;     // field move: the BP the moved field now belongs to (on tour fld_g); else kNone
-  uint32_t fld_g;
-  uint32_t mv_b;      // BP move: the BP whose tour changes (to mv_t); else kNone
-  uint32_t mv_t;
+  uint32_t fld_b;     // field move: the BP the moved field now belongs to; else kNone
+  uint32_t g1, g2;    // the tours the move touches: source and target (kNone, kNone: no move)
   uint32_t bad;       // BPs without fields but with positive demand under this move
 };
 
@@ -220,7 +282,7 @@ __device__ __forceinline__ Move mv_derive(const MvParams &P, const uint8_t *sm, 
     const uint32_t len_t = bt.x >> 16, start_t = bt.x & 0xFFFFu, len_A = bA.x >> 16;
     const uint32_t q = __umulhi(w2, len_t - (A == t ? 1u : 0u) + 1u);
     m.a = a; m.len = 1u; m.c = start_t - (a < start_t ? 1u : 0u) + q;
-    m.fld_b = t; m.fld_g = (bt.y >> 8) & 0xFFu; m.mv_b = kNone; m.mv_t = 0u;
+    m.fld_b = t; m.g1 = (bA.y >> 8) & 0xFFu; m.g2 = (bt.y >> 8) & 0xFFu;
     m.bad = n_bad - ((len_t == 0u && dq[t] > 0u) ? 1u : 0u) + ((len_A == 1u && A != t && dq[A] > 0u) ? 1u : 0u);
     if (raw) { raw[0] = 0u; raw[1] = v; raw[2] = A; raw[3] = a - (bA.x & 0xFFFFu); raw[4] = t; raw[5] = q; }
   } else {
@@ -235,7 +297,7 @@ __device__ __forceinline__ Move mv_derive(const MvParams &P, const uint8_t *sm, 
     const uint16_t *pre = MV_TAB(const uint16_t, M.off_pre);
     m.a = bb.x & 0xFFFFu; m.len = len;
     m.c = (jq <= j) ? (uint32_t)pre[jq] : (uint32_t)pre[jq + 1u] - len;
-    m.fld_b = kNone; m.fld_g = 0u; m.mv_b = b; m.mv_t = t;
+    m.fld_b = kNone; m.g1 = g; m.g2 = t;
     m.bad = n_bad;
     if (raw) { raw[0] = 1u; raw[1] = b; raw[2] = g; raw[3] = (bb.y >> 16) & 0xFFu; raw[4] = t; raw[5] = q; }
   }
@@ -244,7 +306,7 @@ __device__ __forceinline__ Move mv_derive(const MvParams &P, const uint8_t *sm, 
 
 __device__ __forceinline__ Move mv_identity(const MvParams &P, const uint8_t *sm)
 {
-  Move m; m.a = m.len = m.c = 0u; m.fld_b = m.mv_b = kNone; m.fld_g = m.mv_t = 0u;
+  Move m; m.a = m.len = m.c = 0u; m.fld_b = m.g1 = m.g2 = kNone;
   m.bad = MV_TAB(const uint32_t, P.M.off_misc)[0];
   return m;
 }
@@ -253,14 +315,23 @@ __device__ __forceinline__ Move mv_identity(const MvParams &P, const uint8_t *sm
 
 struct EvalOut { bool feasible; double cost, path, makespan; };
 
+// Delta evaluation, exact: a tour the move does not touch keeps the incumbent's L_tour, E, T, T_wait (same
+// operands, same order, same bits), so the worker walks only the <= 2 touched tours in pass 1, and in pass 2
+// those plus the tours whose SU set Algorithm 2 changed.  Within a walked tour every position whose predecessor
+// is the incumbent's reads its legs (and, under an unchanged SU set, its shuttle count) from the tables.
 template <int MASKW>
 __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm, const St &s, const Move &mv)
 {
   const ImgHdr &H = P.H; const MvHdr &M = P.M;
-  const uint32_t n_f = H.n_f, n_b = H.n_b, n_t = H.n_t, n_su = H.n_su;
+  const uint32_t n_b = H.n_b, n_t = H.n_t, n_su = H.n_su;
   const uint4    *pos4 = MV_TAB(const uint4, M.off_pos4);
   const double2  *leg2 = MV_TAB(const double2, M.off_leg2);
   const uint2    *thu  = MV_TAB(const uint2, M.off_thu);
+  const uint2    *tsn  = MV_TAB(const uint2, M.off_tsn);
+  const uint2    *trng = MV_TAB(const uint2, M.off_trng);
+  const double   *tst  = MV_TAB(const double, M.off_tst);
+  const uint32_t *tbad = MV_TAB(const uint32_t, M.off_tbad);
+  const uint64_t *tmask = MV_TAB(const uint64_t, M.off_tmask);
   const uint32_t *dq   = MV_TAB(const uint32_t, M.off_dq);
   const double2  *xy   = MV_TAB(const double2, M.off_xy);
   const uint32_t *cs   = MV_CTAB(uint32_t, H.offc_cs);
@@ -268,79 +339,90 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
   const double inf = __longlong_as_double(0x7FF0000000000000ll);
   EvalOut out; out.feasible = false; out.cost = out.path = out.makespan = inf;
 
-  // position p of the worker's sequence -> index into the incumbent's sequence
-  const uint32_t lo = min(mv.a, mv.c), span = max(mv.a, mv.c) + mv.len - lo;
-  const uint32_t shift = (mv.c <= mv.a) ? (0u - mv.len) : mv.len;
-  const uint32_t c_end = mv.c + mv.len;
+  const uint32_t L = mv.len;
+  const uint32_t ga = min(mv.g1, mv.g2), gb = max(mv.g1, mv.g2);
+  const uint32_t nr = (mv.g1 == kNone) ? 0u : (ga == gb ? 1u : 2u);
   const bool fld = (mv.fld_b != kNone);
+  // worker position -> incumbent index: p -> p outside [lo, lo+span); three breakpoints (Q, K) inside, ascending
+  const uint32_t lo = min(mv.a, mv.c), span = max(mv.a, mv.c) + L - lo;
+  const uint32_t shift = (mv.c <= mv.a) ? (0u - L) : L;
+  uint32_t Q1, K1, Q2, K2, Q3, K3;
+  if (mv.c <= mv.a) { Q1 = mv.c; K1 = mv.a; Q2 = mv.c + L; K2 = mv.c; Q3 = mv.a + L; K3 = mv.a + L; }
+  else              { Q1 = mv.a; K1 = mv.a + L; Q2 = mv.c; K2 = mv.a; Q3 = mv.c + L; K3 = mv.c + L; }
+  auto map_idx = [&](uint32_t p) -> uint32_t {
+    if (p - lo < span) { const uint32_t o = p - mv.c; return (o < L) ? mv.a + o : p + shift; }
+    return p;
+  };
+  // the worker's positions [wb, we) of tour g
+  auto wrange = [&](uint32_t g, uint32_t &wb, uint32_t &we) {
+    const uint2 r = trng[g];
+    wb = r.x - ((mv.g1 < g) ? L : 0u) + ((mv.g2 < g) ? L : 0u);
+    we = wb + (r.y - r.x) - ((g == mv.g1) ? L : 0u) + ((g == mv.g2) ? L : 0u);
+  };
 
-  // ---- S4 pass 1 (L69, L106, L213): route, area, supplies, sum over BPs of the mean field->BP leg.
-  // The HU leg of position p comes from the incumbent's table unless the worker's predecessor differs:
-  // at the moved block's first position, right after it, and right after the gap it left.
-  for (uint32_t g = 0; g < n_t; ++g) { s.d(M.m64_lt + g) = 0.0; s.d(M.m64_e + g) = 0.0; s.w(M.m32_hq + g) = 0u; s.w(M.m32_ng + g) = 0u; }
-  bool feas = (mv.bad == 0u);
-  {
-    uint32_t b_cur = kNone, g_cur = 0, Sq = 0, Hq = 0, k = 0, m = 0, prev = 0 /* HQ */, idx_prev = kNone;
+  // ---- untouched tours: the incumbent's values
+  double makespan = 0.0;                                                       // every T(g) >= 0
+  for (uint32_t g = 0; g < n_t; ++g) {
+    s.d(M.m64_w + g) = tst[3u * n_t + g];
+    s.w(M.m32_s + g) = tsn[g].x;
+#pragma unroll
+    for (int i = 0; i < MASKW; ++i) s.q(M.m64_mask + MASKW * g + i) = tmask[g * MASKW + i];
+    if (g != ga && g != gb) { const double t_g = tst[2u * n_t + g]; if (t_g > makespan) makespan = t_g; }
+  }
+
+  // ---- S4 pass 1 over the touched tours (L69, L106, L213); eq. (2) (L79)
+  uint32_t bad = mv.bad + MV_TAB(const uint32_t, M.off_misc)[1];
+  double lt_a = 0.0, lt_b = 0.0, E_a = 0.0, E_b = 0.0;
+  for (uint32_t r = 0; r < nr; ++r) {
+    const uint32_t g = r ? gb : ga;
+    bad -= tbad[g];
+    uint32_t p, pe;
+    wrange(g, p, pe);
+    uint32_t P0 = p, J0 = map_idx(p), P1 = Q1, J1 = K1, P2 = Q2, J2 = K2, P3 = Q3, J3 = K3;
+    while (P1 < p) { P1 = P2; J1 = J2; P2 = P3; J2 = J3; P3 = kNone; }
+    uint32_t b_cur = kNone, Sq = 0, Hq = 0, k = 0, m = 0, prev_x = kNone /* HQ */, idx = 0;
     double Lt = 0.0, sd = 0.0, sumE = 0.0;
-    for (uint32_t p = 0; p < n_f; ++p) {
-      uint32_t idx = p; bool inb = false;
-      if (p - lo < span) { const uint32_t o = p - mv.c; inb = o < mv.len; idx = inb ? mv.a + o : p + shift; }
+    for (; p < pe; ++p) {
+      ++idx;
+      bool exc = false;
+      if (p == P0) {
+        do { idx = J0; P0 = P1; J0 = J1; P1 = P2; J1 = J2; P2 = P3; J2 = J3; P3 = kNone; } while (p == P0);
+        exc = true;
+      }
       const uint4 en = pos4[idx];
       const double2 lg = leg2[idx];
-      const uint32_t f = en.x & 0xFFFFu;
       uint32_t b = en.x >> 16;
-      const bool moved_f = inb && fld;
-      if (moved_f) b = mv.fld_b;
-      if (b != b_cur) {
-        const uint32_t g = (b == mv.mv_b) ? mv.mv_t : (moved_f ? mv.fld_g : en.w);
-        if (b_cur != kNone) {
-          feas = feas && (Sq >= dq[b_cur]);                                  // eq. (2)
-          sumE = __dadd_rn(sumE, div_small(sd, k, rcp)); ++m;                // R10: only BPs with fields
-          if (g != g_cur) {                                                  // the tour is complete: back to HQ (L21; R2)
-            s.d(M.m64_lt + g_cur) = __dadd_rn(Lt, edge_from_xy(xy, prev + n_b, 0u)); s.w(M.m32_hq + g_cur) = Hq;
-            s.d(M.m64_e + g_cur) = sumE; s.w(M.m32_ng + g_cur) = m;
-            Lt = 0.0; Hq = 0u; sumE = 0.0; m = 0u; prev = 0u;
-          }
-        }
-        g_cur = g; b_cur = b; sd = 0.0; Sq = 0u; k = 0u;
-      }
-      const uint32_t cur = f + 1u;
       double leg_h = lg.x, leg_b = lg.y;
-      if (p == mv.c || p == c_end || idx != idx_prev + 1u) leg_h = edge_from_xy(xy, prev ? prev + n_b : 0u, cur + n_b);
-      if (moved_f) leg_b = edge_from_xy(xy, cur + n_b, 1u + b);
-      idx_prev = idx;
-      Lt = __dadd_rn(Lt, leg_h);                                             // field to field (L69)
-      prev = cur;
-      Hq += en.z; Sq += en.y; ++k;
+      if (exc) {                                   // the predecessor is not the incumbent's: HQ at the tour's start, or around the moved block
+        const uint32_t vf = 1u + n_b + (en.x & 0xFFFFu);
+        leg_h = edge_from_xy(xy, prev_x == kNone ? 0u : 1u + n_b + (prev_x & 0xFFFFu), vf);
+        if (fld && p == mv.c) { b = mv.fld_b; leg_b = edge_from_xy(xy, vf, 1u + b); }
+      }
+      if (b != b_cur) {
+        if (b_cur != kNone) { bad += (Sq < dq[b_cur]) ? 1u : 0u; sumE = __dadd_rn(sumE, div_small(sd, k, rcp)); ++m; }   // R10
+        b_cur = b; sd = 0.0; Sq = 0u; k = 0u;
+      }
+      Lt = __dadd_rn(Lt, leg_h);                                               // field to field (L69)
       sd = __dadd_rn(sd, leg_b);
+      Hq += en.z; Sq += en.y; ++k;
+      prev_x = en.x;
     }
-    feas = feas && (Sq >= dq[b_cur]);
-    sumE = __dadd_rn(sumE, div_small(sd, k, rcp)); ++m;
-    s.d(M.m64_lt + g_cur) = __dadd_rn(Lt, edge_from_xy(xy, prev + n_b, 0u)); s.w(M.m32_hq + g_cur) = Hq;
-    s.d(M.m64_e + g_cur) = sumE; s.w(M.m32_ng + g_cur) = m;
-  }
-  if (!feas) return out;                                                     // discarded (L186; R19)
-
-  // ---- E(g) = 2 (sumE/m) / v_SU (L199, L213; R9); T_wait(g) (eq. (6)); T(g) = L_tour/v_HU + H_q/R_g (L190; R6)
-  const uint64_t *tmask = MV_TAB(const uint64_t, M.off_tmask);
-  const uint32_t *ts = MV_TAB(const uint32_t, M.off_ts);
-  double makespan = 0.0;
-  for (uint32_t g = 0; g < n_t; ++g) {
-    const uint32_t mm = s.w(M.m32_ng + g);
     double E = 0.0;
-    if (mm > 0u) E = __ddiv_rn(__dmul_rn(2.0, div_small(s.d(M.m64_e + g), mm, rcp)), H.v_su);
-    s.d(M.m64_e + g) = E;
-    Mask<MASKW> mk;
-#pragma unroll
-    for (int i = 0; i < MASKW; ++i) mk.w[i] = tmask[g * MASKW + i];
-    mask_store<MASKW>(s, M.m64_mask + MASKW * g, mk);
-    const uint32_t S = ts[g];
-    s.w(M.m32_s + g) = S;
+    if (b_cur != kNone) {
+      bad += (Sq < dq[b_cur]) ? 1u : 0u; sumE = __dadd_rn(sumE, div_small(sd, k, rcp)); ++m;
+      Lt = __dadd_rn(Lt, edge_from_xy(xy, 1u + n_b + (prev_x & 0xFFFFu), 0u));  // back to HQ (L21; R2)
+      E = __ddiv_rn(__dmul_rn(2.0, div_small(sumE, m, rcp)), H.v_su);          // L199, L213; R9
+    }
     const uint2 hu = thu[g];
-    s.d(M.m64_w + g) = wait_time(E, S, cs[mask_top(mk)], hu.x, H.kappa, rcp);
-    const double t_g = __dadd_rn(__ddiv_rn(s.d(M.m64_lt + g), H.v_hu), __ddiv_rn((double)s.w(M.m32_hq + g), (double)hu.y));
-    if (g == 0u || t_g > makespan) makespan = t_g;
+    const double t_g = __dadd_rn(__ddiv_rn(Lt, H.v_hu), __ddiv_rn((double)Hq, (double)hu.y));   // L190; R6
+    if (t_g > makespan) makespan = t_g;
+    const Mask<MASKW> mk = mask_load<MASKW>(s, M.m64_mask + MASKW * g);
+    s.d(M.m64_w + g) = wait_time(E, tsn[g].x, cs[mask_top(mk)], hu.x, H.kappa, rcp);
+    if (r == 0u) { lt_a = Lt; E_a = E; } else { lt_b = Lt; E_b = E; }
   }
+  if (bad != 0u) return out;                                                   // discarded (L186; R19)
+  auto E_of  = [&](uint32_t g) -> double { return g == ga ? E_a : (g == gb ? E_b : tst[n_t + g]); };
+  auto lt_of = [&](uint32_t g) -> double { return g == ga ? lt_a : (g == gb ? lt_b : tst[g]); };
 
   // ---- S6: Algorithm 2 (L209-227), readings R11-R16 (same procedure as in lgx_finish)
   if (n_t >= 2u) {
@@ -363,7 +445,7 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
       Mask<MASKW> mk_max = mask_load<MASKW>(s, M.m64_mask + MASKW * g_max);
       const uint32_t S_max = s.w(M.m32_s + g_max), M_max = cs[mask_top(mk_max)];
       const uint32_t hu_max = thu[g_max].x;
-      const double   E_max = s.d(M.m64_e + g_max);
+      const double   E_max = E_of(g_max);
       // donor's units by rising fill time (L221): the first that brings T_wait(g_max) below T_wait(g_2nd),
       // else the largest (L225; R13).  The test is monotone in the capacity: bisect over the ranks.
       int r = mask_top(mk_min);
@@ -389,7 +471,7 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
       }
       mask_flip(mk_min, r);
       const uint32_t S_min = s.w(M.m32_s + g_min) - cr;
-      const double w_don = wait_time(s.d(M.m64_e + g_min), S_min, cs[mask_top(mk_min)], thu[g_min].x, H.kappa, rcp);
+      const double w_don = wait_time(E_of(g_min), S_min, cs[mask_top(mk_min)], thu[g_min].x, H.kappa, rcp);
       double new_max = w_new > w_don ? w_new : w_don;                        // step 11 (L227; R14)
       if (!two && w_2nd > new_max) new_max = w_2nd;
       if (!(new_max < w_max)) break;
@@ -399,47 +481,50 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
     }
   }
 
-  // ---- S7 pass 2: shuttles per field, eq. (4) (L89) with the tour's mean capacity (R4)
+  // ---- S7 pass 2: shuttles (eq. (4); R4).  T_wait is dead: its row now holds the tour's shuttle sum.
+  uint64_t need = 0ull;
   for (uint32_t g = 0; g < n_t; ++g) {
-    s.w(M.m32_ng + g)    = (uint32_t)mask_count(mask_load<MASKW>(s, M.m64_mask + MASKW * g));
-    s.w(M.m32_magic + g) = 0xFFFFFFFFu / s.w(M.m32_s + g);
-    s.d(M.m64_w + g) = 0.0;                                                  // T_wait is dead: the row holds the shuttle sum
+    const uint2 sn = tsn[g];
+    const bool same = (s.w(M.m32_s + g) == sn.x) && ((uint32_t)mask_count(mask_load<MASKW>(s, M.m64_mask + MASKW * g)) == sn.y);
+    if (g == ga || g == gb || !same) need |= 1ull << g;
+    else s.d(M.m64_w + g) = tst[4u * n_t + g];
   }
-  {
-    uint32_t b_cur = kNone, g_cur = 0, n_g = 0, C_g = 1, magic = 0;
+  while (need) {
+    const uint32_t g = (uint32_t)__ffsll((long long)need) - 1u;
+    need &= need - 1ull;
+    const uint32_t C_g = s.w(M.m32_s + g), n_g = (uint32_t)mask_count(mask_load<MASKW>(s, M.m64_mask + MASKW * g));
+    const uint32_t magic = 0xFFFFFFFFu / C_g;
+    const uint2 sn = tsn[g];
+    const bool recount = !(C_g == sn.x && n_g == sn.y);
+    uint32_t p, pe;
+    wrange(g, p, pe);
+    uint32_t P0 = p, J0 = map_idx(p), P1 = Q1, J1 = K1, P2 = Q2, J2 = K2, P3 = Q3, J3 = K3;
+    while (P1 < p) { P1 = P2; J1 = J2; P2 = P3; J2 = J3; P3 = kNone; }
+    uint32_t idx = 0;
+    bool inblk = false;
     double shut = 0.0;
-    for (uint32_t p = 0; p < n_f; ++p) {
-      uint32_t idx = p; bool inb = false;
-      if (p - lo < span) { const uint32_t o = p - mv.c; inb = o < mv.len; idx = inb ? mv.a + o : p + shift; }
+    for (; p < pe; ++p) {
+      ++idx;
+      if (p == P0) {
+        do { idx = J0; P0 = P1; J0 = J1; P1 = P2; J1 = J2; P2 = P3; J2 = J3; P3 = kNone; } while (p == P0);
+        inblk = (p - mv.c) < L;                  // the moved block's counts were tabulated under another tour's SU set
+      }
       const uint4 en = pos4[idx];
       double leg = leg2[idx].y;
-      uint32_t b = en.x >> 16;
-      const bool moved_f = inb && fld;
-      if (moved_f) { b = mv.fld_b; leg = edge_from_xy(xy, 1u + n_b + (en.x & 0xFFFFu), 1u + b); }
-      if (b != b_cur) {
-        const uint32_t g = (b == mv.mv_b) ? mv.mv_t : (moved_f ? mv.fld_g : en.w);
-        if (b_cur == kNone || g != g_cur) {
-          if (b_cur != kNone) { s.d(M.m64_w + g_cur) = shut; shut = 0.0; }
-          n_g = s.w(M.m32_ng + g); C_g = s.w(M.m32_s + g); magic = s.w(M.m32_magic + g);
-          g_cur = g;
-        }
-        b_cur = b;
-      }
-      const uint32_t xq = en.y * n_g + (C_g - 1u);
-      uint32_t N = __umulhi(xq, magic);
-      uint32_t rem = xq - N * C_g;
-      if (rem >= C_g) { ++N; rem -= C_g; }
-      if (rem >= C_g) { ++N; }
+      uint32_t N = en.w;
+      if (inblk && fld) leg = edge_from_xy(xy, 1u + n_b + (en.x & 0xFFFFu), 1u + mv.fld_b);
+      if (recount || inblk) N = shuttle_count(en.y, n_g, C_g, magic);
       shut = __dadd_rn(shut, __dmul_rn((double)N, leg));
     }
-    s.d(M.m64_w + g_cur) = shut;
+    s.d(M.m64_w + g) = shut;
   }
   // ---- lengths (L106): N_HU(g), N_SU(g) multiply the tour distance, shuttles x2; cost (R1)
   double path = 0.0;
   for (uint32_t g = 0; g < n_t; ++g) {
-    const double lt = s.d(M.m64_lt + g), shut = s.d(M.m64_w + g);
+    const double lt = lt_of(g), shut = s.d(M.m64_w + g);
+    const uint32_t n_g = (uint32_t)mask_count(mask_load<MASKW>(s, M.m64_mask + MASKW * g));
     const double l_hu  = __dmul_rn((double)thu[g].x, lt);
-    const double l_esu = __dadd_rn(__dmul_rn((double)s.w(M.m32_ng + g), lt), shut);
+    const double l_esu = __dadd_rn(__dmul_rn((double)n_g, lt), shut);
     path = __dadd_rn(path, __dadd_rn(__dadd_rn(l_hu, l_esu), shut));
   }
   out.feasible = true; out.path = path; out.makespan = makespan;
