@@ -112,6 +112,63 @@ def _oracle_chunk(name, first, n):
     return o.search(inst.seed, n, first_id=first)
 
 
+def _oracle_moves_chunk(name, first, n):
+    from oracle import lgo
+    from paper_1909_10286_b200 import workloads as wl
+    o = lgo.Oracle(wl.make(name))
+    p0 = o.init_plan()
+    return float(o.move_eval_batch(p0, 1, first, n)[3].mean())
+
+
+def bench_alg1(args, torch, binding, wl):
+    """The paper's own loop (Algorithm 1) on its own problem shape: nearest-neighbour start,
+    one batch of remove/reinsert workers, and N_iters iterations inside the persistent kernel."""
+    import multiprocessing as mp
+    inst = wl.make(args.alg1_workload)
+    g = binding.Instance(inst)
+    sm, tmv = g.query(6), g.query(15)
+    stream = torch.cuda.current_stream()
+    g.init_plan()
+    t0 = time.perf_counter(); p0 = g.init_plan(); t_init = time.perf_counter() - t0
+    n = sm * tmv * 16
+    out = g.move_eval_batch(p0, 1, 0, n); torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(stream)
+    for _ in range(3):
+        g.move_eval_batch(p0, 1, 0, n, out=out)
+    b.record(stream); torch.cuda.synchronize()
+    ms_batch = a.elapsed_time(b) / 3
+    n_workers, eps = sm * tmv, 0.4
+    c0 = g.local_search(p0, inst.seed, 0, 1, 0, history=False)[1]
+    g.local_search(p0, inst.seed, 10, n_workers, int(eps * 2**32), history=False)          # warm-up
+    t0 = time.perf_counter()
+    _, c_star, hc, _ = g.local_search(p0, inst.seed, args.alg1_iters, n_workers, int(eps * 2**32))
+    t_ls = time.perf_counter() - t0
+    res = {"workload": f"{args.alg1_workload}: N_T={inst.n_tours} N_B={inst.n_bps} N_F={inst.n_fields} N_HU={inst.n_hu} N_SU={inst.n_su}",
+           "threads_per_block": tmv, "grid": sm, "smem_bytes": g.query(16),
+           "init_plan_ms": 1e3 * t_init,
+           "move_eval_batch": {"value": n / ms_batch * 1e3, "unit": "workers/s", "workers": n,
+                               "feasible_fraction": float(out[3].float().mean().item())},
+           "local_search": {"iterations": args.alg1_iters, "workers_per_iteration": n_workers, "eps": eps,
+                            "wall_s": t_ls, "iterations_per_s": args.alg1_iters / t_ls,
+                            "worker_evals_per_s": args.alg1_iters * n_workers / t_ls,
+                            "cost_init": c0, "cost_best": c_star, "delta_pct": 100.0 * (c_star - c0) / c0,
+                            "what": "lgx_local_search through the C ABI, host plan in / x* out, wall clock",
+                            "paper_context": "T_solve 81.89 s for 5000 iterations on a Titan V, workers per iteration "
+                                             "not stated (PAPER.md Table 3, L355): another machine, not a target"}}
+    if not args.no_cpu_baseline:
+        cores = os.cpu_count() or 1
+        per = 2048
+        with mp.get_context("fork").Pool(cores) as pool:
+            t0 = time.perf_counter()
+            pool.starmap(_oracle_moves_chunk, [(args.alg1_workload, r * per, per) for r in range(cores)])
+            dt = time.perf_counter() - t0
+        res["cpu_baseline"] = {"value": per * cores / dt, "unit": "workers/s", "cores": cores, "kind": "oracle",
+                               "sample": f"{per * cores} workers of the same batch, {cores} processes, {dt:.1f} s wall"}
+    g.close()
+    return res
+
+
 def run_reference(args):
     """--impl reference: the oracle (the only reference implementation of this tier)."""
     rank = int(os.environ.get("RANK", "0"))
@@ -146,6 +203,9 @@ def main():
     ap.add_argument("--workload", default="medium")
     ap.add_argument("--batch-log2", type=int, default=None, help="candidates per GPU per step (default: config budget, capped 2^28)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--alg1-workload", default="paper_scale", help="instance of the Algorithm 1 leg (SURVEY §8(f) N1/N3)")
+    ap.add_argument("--alg1-iters", type=int, default=1000)
+    ap.add_argument("--no-alg1", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "lgx" else args.warmup
     if args.impl == "reference":
@@ -248,6 +308,9 @@ def main():
                                "feasible_fraction": float(out[3].float().mean().item()),
                                "e2e_host_buffers": {"value": n_h / th, "unit": UNIT, "ids": n_h,
                                                     "d2h_bytes": 25 * n_h, "h2d_bytes": 0}}
+
+    if rank == 0 and world == 1 and not args.no_alg1:
+        extra["alg1"] = bench_alg1(args, torch, binding, wl)
 
     if rank != 0:
         if dist is not None:

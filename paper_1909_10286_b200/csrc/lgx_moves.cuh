@@ -36,6 +36,7 @@ namespace cg = cooperative_groups;
 
 constexpr int      kMvThreads = 512;            // __launch_bounds__ of the move kernels
 constexpr uint32_t kNone      = 0xFFFFFFFFu;
+constexpr uint32_t kSortKeys  = 256;            // (source tour, target tour) pairs up to 16 tours, else the lower tour
 
 // Shared-memory layout of the move kernels (byte offsets from the start of dynamic shared memory):
 //   vertex coordinates | demand quanta | tail of image C (from offc_cs) | incumbent tables | plan store | per-thread state rows
@@ -58,6 +59,8 @@ struct MvHdr {
   uint32_t off_tst;     // f64 [5][n_t]   the incumbent's L_tour(g), E(g), T(g), T_wait(g), shuttle sum(g)
   uint32_t off_tbad;    // u32 [n_t]      BPs of the tour that have fields but miss their demand
   uint32_t off_misc;    // u32 [16]       [0] BPs without fields but with demand; [1] sum of tbad; [4..9] the move being applied
+  uint32_t off_sort;    // u32 [kSortKeys + 1]  counting sort of a round's workers by the tours they touch
+  uint32_t off_order;   // u16 [blockDim.x]     sorted worker of every thread
   uint32_t off_plans;   // 3 plans (x*, x_old, scratch); the batch kernel uses the first
   uint32_t plan_bytes;  // one plan: bp_tour u8[n_b] | bp_pos u8[n_b] | field_bp u16[n_f] | field_pos u16[n_f] | masks u64[n_t*MW]
   uint32_t pl_bpos, pl_fbp, pl_fpos, pl_mask;
@@ -360,6 +363,24 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
     we = wb + (r.y - r.x) - ((g == mv.g1) ? L : 0u) + ((g == mv.g2) ? L : 0u);
   };
 
+  // The legs a worker cannot read from the tables — into each breakpoint from the worker's own predecessor, and
+  // the moved field's leg to its new BP — are computed here, by all lanes together, not inside the divergent walks.
+  uint32_t wb_a = 0, we_a = 0, wb_b = 0, we_b = 0;
+  if (nr > 0u) wrange(ga, wb_a, we_a);
+  if (nr > 1u) wrange(gb, wb_b, we_b);
+  double X1 = 0.0, X2 = 0.0, X3 = 0.0, xlb = 0.0;
+  if (nr > 0u) {
+    auto into = [&](uint32_t q) -> double {
+      if (q >= (uint32_t)H.n_f) return 0.0;                                    // past the last position: never reached
+      const uint32_t vf = 1u + n_b + (pos4[map_idx(q)].x & 0xFFFFu);
+      const bool first = (q == wb_a) || (nr > 1u && q == wb_b);                // first field of its tour: from HQ (L21)
+      const uint32_t vp = first ? 0u : 1u + n_b + (pos4[map_idx(q - 1u)].x & 0xFFFFu);
+      return edge_from_xy(xy, vp, vf);
+    };
+    X1 = into(Q1); X2 = into(Q2); X3 = into(Q3);
+    if (fld) xlb = edge_from_xy(xy, 1u + n_b + (pos4[mv.a].x & 0xFFFFu), 1u + mv.fld_b);
+  }
+
   // ---- untouched tours: the incumbent's values
   double makespan = 0.0;                                                       // every T(g) >= 0
   for (uint32_t g = 0; g < n_t; ++g) {
@@ -376,17 +397,20 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
   for (uint32_t r = 0; r < nr; ++r) {
     const uint32_t g = r ? gb : ga;
     bad -= tbad[g];
-    uint32_t p, pe;
-    wrange(g, p, pe);
+    uint32_t p = r ? wb_b : wb_a;
+    const uint32_t pe = r ? we_b : we_a;
     uint32_t P0 = p, J0 = map_idx(p), P1 = Q1, J1 = K1, P2 = Q2, J2 = K2, P3 = Q3, J3 = K3;
-    while (P1 < p) { P1 = P2; J1 = J2; P2 = P3; J2 = J3; P3 = kNone; }
-    uint32_t b_cur = kNone, Sq = 0, Hq = 0, k = 0, m = 0, prev_x = kNone /* HQ */, idx = 0;
+    double Y0 = 0.0, Y1 = X1, Y2 = X2, Y3 = X3;
+    if (p < pe) Y0 = edge_from_xy(xy, 0u, 1u + n_b + (pos4[J0].x & 0xFFFFu));   // HQ to the tour's first field (L21)
+    while (P1 < p) { P1 = P2; J1 = J2; Y1 = Y2; P2 = P3; J2 = J3; Y2 = Y3; P3 = kNone; }
+    uint32_t b_cur = kNone, Sq = 0, Hq = 0, k = 0, m = 0, x_last = 0, idx = 0;
     double Lt = 0.0, sd = 0.0, sumE = 0.0;
     for (; p < pe; ++p) {
       ++idx;
       bool exc = false;
-      if (p == P0) {
-        do { idx = J0; P0 = P1; J0 = J1; P1 = P2; J1 = J2; P2 = P3; J2 = J3; P3 = kNone; } while (p == P0);
+      double lh = 0.0;
+      if (__builtin_expect(p == P0, 0)) {
+        do { idx = J0; lh = Y0; P0 = P1; J0 = J1; Y0 = Y1; P1 = P2; J1 = J2; Y1 = Y2; P2 = P3; J2 = J3; Y2 = Y3; P3 = kNone; } while (p == P0);
         exc = true;
       }
       const uint4 en = pos4[idx];
@@ -394,23 +418,22 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
       uint32_t b = en.x >> 16;
       double leg_h = lg.x, leg_b = lg.y;
       if (exc) {                                   // the predecessor is not the incumbent's: HQ at the tour's start, or around the moved block
-        const uint32_t vf = 1u + n_b + (en.x & 0xFFFFu);
-        leg_h = edge_from_xy(xy, prev_x == kNone ? 0u : 1u + n_b + (prev_x & 0xFFFFu), vf);
-        if (fld && p == mv.c) { b = mv.fld_b; leg_b = edge_from_xy(xy, vf, 1u + b); }
+        leg_h = lh;
+        if (fld && p == mv.c) { b = mv.fld_b; leg_b = xlb; }
       }
-      if (b != b_cur) {
+      if (__builtin_expect(b != b_cur, 0)) {
         if (b_cur != kNone) { bad += (Sq < dq[b_cur]) ? 1u : 0u; sumE = __dadd_rn(sumE, div_small(sd, k, rcp)); ++m; }   // R10
         b_cur = b; sd = 0.0; Sq = 0u; k = 0u;
       }
       Lt = __dadd_rn(Lt, leg_h);                                               // field to field (L69)
       sd = __dadd_rn(sd, leg_b);
       Hq += en.z; Sq += en.y; ++k;
-      prev_x = en.x;
+      x_last = en.x;
     }
     double E = 0.0;
     if (b_cur != kNone) {
       bad += (Sq < dq[b_cur]) ? 1u : 0u; sumE = __dadd_rn(sumE, div_small(sd, k, rcp)); ++m;
-      Lt = __dadd_rn(Lt, edge_from_xy(xy, 1u + n_b + (prev_x & 0xFFFFu), 0u));  // back to HQ (L21; R2)
+      Lt = __dadd_rn(Lt, edge_from_xy(xy, 1u + n_b + (x_last & 0xFFFFu), 0u));  // back to HQ (L21; R2)
       E = __ddiv_rn(__dmul_rn(2.0, div_small(sumE, m, rcp)), H.v_su);          // L199, L213; R9
     }
     const uint2 hu = thu[g];
@@ -505,15 +528,17 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
     double shut = 0.0;
     for (; p < pe; ++p) {
       ++idx;
-      if (p == P0) {
+      if (__builtin_expect(p == P0, 0)) {
         do { idx = J0; P0 = P1; J0 = J1; P1 = P2; J1 = J2; P2 = P3; J2 = J3; P3 = kNone; } while (p == P0);
         inblk = (p - mv.c) < L;                  // the moved block's counts were tabulated under another tour's SU set
       }
       const uint4 en = pos4[idx];
       double leg = leg2[idx].y;
       uint32_t N = en.w;
-      if (inblk && fld) leg = edge_from_xy(xy, 1u + n_b + (en.x & 0xFFFFu), 1u + mv.fld_b);
-      if (recount || inblk) N = shuttle_count(en.y, n_g, C_g, magic);
+      if (__builtin_expect(recount || inblk, 0)) {
+        if (inblk && fld) leg = xlb;
+        N = shuttle_count(en.y, n_g, C_g, magic);
+      }
       shut = __dadd_rn(shut, __dmul_rn((double)N, leg));
     }
     s.d(M.m64_w + g) = shut;
@@ -555,6 +580,46 @@ __device__ __forceinline__ void mv_prologue(const MvParams &P, uint8_t *sm, St &
   __syncthreads();
 }
 
+// One round of a block = up to blockDim.x consecutive worker ids.  Which thread scores which worker is free, so the
+// round's workers are counting-sorted by the tours their moves touch: the lanes of a warp then walk the same tours
+// (equal trip counts, the same shared-memory words, BP boundaries at the same steps, similar Algorithm-2 paths).
+// Returns the worker (index within the round) this thread scores, or kNone.  Block-wide (barriers inside).
+__device__ __forceinline__ uint32_t mv_sort_round(const MvParams &P, uint8_t *sm, uint64_t id_base, uint32_t n_round, uint32_t tid, uint32_t T)
+{
+  const uint32_t n_t = P.H.n_t;
+  const uint32_t nk = (n_t <= 16u) ? n_t * n_t : n_t;
+  uint32_t *hist = MV_TAB(uint32_t, P.M.off_sort);
+  uint16_t *order = MV_TAB(uint16_t, P.M.off_order);
+  for (uint32_t k = tid; k <= nk; k += T) hist[k] = 0u;
+  __syncthreads();
+  uint32_t key = nk;
+  if (tid < n_round) {
+    const uint64_t id = id_base + tid;
+    uint32_t w[4];
+    philox_block(P, (uint32_t)id, (uint32_t)(id >> 32), 5u, 0u, w);
+    const Move mv = mv_derive(P, sm, w[0], w[1], w[2], nullptr);
+    const uint32_t ga = min(mv.g1, mv.g2), gb = max(mv.g1, mv.g2);
+    key = (n_t <= 16u) ? ga * n_t + gb : ga;
+  }
+  const uint32_t rank = atomicAdd(&hist[key], 1u);
+  __syncthreads();
+  if (tid < 32u) {                                   // exclusive scan of the histogram
+    const uint32_t per = (nk + 1u + 31u) / 32u, k0 = tid * per;
+    uint32_t sum = 0;
+    for (uint32_t k = k0; k < k0 + per && k <= nk; ++k) sum += hist[k];
+    uint32_t incl = sum;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) { const uint32_t o = __shfl_up_sync(0xFFFFFFFFu, incl, off); if ((int)tid >= off) incl += o; }
+    uint32_t run = incl - sum;
+    for (uint32_t k = k0; k < k0 + per && k <= nk; ++k) { const uint32_t h = hist[k]; hist[k] = run; run += h; }
+  }
+  __syncthreads();
+  order[hist[key] + rank] = (uint16_t)tid;
+  __syncthreads();
+  const uint32_t j = order[tid];
+  return j < n_round ? j : kNone;
+}
+
 // ================================================================== batch kernel (L163-165)
 
 template <int MASKW>
@@ -569,8 +634,11 @@ __global__ void __launch_bounds__(kMvThreads, 1) lgx_move_eval_k(const __grid_co
   mv_load_plan<MASKW>(P, sm, plan, tid, T);
   mv_encode<MASKW>(P, sm, plan, tid, T);
   const uint64_t stride = (uint64_t)gridDim.x * T;
-  for (uint64_t i = (uint64_t)blockIdx.x * T + tid; i < P.n; i += stride) {
-    const uint64_t id = P.first_id + i;
+  for (uint64_t base = (uint64_t)blockIdx.x * T; base < P.n; base += stride) {
+    const uint32_t n_round = (uint32_t)min((uint64_t)T, P.n - base);
+    const uint32_t j = mv_sort_round(P, sm, P.first_id + base, n_round, tid, T);
+    if (j == kNone) continue;
+    const uint64_t i = base + j, id = P.first_id + i;
     uint32_t w[4];
     philox_block(P, (uint32_t)id, (uint32_t)(id >> 32), 5u, 0u, w);
     const Move mv = mv_derive(P, sm, w[0], w[1], w[2], nullptr);
@@ -630,8 +698,11 @@ __global__ void __launch_bounds__(kMvThreads, 1) lgx_local_search_k(const __grid
     // ---- steps 7-12: every worker moves x once and scores it; running (cost, id) minimum per thread
     unsigned long long best_bits = ~0ull, best_id = ~0ull;
     const uint64_t id0 = (uint64_t)k * P.n_workers;
-    for (uint64_t i = (uint64_t)blockIdx.x * T + tid; i < P.n_workers; i += (uint64_t)gridDim.x * T) {
-      const uint64_t id = id0 + i;
+    for (uint64_t base = (uint64_t)blockIdx.x * T; base < P.n_workers; base += (uint64_t)gridDim.x * T) {
+      const uint32_t n_round = (uint32_t)min((uint64_t)T, (uint64_t)P.n_workers - base);
+      const uint32_t j = mv_sort_round(P, sm, id0 + base, n_round, tid, T);
+      if (j == kNone) continue;
+      const uint64_t id = id0 + base + j;
       uint32_t w[4];
       philox_block(P, (uint32_t)id, (uint32_t)(id >> 32), 5u, 0u, w);
       const Move mv = mv_derive(P, sm, w[0], w[1], w[2], nullptr);
