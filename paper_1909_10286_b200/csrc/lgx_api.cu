@@ -350,8 +350,11 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
     M.off_c = o;     o = align16(o + (H.imagec_bytes - H.offc_cs));
     M.off_pos4 = o;  o = align16(o + 16u * (uint32_t)nf);
     M.off_leg2 = o;  o = align16(o + 16u * (uint32_t)nf);
+    M.off_pre2 = o;  o = align16(o + 16u * (uint32_t)nf);
     M.off_posf = o;  o = align16(o + 2u * (uint32_t)nf);
     M.off_bp = o;    o = align16(o + 8u * (uint32_t)nb);
+    M.off_bsh = o;   o = align16(o + 8u * (uint32_t)nb);
+    M.off_bpq = o;   o = align16(o + 8u * (uint32_t)nb);
     M.off_pre = o;   o = align16(o + 2u * ((uint32_t)nb + 1u));
     M.off_bpat = o;  o = align16(o + (uint32_t)nb);
     M.off_cnt = o;   o = align16(o + 4u * (uint32_t)nb);
@@ -360,8 +363,8 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
     M.off_tsn = o;   o = align16(o + 8u * (uint32_t)nt);
     M.off_tmask = o; o = align16(o + 8u * (uint32_t)nt * MW);
     M.off_trng = o;  o = align16(o + 8u * (uint32_t)nt);
-    M.off_tst = o;   o = align16(o + 40u * (uint32_t)nt);
-    M.off_tbad = o;  o = align16(o + 4u * (uint32_t)nt);
+    M.off_tst = o;   o = align16(o + 48u * (uint32_t)nt);
+    M.off_thq = o;   o = align16(o + 4u * (uint32_t)nt);
     M.off_misc = o;  o = align16(o + 64u);
     M.off_sort = o;  o = align16(o + 4u * (kSortKeys + 1u));
     M.off_order = o; o = align16(o + 2u * (uint32_t)kMvThreads);

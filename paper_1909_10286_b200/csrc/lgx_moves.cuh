@@ -46,8 +46,11 @@ struct MvHdr {
   uint32_t off_c;       // tail of image C: byte x of image C (x >= offc_cs) sits at off_c + x - offc_cs
   uint32_t off_pos4;    // u32x4 [n_f]    plan order: f | b << 16, s_q[f], h_q[f], shuttle count N under the incumbent's SU sets
   uint32_t off_leg2;    // f64x2 [n_f]    plan order: D(predecessor on the tour or HQ, f), D(f, b)
+  uint32_t off_pre2;    // f64x2 [n_f]    plan order: the tour's running route sum / shuttle sum BEFORE this position
   uint32_t off_posf;    // u16 [n_f]      position of field f in plan order
   uint32_t off_bp;      // u32x2 [n_b]    x = start | len << 16;  y = plan index | tour << 8 | pos << 16
+  uint32_t off_bsh;     // u32x2 [n_b]    S_q(b), area quanta of b's fields
+  uint32_t off_bpq;     // f64 [n_b]      mean field->BP leg of b (0 without fields)
   uint32_t off_pre;     // u16 [n_b + 1]  start of the BP at plan index j; pre[n_b] = n_f
   uint32_t off_bpat;    // u8 [n_b]       BP at plan index j
   uint32_t off_cnt;     // u32 [n_b]      scratch: fields per BP
@@ -56,9 +59,9 @@ struct MvHdr {
   uint32_t off_tsn;     // u32x2 [n_t]    S_g = capacity quanta of the tour's SUs, n_g = their number
   uint32_t off_tmask;   // u64 [n_t*MW]   SU membership by capacity rank
   uint32_t off_trng;    // u32x2 [n_t]    the tour's positions [begin, end) in plan order
-  uint32_t off_tst;     // f64 [5][n_t]   the incumbent's L_tour(g), E(g), T(g), T_wait(g), shuttle sum(g)
-  uint32_t off_tbad;    // u32 [n_t]      BPs of the tour that have fields but miss their demand
-  uint32_t off_misc;    // u32 [16]       [0] BPs without fields but with demand; [1] sum of tbad; [4..9] the move being applied
+  uint32_t off_tst;     // f64 [6][n_t]   the incumbent's L_tour(g), E(g), T(g), T_wait(g), shuttle sum(g), route sum before the leg back to HQ
+  uint32_t off_thq;     // u32 [n_t]      H_q(g)
+  uint32_t off_misc;    // u32 [16]       [0] BPs that miss their demand (eq. (2)); [4..9] the move being applied
   uint32_t off_sort;    // u32 [kSortKeys + 1]  counting sort of a round's workers by the tours they touch
   uint32_t off_order;   // u16 [blockDim.x]     sorted worker of every thread
   uint32_t off_plans;   // 3 plans (x*, x_old, scratch); the batch kernel uses the first
@@ -161,16 +164,14 @@ __device__ void mv_encode(const MvParams &P, uint8_t *sm, const uint8_t *plan, u
     uint32_t acc = 0;
     for (uint32_t g = 0; g < n_t; ++g) { const uint32_t len = tpl[g] >> 8; tpl[g] = acc | (len << 8); acc += len; }
     for (uint32_t b = 0; b < n_b; ++b) bpat[(tpl[p_bt[b]] & 0xFFu) + p_bp[b]] = (uint8_t)b;
-    acc = 0; uint32_t n_bad = 0;
+    acc = 0;
     for (uint32_t j = 0; j < n_b; ++j) {
       const uint32_t b = bpat[j], len = cnt[b];
       pre[j] = (uint16_t)acc;
       bp[b] = make_uint2(acc | (len << 16), j | ((uint32_t)p_bt[b] << 8) | ((uint32_t)p_bp[b] << 16));
       acc += len;
-      if (len == 0u && dq[b] > 0u) ++n_bad;                    // a BP without fields fails eq. (2) unless it needs nothing
     }
     pre[n_b] = (uint16_t)acc;
-    misc[0] = n_bad;
     for (uint32_t g = 0; g < n_t; ++g) { const uint32_t j0 = tpl[g] & 0xFFu, j1 = j0 + (tpl[g] >> 8); trng[g] = make_uint2(pre[j0], pre[j1]); }
   }
   if (tid >= 32u) {
@@ -211,31 +212,45 @@ __device__ void mv_encode(const MvParams &P, uint8_t *sm, const uint8_t *plan, u
     leg2[p] = make_double2(edge_from_xy(xy, pred, 1u + n_b + f), edge_from_xy(xy, 1u + n_b + f, 1u + b));
   }
   __syncthreads();
-  // per tour, one lane each: the walk of DESIGN.md S4 / S7 over the tour's positions, in order
+  // per tour, one lane each: the walk of DESIGN.md S4 / S7 over the tour's positions, in order; it also leaves the
+  // running sums before every position (pre2) and the per-BP supplies, areas and mean legs
+  uint2 *bsh = MV_TAB(uint2, M.off_bsh);
+  double *bpq = MV_TAB(double, M.off_bpq);
+  for (uint32_t b = tid; b < n_b; b += T) { bsh[b] = make_uint2(0u, 0u); bpq[b] = 0.0; }
+  __syncthreads();
   {
     const uint2 *thu = MV_TAB(const uint2, M.off_thu);
     double *tst = MV_TAB(double, M.off_tst);
-    uint32_t *tbad = MV_TAB(uint32_t, M.off_tbad);
+    double2 *pre2 = MV_TAB(double2, M.off_pre2);
+    uint32_t *thq = MV_TAB(uint32_t, M.off_thq);
     const uint32_t n_warps = T >> 5;
     if ((tid & 31u) == 0u)
       for (uint32_t g = tid >> 5; g < n_t; g += n_warps) {
         const uint2 r = trng[g];
         double Lt = 0.0, sd = 0.0, sumE = 0.0, shut = 0.0;
-        uint32_t Hq = 0, Sq = 0, k = 0, m = 0, bad = 0, b_cur = kNone, f_last = 0;
+        uint32_t Hq = 0, Sq = 0, Hb = 0, k = 0, m = 0, b_cur = kNone, f_last = 0;
         for (uint32_t p = r.x; p < r.y; ++p) {
           const uint4 e = pos4[p]; const double2 lg = leg2[p];
           const uint32_t b = e.x >> 16;
           if (b != b_cur) {
-            if (b_cur != kNone) { bad += (Sq < dq[b_cur]) ? 1u : 0u; sumE = __dadd_rn(sumE, div_small(sd, k, rcp)); ++m; }
-            b_cur = b; sd = 0.0; Sq = 0u; k = 0u;
+            if (b_cur != kNone) {
+              const double q = div_small(sd, k, rcp);
+              bsh[b_cur] = make_uint2(Sq, Hb); bpq[b_cur] = q;
+              sumE = __dadd_rn(sumE, q); ++m;
+            }
+            b_cur = b; sd = 0.0; Sq = 0u; Hb = 0u; k = 0u;
           }
-          Lt = __dadd_rn(Lt, lg.x); sd = __dadd_rn(sd, lg.y); Hq += e.z; Sq += e.y; ++k;
+          pre2[p] = make_double2(Lt, shut);
+          Lt = __dadd_rn(Lt, lg.x); sd = __dadd_rn(sd, lg.y); Hq += e.z; Hb += e.z; Sq += e.y; ++k;
           shut = __dadd_rn(shut, __dmul_rn((double)e.w, lg.y));
           f_last = e.x & 0xFFFFu;
         }
         double E = 0.0;
+        const double lt_open = Lt;
         if (b_cur != kNone) {
-          bad += (Sq < dq[b_cur]) ? 1u : 0u; sumE = __dadd_rn(sumE, div_small(sd, k, rcp)); ++m;
+          const double q = div_small(sd, k, rcp);
+          bsh[b_cur] = make_uint2(Sq, Hb); bpq[b_cur] = q;
+          sumE = __dadd_rn(sumE, q); ++m;
           Lt = __dadd_rn(Lt, edge_from_xy(xy, 1u + n_b + f_last, 0u));
           E = __ddiv_rn(__dmul_rn(2.0, div_small(sumE, m, rcp)), H.v_su);
         }
@@ -247,11 +262,16 @@ __device__ void mv_encode(const MvParams &P, uint8_t *sm, const uint8_t *plan, u
         tst[2u * n_t + g] = __dadd_rn(__ddiv_rn(Lt, H.v_hu), __ddiv_rn((double)Hq, (double)hu.y));
         tst[3u * n_t + g] = wait_time(E, sn.x, cs[mask_top(mk)], hu.x, H.kappa, rcp);
         tst[4u * n_t + g] = shut;
-        tbad[g] = bad;
+        tst[5u * n_t + g] = lt_open;
+        thq[g] = Hq;
       }
   }
   __syncthreads();
-  if (tid == 0) { const uint32_t *tbad = MV_TAB(const uint32_t, M.off_tbad); uint32_t a = 0; for (uint32_t g = 0; g < n_t; ++g) a += tbad[g]; misc[1] = a; }
+  if (tid == 0) {                                   // eq. (2) (L79) over all BPs: a BP without fields has S_q = 0
+    uint32_t bad = 0;
+    for (uint32_t b = 0; b < n_b; ++b) bad += (bsh[b].x < dq[b]) ? 1u : 0u;
+    misc[0] = bad;
+  }
   __syncthreads();
 }
 
@@ -262,7 +282,8 @@ struct Move {
   uint32_t a, len, c;
   uint32_t fld_b;     // field move: the BP the moved field now belongs to; else kNone
   uint32_t g1, g2;    // the tours the move touches: source and target (kNone, kNone: no move)
-  uint32_t bad;       // BPs without fields but with positive demand under this move
+  uint32_t src;       // field move: the BP the field leaves; BP move: the moved BP
+  uint32_t jo, jq;    // BP move: its plan index before / after the move (0, 0 for a field move)
 };
 
 // PAPER.md:L158, L184; R35: v = below(w0, N_F+N_B) picks a field or a BP ("since N_F >> N_B it is
@@ -273,8 +294,6 @@ __device__ __forceinline__ Move mv_derive(const MvParams &P, const uint8_t *sm, 
   const ImgHdr &H = P.H; const MvHdr &M = P.M;
   const uint32_t n_f = H.n_f, n_b = H.n_b, n_t = H.n_t;
   const uint2 *bp = MV_TAB(const uint2, M.off_bp);
-  const uint32_t *dq = MV_TAB(const uint32_t, M.off_dq);
-  const uint32_t n_bad = MV_TAB(const uint32_t, M.off_misc)[0];
   const uint32_t v = __umulhi(w0, n_f + n_b);
   Move m;
   if (v < n_f) {
@@ -282,11 +301,11 @@ __device__ __forceinline__ Move mv_derive(const MvParams &P, const uint8_t *sm, 
     const uint32_t A = MV_TAB(const uint4, M.off_pos4)[a].x >> 16;
     const uint32_t t = __umulhi(w1, n_b);
     const uint2 bt = bp[t], bA = bp[A];
-    const uint32_t len_t = bt.x >> 16, start_t = bt.x & 0xFFFFu, len_A = bA.x >> 16;
+    const uint32_t len_t = bt.x >> 16, start_t = bt.x & 0xFFFFu;
     const uint32_t q = __umulhi(w2, len_t - (A == t ? 1u : 0u) + 1u);
     m.a = a; m.len = 1u; m.c = start_t - (a < start_t ? 1u : 0u) + q;
     m.fld_b = t; m.g1 = (bA.y >> 8) & 0xFFu; m.g2 = (bt.y >> 8) & 0xFFu;
-    m.bad = n_bad - ((len_t == 0u && dq[t] > 0u) ? 1u : 0u) + ((len_A == 1u && A != t && dq[A] > 0u) ? 1u : 0u);
+    m.src = A; m.jo = 0u; m.jq = 0u;
     if (raw) { raw[0] = 0u; raw[1] = v; raw[2] = A; raw[3] = a - (bA.x & 0xFFFFu); raw[4] = t; raw[5] = q; }
   } else {
     const uint32_t b = v - n_f;
@@ -301,16 +320,15 @@ __device__ __forceinline__ Move mv_derive(const MvParams &P, const uint8_t *sm, 
     m.a = bb.x & 0xFFFFu; m.len = len;
     m.c = (jq <= j) ? (uint32_t)pre[jq] : (uint32_t)pre[jq + 1u] - len;
     m.fld_b = kNone; m.g1 = g; m.g2 = t;
-    m.bad = n_bad;
+    m.src = b; m.jo = j; m.jq = jq;
     if (raw) { raw[0] = 1u; raw[1] = b; raw[2] = g; raw[3] = (bb.y >> 16) & 0xFFu; raw[4] = t; raw[5] = q; }
   }
   return m;
 }
 
-__device__ __forceinline__ Move mv_identity(const MvParams &P, const uint8_t *sm)
+__device__ __forceinline__ Move mv_identity()
 {
-  Move m; m.a = m.len = m.c = 0u; m.fld_b = m.g1 = m.g2 = kNone;
-  m.bad = MV_TAB(const uint32_t, P.M.off_misc)[0];
+  Move m; m.a = m.len = m.c = 0u; m.fld_b = m.g1 = m.g2 = kNone; m.src = 0u; m.jo = m.jq = 0u;
   return m;
 }
 
@@ -318,10 +336,12 @@ __device__ __forceinline__ Move mv_identity(const MvParams &P, const uint8_t *sm
 
 struct EvalOut { bool feasible; double cost, path, makespan; };
 
-// Delta evaluation, exact: a tour the move does not touch keeps the incumbent's L_tour, E, T, T_wait (same
-// operands, same order, same bits), so the worker walks only the <= 2 touched tours in pass 1, and in pass 2
-// those plus the tours whose SU set Algorithm 2 changed.  Within a walked tour every position whose predecessor
-// is the incumbent's reads its legs (and, under an unchanged SU set, its shuttle count) from the tables.
+// Incremental evaluation, exact.  Everything a move leaves alone keeps the incumbent's value — same operands in the
+// same order, hence the same bits: integer sums (supplies, areas: eq. (2) is decided in O(1)), the mean leg of every
+// BP whose field list is unchanged, L_tour / E / T / T_wait / shuttle sum of the tours the move does not touch.  In a
+// touched tour the FP64 running sums restart from the incumbent's prefix value at the first position the move
+// changes (pre2) and only the rest of the tour is re-added in order; the mean legs of the two BPs a field move
+// changes are re-summed over those BPs alone; E(g) re-sums the tour's per-BP means.
 template <int MASKW>
 __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm, const St &s, const Move &mv)
 {
@@ -329,11 +349,17 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
   const uint32_t n_b = H.n_b, n_t = H.n_t, n_su = H.n_su;
   const uint4    *pos4 = MV_TAB(const uint4, M.off_pos4);
   const double2  *leg2 = MV_TAB(const double2, M.off_leg2);
+  const double2  *pre2 = MV_TAB(const double2, M.off_pre2);
+  const uint2    *bp   = MV_TAB(const uint2, M.off_bp);
+  const uint2    *bsh  = MV_TAB(const uint2, M.off_bsh);
+  const double   *bpq  = MV_TAB(const double, M.off_bpq);
+  const uint8_t  *bpat = MV_TAB(const uint8_t, M.off_bpat);
+  const uint32_t *tpl  = MV_TAB(const uint32_t, M.off_tpl);
   const uint2    *thu  = MV_TAB(const uint2, M.off_thu);
   const uint2    *tsn  = MV_TAB(const uint2, M.off_tsn);
   const uint2    *trng = MV_TAB(const uint2, M.off_trng);
   const double   *tst  = MV_TAB(const double, M.off_tst);
-  const uint32_t *tbad = MV_TAB(const uint32_t, M.off_tbad);
+  const uint32_t *thq  = MV_TAB(const uint32_t, M.off_thq);
   const uint64_t *tmask = MV_TAB(const uint64_t, M.off_tmask);
   const uint32_t *dq   = MV_TAB(const uint32_t, M.off_dq);
   const double2  *xy   = MV_TAB(const double2, M.off_xy);
@@ -346,6 +372,23 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
   const uint32_t ga = min(mv.g1, mv.g2), gb = max(mv.g1, mv.g2);
   const uint32_t nr = (mv.g1 == kNone) ? 0u : (ga == gb ? 1u : 2u);
   const bool fld = (mv.fld_b != kNone);
+  const uint32_t A = mv.src, t = mv.fld_b;
+
+  // ---- S5: eq. (2) (L79) — only the two BPs of a field move change their supply
+  uint32_t h_blk = 0;                                                         // area quanta that change tours
+  {
+    uint32_t bad = MV_TAB(const uint32_t, M.off_misc)[0];
+    if (fld) {
+      const uint4 ef = pos4[mv.a];
+      h_blk = ef.z;
+      if (A != t) {
+        const uint32_t SA = bsh[A].x, ST = bsh[t].x, dA = dq[A], dT = dq[t];
+        bad = bad - (SA < dA ? 1u : 0u) - (ST < dT ? 1u : 0u) + (SA - ef.y < dA ? 1u : 0u) + (ST + ef.y < dT ? 1u : 0u);
+      }
+    } else if (nr > 0u) h_blk = bsh[A].y;
+    if (bad != 0u) return out;                                                 // discarded (L186; R19)
+  }
+
   // worker position -> incumbent index: p -> p outside [lo, lo+span); three breakpoints (Q, K) inside, ascending
   const uint32_t lo = min(mv.a, mv.c), span = max(mv.a, mv.c) + L - lo;
   const uint32_t shift = (mv.c <= mv.a) ? (0u - L) : L;
@@ -361,6 +404,11 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
     const uint2 r = trng[g];
     wb = r.x - ((mv.g1 < g) ? L : 0u) + ((mv.g2 < g) ? L : 0u);
     we = wb + (r.y - r.x) - ((g == mv.g1) ? L : 0u) + ((g == mv.g2) ? L : 0u);
+  };
+  // first position of [wb, we) the move changes (a breakpoint), else we
+  auto first_change = [&](uint32_t wb, uint32_t we) -> uint32_t {
+    const uint32_t q = (Q1 >= wb) ? Q1 : ((Q2 >= wb) ? Q2 : ((Q3 >= wb) ? Q3 : we));
+    return min(q, we);
   };
 
   // The legs a worker cannot read from the tables — into each breakpoint from the worker's own predecessor, and
@@ -378,7 +426,7 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
       return edge_from_xy(xy, vp, vf);
     };
     X1 = into(Q1); X2 = into(Q2); X3 = into(Q3);
-    if (fld) xlb = edge_from_xy(xy, 1u + n_b + (pos4[mv.a].x & 0xFFFFu), 1u + mv.fld_b);
+    if (fld) xlb = edge_from_xy(xy, 1u + n_b + (pos4[mv.a].x & 0xFFFFu), 1u + t);
   }
 
   // ---- untouched tours: the incumbent's values
@@ -391,59 +439,82 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
     if (g != ga && g != gb) { const double t_g = tst[2u * n_t + g]; if (t_g > makespan) makespan = t_g; }
   }
 
-  // ---- S4 pass 1 over the touched tours (L69, L106, L213); eq. (2) (L79)
-  uint32_t bad = mv.bad + MV_TAB(const uint32_t, M.off_misc)[1];
+  // ---- the two BPs of a field move: their mean field->BP leg, re-summed in the worker's order (L213)
+  double qA = 0.0, qT = 0.0;
+  uint32_t kA = 0, kT = 0;
+  if (fld) {
+    const uint2 bA = bp[A], bT = bp[t];
+    const uint32_t jA = bA.y & 0xFFu, jT = bT.y & 0xFFu;
+    auto mean_leg = [&](uint32_t ws, uint32_t k) -> double {
+      double sd = 0.0;
+      for (uint32_t p = ws; p < ws + k; ++p) sd = __dadd_rn(sd, (p == mv.c) ? xlb : leg2[map_idx(p)].y);
+      return div_small(sd, k, rcp);
+    };
+    if (A == t) { kA = bA.x >> 16; qA = mean_leg(bA.x & 0xFFFFu, kA); }
+    else {
+      kA = (bA.x >> 16) - 1u; kT = (bT.x >> 16) + 1u;
+      if (kA > 0u) qA = mean_leg((bA.x & 0xFFFFu) + (jT < jA ? 1u : 0u), kA);
+      qT = mean_leg((bT.x & 0xFFFFu) - (jA < jT ? 1u : 0u), kT);
+    }
+  }
+  // worker plan index -> incumbent plan index (a BP move relocates one BP in the plan order)
+  auto jmap = [&](uint32_t jj) -> uint32_t {
+    if (fld) return jj;
+    if (jj == mv.jq) return mv.jo;
+    if (mv.jq <= mv.jo) return (jj > mv.jq && jj <= mv.jo) ? jj - 1u : jj;
+    return (jj >= mv.jo && jj < mv.jq) ? jj + 1u : jj;
+  };
+
+  // ---- S4 for the touched tours (L69, L106, L213)
   double lt_a = 0.0, lt_b = 0.0, E_a = 0.0, E_b = 0.0;
+  uint32_t p0_a = 0, p0_b = 0;
   for (uint32_t r = 0; r < nr; ++r) {
     const uint32_t g = r ? gb : ga;
-    bad -= tbad[g];
-    uint32_t p = r ? wb_b : wb_a;
-    const uint32_t pe = r ? we_b : we_a;
-    uint32_t P0 = p, J0 = map_idx(p), P1 = Q1, J1 = K1, P2 = Q2, J2 = K2, P3 = Q3, J3 = K3;
-    double Y0 = 0.0, Y1 = X1, Y2 = X2, Y3 = X3;
-    if (p < pe) Y0 = edge_from_xy(xy, 0u, 1u + n_b + (pos4[J0].x & 0xFFFFu));   // HQ to the tour's first field (L21)
-    while (P1 < p) { P1 = P2; J1 = J2; Y1 = Y2; P2 = P3; J2 = J3; Y2 = Y3; P3 = kNone; }
-    uint32_t b_cur = kNone, Sq = 0, Hq = 0, k = 0, m = 0, x_last = 0, idx = 0;
-    double Lt = 0.0, sd = 0.0, sumE = 0.0;
-    for (; p < pe; ++p) {
-      ++idx;
-      bool exc = false;
-      double lh = 0.0;
-      if (__builtin_expect(p == P0, 0)) {
-        do { idx = J0; lh = Y0; P0 = P1; J0 = J1; Y0 = Y1; P1 = P2; J1 = J2; Y1 = Y2; P2 = P3; J2 = J3; Y2 = Y3; P3 = kNone; } while (p == P0);
-        exc = true;
-      }
-      const uint4 en = pos4[idx];
-      const double2 lg = leg2[idx];
-      uint32_t b = en.x >> 16;
-      double leg_h = lg.x, leg_b = lg.y;
-      if (exc) {                                   // the predecessor is not the incumbent's: HQ at the tour's start, or around the moved block
-        leg_h = lh;
-        if (fld && p == mv.c) { b = mv.fld_b; leg_b = xlb; }
-      }
-      if (__builtin_expect(b != b_cur, 0)) {
-        if (b_cur != kNone) { bad += (Sq < dq[b_cur]) ? 1u : 0u; sumE = __dadd_rn(sumE, div_small(sd, k, rcp)); ++m; }   // R10
-        b_cur = b; sd = 0.0; Sq = 0u; k = 0u;
-      }
-      Lt = __dadd_rn(Lt, leg_h);                                               // field to field (L69)
-      sd = __dadd_rn(sd, leg_b);
-      Hq += en.z; Sq += en.y; ++k;
-      x_last = en.x;
-    }
+    const uint32_t wb = r ? wb_b : wb_a, we = r ? we_b : we_a;
+    // E(g): the tour's BPs in the worker's plan order, each with its mean leg (R10: only BPs with fields)
     double E = 0.0;
-    if (b_cur != kNone) {
-      bad += (Sq < dq[b_cur]) ? 1u : 0u; sumE = __dadd_rn(sumE, div_small(sd, k, rcp)); ++m;
-      Lt = __dadd_rn(Lt, edge_from_xy(xy, 1u + n_b + (x_last & 0xFFFFu), 0u));  // back to HQ (L21; R2)
-      E = __ddiv_rn(__dmul_rn(2.0, div_small(sumE, m, rcp)), H.v_su);          // L199, L213; R9
+    {
+      const uint32_t tp = tpl[g];
+      uint32_t js = tp & 0xFFu, jl = tp >> 8;
+      if (!fld) { js = js - ((mv.g1 < g) ? 1u : 0u) + ((mv.g2 < g) ? 1u : 0u); jl = jl - ((g == mv.g1) ? 1u : 0u) + ((g == mv.g2) ? 1u : 0u); }
+      double sumE = 0.0; uint32_t m = 0;
+      for (uint32_t jj = js; jj < js + jl; ++jj) {
+        const uint32_t b = bpat[jmap(jj)];
+        uint32_t k = bp[b].x >> 16; double q = bpq[b];
+        if (fld) { if (b == A) { k = kA; q = qA; } else if (b == t) { k = kT; q = qT; } }
+        if (k > 0u) { sumE = __dadd_rn(sumE, q); ++m; }
+      }
+      if (m > 0u) E = __ddiv_rn(__dmul_rn(2.0, div_small(sumE, m, rcp)), H.v_su);    // L199, L213; R9
     }
+    // L_tour(g): the incumbent's running sum before the first changed position, the rest re-added in order
+    const uint2 rg = trng[g];
+    const uint32_t p0 = first_change(wb, we);
+    double Lt = (p0 - wb == rg.y - rg.x) ? tst[5u * n_t + g] : pre2[rg.x + (p0 - wb)].x;
+    {
+      uint32_t P1 = Q1, J1 = K1, P2 = Q2, J2 = K2, P3 = Q3, J3 = K3;
+      double Y1 = X1, Y2 = X2, Y3 = X3;
+      while (P1 < p0) { P1 = P2; J1 = J2; Y1 = Y2; P2 = P3; J2 = J3; Y2 = Y3; P3 = kNone; }
+      uint32_t idx = 0;
+      for (uint32_t p = p0; p < we; ++p) {
+        ++idx;
+        if (__builtin_expect(p == P1, 0)) {
+          double lh = 0.0;
+          do { idx = J1; lh = Y1; P1 = P2; J1 = J2; Y1 = Y2; P2 = P3; J2 = J3; Y2 = Y3; P3 = kNone; } while (p == P1);
+          Lt = __dadd_rn(Lt, lh);
+          continue;
+        }
+        Lt = __dadd_rn(Lt, leg2[idx].x);                                       // field to field (L69)
+      }
+    }
+    if (we > wb) Lt = __dadd_rn(Lt, edge_from_xy(xy, 1u + n_b + (pos4[map_idx(we - 1u)].x & 0xFFFFu), 0u));   // back to HQ (L21; R2)
+    const uint32_t Hq = thq[g] - ((g == mv.g1) ? h_blk : 0u) + ((g == mv.g2) ? h_blk : 0u);
     const uint2 hu = thu[g];
     const double t_g = __dadd_rn(__ddiv_rn(Lt, H.v_hu), __ddiv_rn((double)Hq, (double)hu.y));   // L190; R6
     if (t_g > makespan) makespan = t_g;
     const Mask<MASKW> mk = mask_load<MASKW>(s, M.m64_mask + MASKW * g);
     s.d(M.m64_w + g) = wait_time(E, tsn[g].x, cs[mask_top(mk)], hu.x, H.kappa, rcp);
-    if (r == 0u) { lt_a = Lt; E_a = E; } else { lt_b = Lt; E_b = E; }
+    if (r == 0u) { lt_a = Lt; E_a = E; p0_a = p0; } else { lt_b = Lt; E_b = E; p0_b = p0; }
   }
-  if (bad != 0u) return out;                                                   // discarded (L186; R19)
   auto E_of  = [&](uint32_t g) -> double { return g == ga ? E_a : (g == gb ? E_b : tst[n_t + g]); };
   auto lt_of = [&](uint32_t g) -> double { return g == ga ? lt_a : (g == gb ? lt_b : tst[g]); };
 
@@ -521,11 +592,17 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
     const bool recount = !(C_g == sn.x && n_g == sn.y);
     uint32_t p, pe;
     wrange(g, p, pe);
+    double shut = 0.0;
+    if (!recount) {                              // a touched tour under its old SU set: restart from the incumbent's prefix
+      const uint2 rg = trng[g];
+      const uint32_t p0 = (g == ga) ? p0_a : p0_b;
+      shut = (p0 - p == rg.y - rg.x) ? tst[4u * n_t + g] : pre2[rg.x + (p0 - p)].y;
+      p = p0;
+    }
     uint32_t P0 = p, J0 = map_idx(p), P1 = Q1, J1 = K1, P2 = Q2, J2 = K2, P3 = Q3, J3 = K3;
     while (P1 < p) { P1 = P2; J1 = J2; P2 = P3; J2 = J3; P3 = kNone; }
     uint32_t idx = 0;
     bool inblk = false;
-    double shut = 0.0;
     for (; p < pe; ++p) {
       ++idx;
       if (__builtin_expect(p == P0, 0)) {
@@ -676,7 +753,7 @@ __global__ void __launch_bounds__(kMvThreads, 1) lgx_local_search_k(const __grid
   mv_load_plan<MASKW>(P, sm, x_best, tid, T);
   mv_encode<MASKW>(P, sm, x_best, tid, T);
   if (tid == 0) {
-    const EvalOut r = mv_eval<MASKW>(P, sm, s, mv_identity(P, sm));
+    const EvalOut r = mv_eval<MASKW>(P, sm, s, mv_identity());
     s_cstar = (unsigned long long)__double_as_longlong(r.cost);
     if (r.feasible) {
       uint64_t *mk = reinterpret_cast<uint64_t *>(x_best + M.pl_mask);
