@@ -372,6 +372,75 @@ int lgo_su_local_min(int32_t n_tours, const double *E_h, const int32_t *n_hu,
   return m;
 }
 
+/* ------------------------------------------------------------------ embedded HU assignment (NEXT row N2) */
+
+/* "tours with minimum and maximum completion times, g_min and g_max, are identified, before
+ * their assigned number of HUs ... is decreased and increased by one HU, respectively.  This is repeated until
+ * the maximum completion time over all tours cannot be further reduced."  L203: for non-uniform HUs "an
+ * equivalent method is employed ... where the set of available HUs classes is now sorted according to rising
+ * in-field working rates".  Reading R39: the procedure is Algorithm 2 with the completion time
+ * T(g) = road_h(g) + H_q(g)/R_g in place of T_wait and the rates in place of the fill times: donor = the tour
+ * with the smallest T among the others, its units tried by rising (rate, index), the first that brings
+ * T(g_max) below T(g_2nd) or else the fastest is moved, the move is kept while the maximum T strictly
+ * decreases; a tour keeps >= 1 HU; at most N_HU moves.  Returns the accepted moves; T receives the final times. */
+static double tour_time(int g, double road_h, int64_t Hq, int n_hu, const int64_t *r_q, const uint8_t *hu_tour)
+{
+  int64_t R = 0;
+  for (int u = 0; u < n_hu; u++) if (hu_tour[u] == g) R += r_q[u];
+  return road_h + (double)Hq / (double)R;
+}
+
+static int hu_balance(int n_t, const double *road_h, const int64_t *Hq, int n_hu, const int64_t *r_q,
+                      uint8_t *hu_tour, double *T)
+{
+  int moves = 0;
+  for (int g = 0; g < n_t; g++) T[g] = tour_time(g, road_h[g], Hq[g], n_hu, r_q, hu_tour);
+  for (int iter = 0; iter < n_hu; iter++) {
+    if (n_t < 2) break;
+    for (int g = 0; g < n_t; g++) T[g] = tour_time(g, road_h[g], Hq[g], n_hu, r_q, hu_tour);
+    int g_max = 0;
+    for (int g = 1; g < n_t; g++) if (T[g] > T[g_max]) g_max = g;
+    double old_max = T[g_max];
+    int g_2nd = -1;
+    for (int g = 0; g < n_t; g++) if (g != g_max && (g_2nd < 0 || T[g] > T[g_2nd])) g_2nd = g;
+    int g_min = -1;
+    for (int g = 0; g < n_t; g++)
+      if (g != g_max && g != g_2nd && (g_min < 0 || T[g] < T[g_min])) g_min = g;
+    if (g_min < 0) g_min = g_2nd;
+    int n_min = 0;
+    for (int u = 0; u < n_hu; u++) if (hu_tour[u] == g_min) n_min++;
+    if (n_min <= 1) break;
+    int moved = -1;
+    uint8_t *tried = (uint8_t *)calloc((size_t)n_hu, 1);
+    for (int t = 0; t < n_min; t++) {
+      int u = -1;
+      for (int w = 0; w < n_hu; w++)
+        if (hu_tour[w] == g_min && !tried[w] && (u < 0 || r_q[w] < r_q[u])) u = w;
+      tried[u] = 1;
+      hu_tour[u] = (uint8_t)g_max;
+      double t_new = tour_time(g_max, road_h[g_max], Hq[g_max], n_hu, r_q, hu_tour);
+      if (t_new < T[g_2nd] || t == n_min - 1) { moved = u; break; }
+      hu_tour[u] = (uint8_t)g_min;
+    }
+    free(tried);
+    double new_max = 0.0;
+    for (int g = 0; g < n_t; g++) {
+      double t = tour_time(g, road_h[g], Hq[g], n_hu, r_q, hu_tour);
+      if (g == 0 || t > new_max) new_max = t;
+    }
+    if (new_max < old_max) moves++;
+    else { hu_tour[moved] = (uint8_t)g_min; break; }
+  }
+  for (int g = 0; g < n_t; g++) T[g] = tour_time(g, road_h[g], Hq[g], n_hu, r_q, hu_tour);
+  return moves;
+}
+
+int lgo_hu_balance(int32_t n_tours, const double *road_h, const int64_t *area_q, int32_t n_hu, const int64_t *rate_q,
+                   uint8_t *hu_tour, double *time_h)
+{
+  return hu_balance(n_tours, road_h, area_q, n_hu, rate_q, hu_tour, time_h);
+}
+
 /* ------------------------------------------------------------------ S4, S5, S7 */
 
 int lgo_score(const lgo_instance *I,
@@ -382,6 +451,23 @@ int lgo_score(const lgo_instance *I,
               double *tour_wait_h, double *tour_len_km, int64_t *bp_supply_q,
               int64_t *field_shuttles, uint8_t *su_tour_final)
 {
+  return lgo_score_ex(I, bp_tour, bp_pos, field_bp, field_pos, hu_tour, su_tour_init, 0, scalars, tour_route_km,
+                      tour_time_h, tour_E_h, tour_wait_h, tour_len_km, bp_supply_q, field_shuttles, su_tour_final, NULL);
+}
+
+/* lgo_score with the embedded HU assignment (hu_balance != 0: PAPER.md:L190, L203; R39) run between pass 1 and
+ * Algorithm 2 (the paper's order: "First, the assignment of HUs ... Second ... SUs", L190-192).
+ * hu_tour_final (may be NULL) receives the HU sets the cost was computed with. */
+int lgo_score_ex(const lgo_instance *I,
+              const uint8_t *bp_tour, const uint8_t *bp_pos,
+              const uint16_t *field_bp, const uint16_t *field_pos,
+              const uint8_t *hu_tour_in, const uint8_t *su_tour_init, int hu_balance_on,
+              double *scalars, double *tour_route_km, double *tour_time_h, double *tour_E_h,
+              double *tour_wait_h, double *tour_len_km, int64_t *bp_supply_q,
+              int64_t *field_shuttles, uint8_t *su_tour_final, uint8_t *hu_tour_final)
+{
+  const uint8_t *hu_tour = hu_tour_in;
+  uint8_t *hu_work = NULL;
   if (!I || !bp_tour || !bp_pos || !field_bp || !field_pos || !hu_tour || !su_tour_init || !scalars)
     return LGO_EINVAL;
   const int nt = I->n_t, nb = I->n_b, nf = I->n_f;
@@ -458,12 +544,27 @@ int lgo_score(const lgo_instance *I,
     for (int i = 1; i <= 6; i++) scalars[i] = INFINITY;
     scalars[7] = 0.0;
     if (su_tour_final) memcpy(su_tour_final, su, (size_t)I->n_su);
+    if (hu_tour_final) memcpy(hu_tour_final, hu_tour_in, (size_t)I->n_hu);
     if (tour_time_h) for (int g = 0; g < nt; g++) tour_time_h[g] = INFINITY;
     if (tour_wait_h) for (int g = 0; g < nt; g++) tour_wait_h[g] = INFINITY;
     if (tour_len_km) for (int g = 0; g < nt; g++) tour_len_km[g] = INFINITY;
     if (field_shuttles) for (int f = 0; f < nf; f++) field_shuttles[f] = 0;
     goto done;
   }
+
+  /* Embedded HU assignment (NEXT row N2; L190, L203; R39): before the SUs, as the paper lists them. */
+  if (hu_balance_on) {
+    hu_work = (uint8_t *)malloc((size_t)I->n_hu);
+    double *road = (double *)malloc(sizeof(double) * (size_t)nt), *Tt = (double *)malloc(sizeof(double) * (size_t)nt);
+    memcpy(hu_work, hu_tour_in, (size_t)I->n_hu);
+    for (int g = 0; g < nt; g++) road[g] = Lt[g] / I->v_hu;
+    hu_balance(nt, road, Hq, I->n_hu, I->r_q, hu_work, Tt);
+    free(road); free(Tt);
+    hu_tour = hu_work;
+    for (int g = 0; g < nt; g++) n_hu[g] = 0;
+    for (int u = 0; u < I->n_hu; u++) n_hu[hu_tour[u]]++;
+  }
+  if (hu_tour_final) memcpy(hu_tour_final, hu_tour, (size_t)I->n_hu);
 
   /* S6 — embedded local minimisation of the SU assignment (Algorithm 2). */
   int moves = su_local_min(nt, E, n_hu, I->n_su, I->c_q, su, I->kappa, W);
@@ -505,29 +606,30 @@ int lgo_score(const lgo_instance *I,
 
 done:
   free(tour_nbp); free(tour_bp); free(bp_nf); free(bp_field); free(n_hu); free(n_su);
-  free(Lt); free(E); free(W); free(Hq); free(Sq); free(su);
+  free(Lt); free(E); free(W); free(Hq); free(Sq); free(su); free(hu_work);
   return rc;
 }
 
 /* ------------------------------------------------------------------ batch + S8 */
 
 typedef struct {
-  uint8_t *bp_tour, *bp_pos, *hu_tour, *su_init, *su_final; uint16_t *field_bp, *field_pos;
+  uint8_t *bp_tour, *bp_pos, *hu_tour, *hu_final, *su_init, *su_final; uint16_t *field_bp, *field_pos;
 } plan_buf;
 
 static int plan_alloc(const lgo_instance *I, plan_buf *P)
 {
   P->bp_tour = (uint8_t *)malloc((size_t)I->n_b); P->bp_pos = (uint8_t *)malloc((size_t)I->n_b);
-  P->hu_tour = (uint8_t *)malloc((size_t)I->n_hu); P->su_init = (uint8_t *)malloc((size_t)I->n_su);
+  P->hu_tour = (uint8_t *)malloc((size_t)I->n_hu); P->hu_final = (uint8_t *)malloc((size_t)I->n_hu);
+  P->su_init = (uint8_t *)malloc((size_t)I->n_su);
   P->su_final = (uint8_t *)malloc((size_t)I->n_su);
   P->field_bp = (uint16_t *)malloc(sizeof(uint16_t) * (size_t)I->n_f);
   P->field_pos = (uint16_t *)malloc(sizeof(uint16_t) * (size_t)I->n_f);
-  return (P->bp_tour && P->bp_pos && P->hu_tour && P->su_init && P->su_final && P->field_bp && P->field_pos)
+  return (P->bp_tour && P->bp_pos && P->hu_tour && P->hu_final && P->su_init && P->su_final && P->field_bp && P->field_pos)
          ? LGO_OK : LGO_ENOMEM;
 }
 static void plan_free(plan_buf *P)
 {
-  free(P->bp_tour); free(P->bp_pos); free(P->hu_tour); free(P->su_init); free(P->su_final);
+  free(P->bp_tour); free(P->bp_pos); free(P->hu_tour); free(P->hu_final); free(P->su_init); free(P->su_final);
   free(P->field_bp); free(P->field_pos);
 }
 
@@ -757,8 +859,8 @@ static void worker_eval(const lgo_instance *I, const plan_buf *X, plan_buf *Y, u
   memcpy(Y->field_pos, X->field_pos, sizeof(uint16_t) * (size_t)I->n_f);
   memcpy(Y->hu_tour, X->hu_tour, (size_t)I->n_hu); memcpy(Y->su_init, X->su_init, (size_t)I->n_su);
   lgo_apply_move(I, w[0], w[1], w[2], Y->bp_tour, Y->bp_pos, Y->field_bp, Y->field_pos);
-  lgo_score(I, Y->bp_tour, Y->bp_pos, Y->field_bp, Y->field_pos, Y->hu_tour, Y->su_init, sc,
-            NULL, NULL, NULL, NULL, NULL, NULL, NULL, Y->su_final);
+  lgo_score_ex(I, Y->bp_tour, Y->bp_pos, Y->field_bp, Y->field_pos, Y->hu_tour, Y->su_init, (I->flags & LGO_FLAG_HU_BALANCE) != 0, sc,
+               NULL, NULL, NULL, NULL, NULL, NULL, NULL, Y->su_final, Y->hu_final);
 }
 
 int lgo_move_eval_batch(const lgo_instance *I,
@@ -808,10 +910,12 @@ int lgo_local_search(const lgo_instance *I,
   memcpy(best.field_bp, field_bp, nf2); memcpy(best.field_pos, field_pos, nf2);
   memcpy(best.hu_tour, hu_tour, (size_t)I->n_hu); memcpy(best.su_init, su_tour, (size_t)I->n_su);
   double sc[8];
-  int rc = lgo_score(I, best.bp_tour, best.bp_pos, best.field_bp, best.field_pos, best.hu_tour, best.su_init, sc,
-                     NULL, NULL, NULL, NULL, NULL, NULL, NULL, best.su_final);
+  int rc = lgo_score_ex(I, best.bp_tour, best.bp_pos, best.field_bp, best.field_pos, best.hu_tour, best.su_init,
+                        (I->flags & LGO_FLAG_HU_BALANCE) != 0, sc,
+                        NULL, NULL, NULL, NULL, NULL, NULL, NULL, best.su_final, best.hu_final);
   if (rc != LGO_OK) goto out;
   memcpy(best.su_init, best.su_final, (size_t)I->n_su);
+  memcpy(best.hu_tour, best.hu_final, (size_t)I->n_hu);
   double c_star = sc[6];
   PLAN_COPY(old, best);
   for (uint32_t k = 0; k < n_iters; k++) {
@@ -824,7 +928,10 @@ int lgo_local_search(const lgo_instance *I,
       uint64_t id = (uint64_t)k * n_workers + i;
       worker_eval(I, &cur, &Y, seed, id, sc);
       uint64_t bits; memcpy(&bits, &sc[6], 8);
-      if (!have || bits < bbits) { bbits = bits; bid = id; have = 1; PLAN_COPY(win, Y); memcpy(win.su_init, Y.su_final, (size_t)I->n_su); }
+      if (!have || bits < bbits) {
+        bbits = bits; bid = id; have = 1; PLAN_COPY(win, Y);
+        memcpy(win.su_init, Y.su_final, (size_t)I->n_su); memcpy(win.hu_tour, Y.hu_final, (size_t)I->n_hu);
+      }
     }
     double c_win; memcpy(&c_win, &bbits, 8);
     if (hist_cost) hist_cost[k] = c_win;

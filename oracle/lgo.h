@@ -23,6 +23,7 @@ extern "C" {
 #define LGO_ENOMEM  (-4)
 
 #define LGO_Q 1024   /* quanta per unit (t, ha, ha/h); R18 */
+#define LGO_FLAG_HU_BALANCE 2u   /* desc.flags bit 1: Algorithm 1's workers embed the HU assignment (N2; R39) */
 
 /* Same field order as the product's lgx_instance_desc (restated, not shared). */
 typedef struct {
@@ -77,6 +78,21 @@ int lgo_score(const lgo_instance *inst,
               int64_t *bp_supply_q,       /* [N_B] S_q(b)                    */
               int64_t *field_shuttles,    /* [N_F] eq. (4) count             */
               uint8_t *su_tour_final);    /* [N_SU]                          */
+
+/* lgo_score with the embedded HU assignment of PAPER.md:L190, L203 (R39) when hu_balance != 0; hu_tour_final
+ * (may be NULL) receives the HU sets the cost was computed with (= the input for an infeasible plan). */
+int lgo_score_ex(const lgo_instance *inst,
+                 const uint8_t *bp_tour, const uint8_t *bp_pos,
+                 const uint16_t *field_bp, const uint16_t *field_pos,
+                 const uint8_t *hu_tour, const uint8_t *su_tour_init, int hu_balance,
+                 double *scalars, double *tour_route_km, double *tour_time_h, double *tour_E_h,
+                 double *tour_wait_h, double *tour_len_km, int64_t *bp_supply_q,
+                 int64_t *field_shuttles, uint8_t *su_tour_final, uint8_t *hu_tour_final);
+
+/* The HU assignment alone on explicit numbers (for hand traces): road_h[g] = L_tour(g)/v_HU, area_q[g] = H_q(g),
+ * rate_q per unit; hu_tour in/out; time_h out = T(g); returns the accepted moves. */
+int lgo_hu_balance(int32_t n_tours, const double *road_h, const int64_t *area_q, int32_t n_hu, const int64_t *rate_q,
+                   uint8_t *hu_tour, double *time_h);
 
 /* S6 alone (Algorithm 2) on explicit numbers, for traces B and C.
  * cap_q: capacities in quanta; su_tour in/out; wait_h out; returns accepted moves.    */

@@ -43,6 +43,8 @@ _lib.lgo_quantum.restype = C.c_int64
 _lib.lgo_quantum.argtypes = [C.c_void_p, C.c_int, C.c_int32]
 _lib.lgo_decode.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64] + [C.c_void_p] * 6
 _lib.lgo_score.argtypes = [C.c_void_p] + [C.c_void_p] * 15
+_lib.lgo_score_ex.argtypes = [C.c_void_p] + [C.c_void_p] * 6 + [C.c_int] + [C.c_void_p] * 10
+_lib.lgo_hu_balance.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.lgo_su_local_min.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p,
                                   C.c_void_p, C.c_double, C.c_void_p]
 _lib.lgo_eval_batch.argtypes = [C.c_void_p, C.c_uint64, C.c_void_p, C.c_uint64, C.c_uint64] + [C.c_void_p] * 4
@@ -137,7 +139,7 @@ class Oracle:
         if rc: raise OracleError(rc)
         return dict(bp_tour=bt, bp_pos=bp, field_bp=fb, field_pos=fp, hu_tour=hu, su_tour=su)
 
-    def score(self, plan):
+    def score(self, plan, hu_balance=False):
         a = lambda k, t: np.ascontiguousarray(plan[k], dtype=t)
         bt, bp = a("bp_tour", np.uint8), a("bp_pos", np.uint8)
         fb, fp = a("field_bp", np.uint16), a("field_pos", np.uint16)
@@ -145,15 +147,15 @@ class Oracle:
         sc = np.zeros(8); nt = self.n_t
         route, time_h, E, W, Lg = (np.zeros(nt) for _ in range(5))
         Sq = np.zeros(self.n_b, np.int64); sh = np.zeros(self.n_f, np.int64)
-        suf = np.zeros(self.n_su, np.uint8)
-        rc = _lib.lgo_score(self._h, bt.ctypes.data, bp.ctypes.data, fb.ctypes.data, fp.ctypes.data,
-                            hu.ctypes.data, su.ctypes.data, sc.ctypes.data, route.ctypes.data,
-                            time_h.ctypes.data, E.ctypes.data, W.ctypes.data, Lg.ctypes.data,
-                            Sq.ctypes.data, sh.ctypes.data, suf.ctypes.data)
+        suf = np.zeros(self.n_su, np.uint8); huf = np.zeros(self.n_hu, np.uint8)
+        rc = _lib.lgo_score_ex(self._h, bt.ctypes.data, bp.ctypes.data, fb.ctypes.data, fp.ctypes.data,
+                               hu.ctypes.data, su.ctypes.data, 1 if hu_balance else 0, sc.ctypes.data, route.ctypes.data,
+                               time_h.ctypes.data, E.ctypes.data, W.ctypes.data, Lg.ctypes.data,
+                               Sq.ctypes.data, sh.ctypes.data, suf.ctypes.data, huf.ctypes.data)
         if rc: raise OracleError(rc)
         return dict(feasible=bool(sc[0]), L_HU=sc[1], L_eSU=sc[2], L_lSU=sc[3], path=sc[4],
                     makespan=sc[5], cost=sc[6], moves=int(sc[7]), route=route, T=time_h, E=E,
-                    wait=W, L=Lg, bp_supply_q=Sq, shuttles=sh, su_tour_final=suf)
+                    wait=W, L=Lg, bp_supply_q=Sq, shuttles=sh, su_tour_final=suf, hu_tour_final=huf)
 
     def score_fast(self, bt, bp, fb, fp, hu, su, sc):
         """score() without array outputs, on pre-typed contiguous arrays (brute force)."""
@@ -222,3 +224,13 @@ class Oracle:
                                    C.byref(c), hc.ctypes.data, hi.ctypes.data)
         if rc: raise OracleError(rc)
         return dict(zip([k for k, _ in PLAN_KEYS], a)), c.value, hc, hi
+
+
+def hu_balance(road_h, area_q, rate_q, hu_tour):
+    """The embedded HU assignment alone (R39) on explicit numbers.
+    Returns (moves, hu_tour, T)."""
+    road = np.ascontiguousarray(road_h, dtype=np.float64); nt = len(road)
+    aq = np.ascontiguousarray(area_q, dtype=np.int64); rq = np.ascontiguousarray(rate_q, dtype=np.int64)
+    hu = np.array(hu_tour, dtype=np.uint8, copy=True); T = np.zeros(nt)
+    m = _lib.lgo_hu_balance(nt, road.ctypes.data, aq.ctypes.data, len(rq), rq.ctypes.data, hu.ctypes.data, T.ctypes.data)
+    return m, hu, T
