@@ -29,6 +29,9 @@ extern "C" {
 #define LGX_ECUDA    (-3)   /* CUDA runtime error; text via lgx_strerror(LGX_ECUDA)          */
 #define LGX_ENOMEM   (-4)
 
+/* lgx_instance_desc.flags */
+#define LGX_FLAG_HU_BALANCE 2u   /* lgx_move_eval_batch / lgx_local_search embed the HU assignment of PAPER.md:L190, L203 */
+
 typedef struct lgx_instance lgx_instance;   /* opaque; owns host + device copies */
 
 /* Problem statement (Table 1 L51-65 and the list under it, L65; §2.1).
@@ -52,7 +55,7 @@ typedef struct {
   double   su_fill_h_per_t;                  /* kappa: t_SU^load = kappa * capacity (L96 (iii))  */
   double   w_path, w_time;                   /* cost = w_path*path_km + w_time*makespan_h (R1)   */
   uint32_t extra_field_thresh;               /* decoder knob: P(extra field) = thresh / 2^32     */
-  uint32_t flags;                            /* reserved, must be 0                              */
+  uint32_t flags;                            /* 0 or LGX_FLAG_HU_BALANCE (other bits: LGX_EINVAL) */
 } lgx_instance_desc;
 
 /* Instance encoder.  Quantises supply/area/demand/rate/capacity to Q=1024

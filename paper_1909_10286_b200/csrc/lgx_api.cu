@@ -112,7 +112,7 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   if (!(std::isfinite(d->v_hu_road_kmh) && d->v_hu_road_kmh > 0.0)) return LGX_EINVAL;
   if (!(std::isfinite(d->v_su_road_kmh) && d->v_su_road_kmh > 0.0)) return LGX_EINVAL;
   if (!fin_nonneg(d->su_fill_h_per_t) || !fin_nonneg(d->w_path) || !fin_nonneg(d->w_time)) return LGX_EINVAL;
-  if (d->flags != 0u) return LGX_EINVAL;
+  if ((d->flags & ~(uint32_t)LGX_FLAG_HU_BALANCE) != 0u) return LGX_EINVAL;
   const int nf = d->n_fields, nb = d->n_bps, nhu = d->n_hu_total, nsu = d->n_su_total, nt = d->n_tours;
   for (int f = 0; f < nf; ++f)
     if (!std::isfinite(d->field_x[f]) || !std::isfinite(d->field_y[f]) || !fin_nonneg(d->field_supply_t[f]) ||
@@ -145,6 +145,7 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   H.thresh = d->extra_field_thresh;
   H.v_hu = d->v_hu_road_kmh; H.v_su = d->v_su_road_kmh; H.kappa = d->su_fill_h_per_t;
   H.w_path = d->w_path; H.w_time = d->w_time;
+  H.flags = d->flags;
   H.perm16 = nf > 255 ? 1 : 0;
   H.mask_words = nsu > 64 ? 2u : 1u;
   const uint32_t MW = H.mask_words;
@@ -252,6 +253,9 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   H.offc_unit = off; off = align16(off + (uint32_t)nsu);
   H.offc_rank = off; off = align16(off + (uint32_t)nsu);
   H.offc_rq   = off; off = align16(off + 4u * (uint32_t)nhu);
+  H.offc_hrs  = off; off = align16(off + 4u * (uint32_t)nhu);
+  H.offc_hunit = off; off = align16(off + (uint32_t)nhu);
+  H.offc_hrank = off; off = align16(off + (uint32_t)nhu);
   H.imagec_bytes = off;
 
   I->image.assign(H.image_bytes, 0);
@@ -297,6 +301,13 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   for (int r = 0; r < nsu; ++r) {
     cc[r] = (uint32_t)c_q[order[r]];
     imc[H.offc_unit + r] = (uint8_t)order[r]; imc[H.offc_rank + order[r]] = (uint8_t)r;
+  }
+  {   // HUs ascending by (rate quanta, unit index): "sorted according to rising in-field working rates"
+    std::vector<int> ho(nhu);
+    std::iota(ho.begin(), ho.end(), 0);
+    std::stable_sort(ho.begin(), ho.end(), [&](int a, int b) { return r_q[a] < r_q[b]; });
+    uint32_t *hrs = reinterpret_cast<uint32_t *>(imc + H.offc_hrs);
+    for (int r = 0; r < nhu; ++r) { hrs[r] = (uint32_t)r_q[ho[r]]; imc[H.offc_hunit + r] = (uint8_t)ho[r]; imc[H.offc_hrank + ho[r]] = (uint8_t)r; }
   }
   double *rcp = reinterpret_cast<double *>(imc + H.offc_rcp);
   rcp[0] = 0.0;
@@ -360,10 +371,11 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
     M.off_cnt = o;   o = align16(o + 4u * (uint32_t)nb);
     M.off_tpl = o;   o = align16(o + 4u * (uint32_t)nt);
     M.off_thu = o;   o = align16(o + 8u * (uint32_t)nt);
+    M.off_thm = o;   o = align16(o + 8u * (uint32_t)nt);
     M.off_tsn = o;   o = align16(o + 8u * (uint32_t)nt);
     M.off_tmask = o; o = align16(o + 8u * (uint32_t)nt * MW);
     M.off_trng = o;  o = align16(o + 8u * (uint32_t)nt);
-    M.off_tst = o;   o = align16(o + 48u * (uint32_t)nt);
+    M.off_tst = o;   o = align16(o + 56u * (uint32_t)nt);
     M.off_thq = o;   o = align16(o + 4u * (uint32_t)nt);
     M.off_misc = o;  o = align16(o + 64u);
     M.off_sort = o;  o = align16(o + 4u * (kSortKeys + 1u));
@@ -372,20 +384,26 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
     q += (uint32_t)nb; M.pl_bpos = q; q += (uint32_t)nb; q = (q + 1u) & ~1u;
     M.pl_fbp = q; q += 2u * (uint32_t)nf; M.pl_fpos = q; q += 2u * (uint32_t)nf; q = (q + 7u) & ~7u;
     M.pl_mask = q; q += 8u * (uint32_t)nt * MW;
+    M.pl_hmask = q; q += 8u * (uint32_t)nt;
     M.plan_bytes = align16(q);
     M.off_plans = o; o += 3u * M.plan_bytes;
     M.off_state = o;
     uint32_t r = 0;
     M.m64_w = r; r += (uint32_t)nt;
-    M.m64_mask = r; r += (uint32_t)nt * MW; M.m64_bmask = r; r += (uint32_t)nt * MW; M.m64_rows = r;
+    M.m64_mask = r; r += (uint32_t)nt * MW; M.m64_bmask = r; r += (uint32_t)nt * MW;
+    const bool hb = (H.flags & LGX_FLAG_HU_BALANCE) != 0u;
+    if (hb) { M.m64_t = r; r += (uint32_t)nt; M.m64_hmask = r; r += (uint32_t)nt; M.m64_bhmask = r; r += (uint32_t)nt; }
+    M.m64_rows = r;
     r = 0;
-    M.m32_s = r; r += (uint32_t)nt; M.m32_rows = r;
-    M.slot_words = 2u + (uint32_t)nt * MW;
+    M.m32_s = r; r += (uint32_t)nt;
+    if (hb) { M.m32_r = r; r += (uint32_t)nt; }
+    M.m32_rows = r;
+    M.slot_words = 2u + (uint32_t)nt * MW + (uint32_t)nt;
     const int64_t mv_state = 8ll * M.m64_rows + 4ll * M.m32_rows;
     int64_t tm = (budget - 256 - (int64_t)M.off_state) / mv_state;      // static smem of the reductions
     tm = std::min<int64_t>(tm, kMvThreads) / 32 * 32;
     if (const char *ev = std::getenv("LGX_THREADS_MV")) { const int v = std::atoi(ev); if (v >= 64 && v <= tm) tm = v / 32 * 32; }
-    if (nt > 64) tm = 0;                                                  // the workers keep a 64-bit set of tours
+    if (nt > 64 || nhu > 64) tm = 0;                                      // 64-bit sets of tours and of HUs
     I->threads_mv = tm >= 64 ? (int)tm : 0;                               // 0: the move kernels do not fit (LGX_ETOOBIG there)
     I->smem_mv = (size_t)M.off_state + (size_t)mv_state * (size_t)std::max<int64_t>(tm, 0);
     std::vector<double> xy(2 * (size_t)(1 + nb + nf));
@@ -636,8 +654,11 @@ using MvKernelFn = void (*)(const MvParams);
 void pick_move_kernels(const ImgHdr &h, MvKernelFn &kb, MvKernelFn &ks)
 {
   kb = ks = nullptr;
-  if (h.mask_words == 1u) { kb = lgx_move_eval_k<1>; ks = lgx_local_search_k<1>; }
-  if (h.mask_words == 2u) { kb = lgx_move_eval_k<2>; ks = lgx_local_search_k<2>; }
+  const bool hb = (h.flags & LGX_FLAG_HU_BALANCE) != 0u;
+  if (h.mask_words == 1u && !hb) { kb = lgx_move_eval_k<1, false>; ks = lgx_local_search_k<1, false>; }
+  if (h.mask_words == 2u && !hb) { kb = lgx_move_eval_k<2, false>; ks = lgx_local_search_k<2, false>; }
+  if (h.mask_words == 1u && hb)  { kb = lgx_move_eval_k<1, true>;  ks = lgx_local_search_k<1, true>; }
+  if (h.mask_words == 2u && hb)  { kb = lgx_move_eval_k<2, true>;  ks = lgx_local_search_k<2, true>; }
 }
 
 // A plan is valid when every BP sits on exactly one tour at a unique position 0..len-1, every field on exactly

@@ -53,6 +53,10 @@ struct ImgHdr {
   uint32_t offc_dfb, offc_xy, offc_s, offc_cs, offc_rcp, offc_unit;
   uint32_t offc_rq;         // u32 [n_hu]  HU rate quanta
   uint32_t offc_rank;       // u8  [n_su]  unit -> rank
+  uint32_t offc_hrs;        // u32 [n_hu]  HU rate quanta by rank (ascending (rate, unit)): the embedded HU assignment (N2)
+  uint32_t offc_hunit;      // u8  [n_hu]  rank -> HU
+  uint32_t offc_hrank;      // u8  [n_hu]  HU -> rank
+  uint32_t flags;           // lgx_instance_desc.flags (bit 1: Algorithm 1's workers embed the HU assignment)
   uint32_t imagec_bytes;
 
   // ---- state rows of the decode/walk kernel

@@ -55,23 +55,25 @@ struct MvHdr {
   uint32_t off_bpat;    // u8 [n_b]       BP at plan index j
   uint32_t off_cnt;     // u32 [n_b]      scratch: fields per BP
   uint32_t off_tpl;     // u32 [n_t]      first plan index | BPs on the tour << 8
-  uint32_t off_thu;     // u32x2 [n_t]    n_HU(g), R_g (fixed during a search: R20)
+  uint32_t off_thu;     // u32x2 [n_t]    n_HU(g), R_g of the incumbent (fixed during a search unless the HU assignment is embedded: R20, R39)
+  uint32_t off_thm;     // u64 [n_t]      HU membership by rate rank
   uint32_t off_tsn;     // u32x2 [n_t]    S_g = capacity quanta of the tour's SUs, n_g = their number
   uint32_t off_tmask;   // u64 [n_t*MW]   SU membership by capacity rank
   uint32_t off_trng;    // u32x2 [n_t]    the tour's positions [begin, end) in plan order
-  uint32_t off_tst;     // f64 [6][n_t]   the incumbent's L_tour(g), E(g), T(g), T_wait(g), shuttle sum(g), route sum before the leg back to HQ
+  uint32_t off_tst;     // f64 [7][n_t]   the incumbent's L_tour(g), E(g), T(g), T_wait(g), shuttle sum(g), route sum before the leg back to HQ, L_tour(g)/v_HU
   uint32_t off_thq;     // u32 [n_t]      H_q(g)
   uint32_t off_misc;    // u32 [16]       [0] BPs that miss their demand (eq. (2)); [4..9] the move being applied
   uint32_t off_sort;    // u32 [kSortKeys + 1]  counting sort of a round's workers by the tours they touch
   uint32_t off_order;   // u16 [blockDim.x]     sorted worker of every thread
   uint32_t off_plans;   // 3 plans (x*, x_old, scratch); the batch kernel uses the first
-  uint32_t plan_bytes;  // one plan: bp_tour u8[n_b] | bp_pos u8[n_b] | field_bp u16[n_f] | field_pos u16[n_f] | masks u64[n_t*MW]
-  uint32_t pl_bpos, pl_fbp, pl_fpos, pl_mask;
+  uint32_t plan_bytes;  // one plan: bp_tour u8[n_b] | bp_pos u8[n_b] | field_bp u16[n_f] | field_pos u16[n_f] | SU masks u64[n_t*MW] | HU masks u64[n_t]
+  uint32_t pl_bpos, pl_fbp, pl_fpos, pl_mask, pl_hmask;
   uint32_t off_state;   // per-thread rows (64-bit region, then 32-bit region)
   uint32_t m64_w, m64_mask, m64_bmask, m64_rows;
   uint32_t m32_s, m32_rows;
-  uint32_t slot_words;  // 64-bit words per block slot: cost bits, id, masks
-  uint32_t pad_[3];
+  uint32_t m64_t, m64_hmask, m64_bhmask, m32_r;   // rows of the embedded HU assignment (only with LGX_FLAG_HU_BALANCE)
+  uint32_t slot_words;  // 64-bit words per block slot: cost bits, id, SU masks, HU masks
+  uint32_t pad_[2];
 };
 
 struct MvParams {
@@ -110,7 +112,7 @@ __device__ __forceinline__ uint32_t shuttle_count(uint32_t s_q, uint32_t n_g, ui
 // ------------------------------------------------------------------ plan -> shared memory
 
 // Copy the plan arrays from global memory into a plan slot; SU sets become masks over capacity ranks.
-// Also fills the per-tour HU table (n_HU(g), R_g = sum of rate quanta, L69; R7).
+// HU sets likewise, over rate ranks (at most 64 HUs).
 template <int MASKW>
 __device__ void mv_load_plan(const MvParams &P, uint8_t *sm, uint8_t *plan, uint32_t tid, uint32_t T)
 {
@@ -120,14 +122,12 @@ __device__ void mv_load_plan(const MvParams &P, uint8_t *sm, uint8_t *plan, uint
   uint16_t *fb = reinterpret_cast<uint16_t *>(plan + M.pl_fbp), *fp = reinterpret_cast<uint16_t *>(plan + M.pl_fpos);
   for (uint32_t f = tid; f < n_f; f += T) { fb[f] = P.field_bp[f]; fp[f] = P.field_pos[f]; }
   if (tid == 0) {
-    uint64_t *mk = reinterpret_cast<uint64_t *>(plan + M.pl_mask);
-    const uint8_t *rank_of = MV_CTAB(uint8_t, H.offc_rank);
-    const uint32_t *rq = MV_CTAB(uint32_t, H.offc_rq);
-    uint2 *thu = MV_TAB(uint2, M.off_thu);
+    uint64_t *mk = reinterpret_cast<uint64_t *>(plan + M.pl_mask), *hm = reinterpret_cast<uint64_t *>(plan + M.pl_hmask);
+    const uint8_t *rank_of = MV_CTAB(uint8_t, H.offc_rank), *hrank_of = MV_CTAB(uint8_t, H.offc_hrank);
     for (uint32_t i = 0; i < n_t * MASKW; ++i) mk[i] = 0ull;
-    for (uint32_t g = 0; g < n_t; ++g) thu[g] = make_uint2(0u, 0u);
+    for (uint32_t g = 0; g < n_t; ++g) hm[g] = 0ull;
     for (uint32_t u = 0; u < (uint32_t)H.n_su; ++u) { const uint32_t r = rank_of[u]; mk[P.su_tour[u] * MASKW + (r >> 6)] |= 1ull << (r & 63u); }
-    for (uint32_t u = 0; u < (uint32_t)H.n_hu; ++u) { uint2 &t = thu[P.hu_tour[u]]; t.x += 1u; t.y += rq[u]; }
+    for (uint32_t u = 0; u < (uint32_t)H.n_hu; ++u) hm[P.hu_tour[u]] |= 1ull << hrank_of[u];
   }
   __syncthreads();
 }
@@ -185,6 +185,14 @@ __device__ void mv_encode(const MvParams &P, uint8_t *sm, const uint8_t *plan, u
         while (w) { const int r = __ffsll((long long)w) - 1; w &= w - 1; S += cs[64 * i + r]; }
       }
       tsn[g] = make_uint2(S, n);
+      // n_HU(g), R_g = sum of the tour's rate quanta (L69; R7)
+      const uint32_t *hrs = MV_CTAB(uint32_t, H.offc_hrs);
+      uint64_t hw = reinterpret_cast<const uint64_t *>(plan + M.pl_hmask)[g];
+      MV_TAB(uint64_t, M.off_thm)[g] = hw;
+      uint32_t R = 0;
+      const uint32_t nh = (uint32_t)__popcll(hw);
+      while (hw) { const int r = __ffsll((long long)hw) - 1; hw &= hw - 1; R += hrs[r]; }
+      MV_TAB(uint2, M.off_thu)[g] = make_uint2(nh, R);
     }
   }
   __syncthreads();
@@ -259,7 +267,9 @@ __device__ void mv_encode(const MvParams &P, uint8_t *sm, const uint8_t *plan, u
 #pragma unroll
         for (int i = 0; i < MASKW; ++i) mk.w[i] = tmask[g * MASKW + i];
         tst[g] = Lt; tst[n_t + g] = E;
-        tst[2u * n_t + g] = __dadd_rn(__ddiv_rn(Lt, H.v_hu), __ddiv_rn((double)Hq, (double)hu.y));
+        const double road = __ddiv_rn(Lt, H.v_hu);
+        tst[2u * n_t + g] = __dadd_rn(road, __ddiv_rn((double)Hq, (double)hu.y));
+        tst[6u * n_t + g] = road;
         tst[3u * n_t + g] = wait_time(E, sn.x, cs[mask_top(mk)], hu.x, H.kappa, rcp);
         tst[4u * n_t + g] = shut;
         tst[5u * n_t + g] = lt_open;
@@ -342,7 +352,7 @@ struct EvalOut { bool feasible; double cost, path, makespan; };
 // touched tour the FP64 running sums restart from the incumbent's prefix value at the first position the move
 // changes (pre2) and only the rest of the tour is re-added in order; the mean legs of the two BPs a field move
 // changes are re-summed over those BPs alone; E(g) re-sums the tour's per-BP means.
-template <int MASKW>
+template <int MASKW, bool HB>
 __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm, const St &s, const Move &mv)
 {
   const ImgHdr &H = P.H; const MvHdr &M = P.M;
@@ -437,6 +447,7 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
 #pragma unroll
     for (int i = 0; i < MASKW; ++i) s.q(M.m64_mask + MASKW * g + i) = tmask[g * MASKW + i];
     if (g != ga && g != gb) { const double t_g = tst[2u * n_t + g]; if (t_g > makespan) makespan = t_g; }
+    if (HB) { s.d(M.m64_t + g) = tst[2u * n_t + g]; s.q(M.m64_hmask + g) = MV_TAB(const uint64_t, M.off_thm)[g]; s.w(M.m32_r + g) = thu[g].y; }
   }
 
   // ---- the two BPs of a field move: their mean field->BP leg, re-summed in the worker's order (L213)
@@ -466,8 +477,8 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
   };
 
   // ---- S4 for the touched tours (L69, L106, L213)
-  double lt_a = 0.0, lt_b = 0.0, E_a = 0.0, E_b = 0.0;
-  uint32_t p0_a = 0, p0_b = 0;
+  double lt_a = 0.0, lt_b = 0.0, E_a = 0.0, E_b = 0.0, road_a = 0.0, road_b = 0.0;
+  uint32_t p0_a = 0, p0_b = 0, hq_a = 0, hq_b = 0;
   for (uint32_t r = 0; r < nr; ++r) {
     const uint32_t g = r ? gb : ga;
     const uint32_t wb = r ? wb_b : wb_a, we = r ? we_b : we_a;
@@ -509,14 +520,68 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
     if (we > wb) Lt = __dadd_rn(Lt, edge_from_xy(xy, 1u + n_b + (pos4[map_idx(we - 1u)].x & 0xFFFFu), 0u));   // back to HQ (L21; R2)
     const uint32_t Hq = thq[g] - ((g == mv.g1) ? h_blk : 0u) + ((g == mv.g2) ? h_blk : 0u);
     const uint2 hu = thu[g];
-    const double t_g = __dadd_rn(__ddiv_rn(Lt, H.v_hu), __ddiv_rn((double)Hq, (double)hu.y));   // L190; R6
+    const double road = __ddiv_rn(Lt, H.v_hu);
+    const double t_g = __dadd_rn(road, __ddiv_rn((double)Hq, (double)hu.y));   // L190; R6
     if (t_g > makespan) makespan = t_g;
+    if (HB) s.d(M.m64_t + g) = t_g;
     const Mask<MASKW> mk = mask_load<MASKW>(s, M.m64_mask + MASKW * g);
     s.d(M.m64_w + g) = wait_time(E, tsn[g].x, cs[mask_top(mk)], hu.x, H.kappa, rcp);
-    if (r == 0u) { lt_a = Lt; E_a = E; p0_a = p0; } else { lt_b = Lt; E_b = E; p0_b = p0; }
+    if (r == 0u) { lt_a = Lt; E_a = E; p0_a = p0; road_a = road; hq_a = Hq; } else { lt_b = Lt; E_b = E; p0_b = p0; road_b = road; hq_b = Hq; }
   }
   auto E_of  = [&](uint32_t g) -> double { return g == ga ? E_a : (g == gb ? E_b : tst[n_t + g]); };
   auto lt_of = [&](uint32_t g) -> double { return g == ga ? lt_a : (g == gb ? lt_b : tst[g]); };
+  auto nhu_of = [&](uint32_t g) -> uint32_t { return HB ? (uint32_t)__popcll(s.q(M.m64_hmask + g)) : thu[g].x; };
+
+  // ---- the embedded HU assignment (N2; L190, L203; R39): Algorithm 2's procedure on T(g) = L_tour/v_HU + H_q/R_g,
+  // the donor's units tried by rising rate; before the SUs, as the paper lists them
+  if (HB) {
+    if (n_t >= 2u) {
+      const uint32_t *hrs = MV_CTAB(uint32_t, H.offc_hrs);
+      auto road_of = [&](uint32_t g) -> double { return g == ga ? road_a : (g == gb ? road_b : tst[6u * n_t + g]); };
+      auto hq_of   = [&](uint32_t g) -> double { return (double)(g == ga ? hq_a : (g == gb ? hq_b : thq[g])); };
+      bool changed = false;
+      for (uint32_t iter = 0; iter < (uint32_t)H.n_hu; ++iter) {
+        uint32_t g_max = 0, g_2nd = kNone; double t_max = s.d(M.m64_t), t_2nd = 0.0;
+        for (uint32_t g = 1; g < n_t; ++g) {
+          const double w = s.d(M.m64_t + g);
+          if (w > t_max) { t_2nd = t_max; g_2nd = g_max; t_max = w; g_max = g; }
+          else if (g_2nd == kNone || w > t_2nd) { t_2nd = w; g_2nd = g; }
+        }
+        uint32_t g_min = kNone; double t_min = 0.0;
+        for (uint32_t g = 0; g < n_t; ++g) {
+          const double w = s.d(M.m64_t + g);
+          if (g != g_max && g != g_2nd && (g_min == kNone || w < t_min)) { t_min = w; g_min = g; }
+        }
+        const bool two = (g_min == kNone);
+        if (two) g_min = g_2nd;
+        const uint64_t hm_min = s.q(M.m64_hmask + g_min);
+        if (__popcll(hm_min) <= 1) break;
+        const uint32_t R_max = s.w(M.m32_r + g_max);
+        const double road_max = road_of(g_max), hq_max = hq_of(g_max);
+        uint64_t rest = hm_min; int r; uint32_t rr; double t_new;
+        for (;;) {
+          r = __ffsll((long long)rest) - 1; rest &= rest - 1ull; rr = hrs[r];
+          t_new = __dadd_rn(road_max, __ddiv_rn(hq_max, (double)(R_max + rr)));
+          if (t_new < t_2nd || rest == 0ull) break;
+        }
+        const uint32_t R_min = s.w(M.m32_r + g_min) - rr;
+        const double t_don = __dadd_rn(road_of(g_min), __ddiv_rn(hq_of(g_min), (double)R_min));
+        double new_max = t_new > t_don ? t_new : t_don;
+        if (!two && t_2nd > new_max) new_max = t_2nd;
+        if (!(new_max < t_max)) break;
+        s.q(M.m64_hmask + g_min) = hm_min ^ (1ull << r); s.w(M.m32_r + g_min) = R_min; s.d(M.m64_t + g_min) = t_don;
+        s.q(M.m64_hmask + g_max) ^= (1ull << r);         s.w(M.m32_r + g_max) = R_max + rr; s.d(M.m64_t + g_max) = t_new;
+        changed = true;
+      }
+      if (changed)                                       // eq. (6) divides by the HU count (R7)
+        for (uint32_t g = 0; g < n_t; ++g) {
+          const Mask<MASKW> mk = mask_load<MASKW>(s, M.m64_mask + MASKW * g);
+          s.d(M.m64_w + g) = wait_time(E_of(g), tsn[g].x, cs[mask_top(mk)], nhu_of(g), H.kappa, rcp);
+        }
+    }
+    makespan = 0.0;
+    for (uint32_t g = 0; g < n_t; ++g) { const double t_g = s.d(M.m64_t + g); if (t_g > makespan) makespan = t_g; }
+  }
 
   // ---- S6: Algorithm 2 (L209-227), readings R11-R16 (same procedure as in lgx_finish)
   if (n_t >= 2u) {
@@ -538,7 +603,7 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
       if (mask_count(mk_min) <= 1) break;                                    // R15
       Mask<MASKW> mk_max = mask_load<MASKW>(s, M.m64_mask + MASKW * g_max);
       const uint32_t S_max = s.w(M.m32_s + g_max), M_max = cs[mask_top(mk_max)];
-      const uint32_t hu_max = thu[g_max].x;
+      const uint32_t hu_max = nhu_of(g_max);
       const double   E_max = E_of(g_max);
       // donor's units by rising fill time (L221): the first that brings T_wait(g_max) below T_wait(g_2nd),
       // else the largest (L225; R13).  The test is monotone in the capacity: bisect over the ranks.
@@ -565,7 +630,7 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
       }
       mask_flip(mk_min, r);
       const uint32_t S_min = s.w(M.m32_s + g_min) - cr;
-      const double w_don = wait_time(E_of(g_min), S_min, cs[mask_top(mk_min)], thu[g_min].x, H.kappa, rcp);
+      const double w_don = wait_time(E_of(g_min), S_min, cs[mask_top(mk_min)], nhu_of(g_min), H.kappa, rcp);
       double new_max = w_new > w_don ? w_new : w_don;                        // step 11 (L227; R14)
       if (!two && w_2nd > new_max) new_max = w_2nd;
       if (!(new_max < w_max)) break;
@@ -625,7 +690,7 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
   for (uint32_t g = 0; g < n_t; ++g) {
     const double lt = lt_of(g), shut = s.d(M.m64_w + g);
     const uint32_t n_g = (uint32_t)mask_count(mask_load<MASKW>(s, M.m64_mask + MASKW * g));
-    const double l_hu  = __dmul_rn((double)thu[g].x, lt);
+    const double l_hu  = __dmul_rn((double)nhu_of(g), lt);
     const double l_esu = __dadd_rn(__dmul_rn((double)n_g, lt), shut);
     path = __dadd_rn(path, __dadd_rn(__dadd_rn(l_hu, l_esu), shut));
   }
@@ -699,7 +764,7 @@ __device__ __forceinline__ uint32_t mv_sort_round(const MvParams &P, uint8_t *sm
 
 // ================================================================== batch kernel (L163-165)
 
-template <int MASKW>
+template <int MASKW, bool HB>
 __global__ void __launch_bounds__(kMvThreads, 1) lgx_move_eval_k(const __grid_constant__ MvParams P)
 {
   extern __shared__ __align__(16) uint8_t smem[];
@@ -719,7 +784,7 @@ __global__ void __launch_bounds__(kMvThreads, 1) lgx_move_eval_k(const __grid_co
     uint32_t w[4];
     philox_block(P, (uint32_t)id, (uint32_t)(id >> 32), 5u, 0u, w);
     const Move mv = mv_derive(P, sm, w[0], w[1], w[2], nullptr);
-    const EvalOut r = mv_eval<MASKW>(P, sm, s, mv);
+    const EvalOut r = mv_eval<MASKW, HB>(P, sm, s, mv);
     if (P.cost)       P.cost[i] = r.cost;
     if (P.path_km)    P.path_km[i] = r.path;
     if (P.makespan_h) P.makespan_h[i] = r.makespan;
@@ -729,7 +794,7 @@ __global__ void __launch_bounds__(kMvThreads, 1) lgx_move_eval_k(const __grid_co
 
 // ================================================================== Algorithm 1 steps 4-16, persistent
 
-template <int MASKW>
+template <int MASKW, bool HB>
 __global__ void __launch_bounds__(kMvThreads, 1) lgx_local_search_k(const __grid_constant__ MvParams P)
 {
   extern __shared__ __align__(16) uint8_t smem[];
@@ -753,11 +818,12 @@ __global__ void __launch_bounds__(kMvThreads, 1) lgx_local_search_k(const __grid
   mv_load_plan<MASKW>(P, sm, x_best, tid, T);
   mv_encode<MASKW>(P, sm, x_best, tid, T);
   if (tid == 0) {
-    const EvalOut r = mv_eval<MASKW>(P, sm, s, mv_identity());
+    const EvalOut r = mv_eval<MASKW, HB>(P, sm, s, mv_identity());
     s_cstar = (unsigned long long)__double_as_longlong(r.cost);
     if (r.feasible) {
       uint64_t *mk = reinterpret_cast<uint64_t *>(x_best + M.pl_mask);
       for (uint32_t i = 0; i < n_t * MASKW; ++i) mk[i] = s.q(M.m64_mask + i);
+      if (HB) { uint64_t *hm = reinterpret_cast<uint64_t *>(x_best + M.pl_hmask); for (uint32_t g = 0; g < n_t; ++g) hm[g] = s.q(M.m64_hmask + g); }
     }
   }
   __syncthreads();
@@ -783,11 +849,14 @@ __global__ void __launch_bounds__(kMvThreads, 1) lgx_local_search_k(const __grid
       uint32_t w[4];
       philox_block(P, (uint32_t)id, (uint32_t)(id >> 32), 5u, 0u, w);
       const Move mv = mv_derive(P, sm, w[0], w[1], w[2], nullptr);
-      const EvalOut r = mv_eval<MASKW>(P, sm, s, mv);
+      const EvalOut r = mv_eval<MASKW, HB>(P, sm, s, mv);
       const unsigned long long bits = (unsigned long long)__double_as_longlong(r.cost);
       if (bits < best_bits || (bits == best_bits && id < best_id)) {
         best_bits = bits; best_id = id;
-        if (r.feasible) for (uint32_t q = 0; q < n_t * MASKW; ++q) s.q(M.m64_bmask + q) = s.q(M.m64_mask + q);
+        if (r.feasible) {
+          for (uint32_t q = 0; q < n_t * MASKW; ++q) s.q(M.m64_bmask + q) = s.q(M.m64_mask + q);
+          if (HB) for (uint32_t g = 0; g < n_t; ++g) s.q(M.m64_bhmask + g) = s.q(M.m64_hmask + g);
+        }
       }
     }
     // ---- step 13 (L167): i* = arg min C_i.  warp -> block -> one slot per block -> grid barrier -> every block folds
@@ -813,7 +882,10 @@ __global__ void __launch_bounds__(kMvThreads, 1) lgx_local_search_k(const __grid
     unsigned long long *slot = P.slots + ((size_t)(k & 1u) * gridDim.x + blockIdx.x) * SW;
     if (tid == 0u) { slot[0] = s_win[0]; slot[1] = s_win[1]; }
     if (best_id == s_win[1] && best_id != ~0ull)                             // the block's winner publishes its SU sets
+    {
       for (uint32_t q = 0; q < n_t * MASKW; ++q) slot[2 + q] = s.q(M.m64_bmask + q);
+      if (HB) for (uint32_t g = 0; g < n_t; ++g) slot[2 + n_t * MASKW + g] = s.q(M.m64_bhmask + g);
+    }
     grid.sync();
     if (tid < 32u) {
       const unsigned long long *all = P.slots + (size_t)(k & 1u) * gridDim.x * SW;
@@ -870,6 +942,7 @@ __global__ void __launch_bounds__(kMvThreads, 1) lgx_local_search_k(const __grid
         const unsigned long long *wm = P.slots + ((size_t)(k & 1u) * gridDim.x + (size_t)s_win[2]) * SW + 2;
         uint64_t *mk = reinterpret_cast<uint64_t *>(x_tmp + M.pl_mask);
         for (uint32_t q = tid; q < n_t * MASKW; q += T) mk[q] = __ldcg(wm + q);
+        if (HB) { uint64_t *hm = reinterpret_cast<uint64_t *>(x_tmp + M.pl_hmask); for (uint32_t g = tid; g < n_t; g += T) hm[g] = __ldcg(wm + n_t * MASKW + g); }
       }
       __syncthreads();
       const bool improves = win_bits < s_cstar;
@@ -893,6 +966,9 @@ __global__ void __launch_bounds__(kMvThreads, 1) lgx_local_search_k(const __grid
           uint64_t w = mk[g * MASKW + i];
           while (w) { const int r = __ffsll((long long)w) - 1; w &= w - 1; P.su_tour[unit_of[64 * i + r]] = (uint8_t)g; }
         }
+      const uint64_t *hm = reinterpret_cast<const uint64_t *>(x_best + M.pl_hmask);
+      const uint8_t *hunit_of = MV_CTAB(uint8_t, H.offc_hunit);
+      for (uint32_t g = 0; g < n_t; ++g) { uint64_t w = hm[g]; while (w) { const int r = __ffsll((long long)w) - 1; w &= w - 1; P.hu_tour[hunit_of[r]] = (uint8_t)g; } }
       *P.best_cost = __longlong_as_double((long long)s_cstar);
     }
   }

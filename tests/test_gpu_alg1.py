@@ -176,3 +176,31 @@ def test_local_search_edge_cases(ctxs):
     got = gt.local_search(pt, 2, 30, 64, 0x40000000)
     assert np.array_equal(got[3], want[3]) and np.array_equal(got[2], want[2]) and got[1] == want[1]
     assert_plan_equal(got[0], want[0], "toy/infeasible start")
+
+
+@pytest.mark.parametrize("name,n,n_iters,n_workers", [("toy", 4096, 30, 100), ("small", 8192, 40, 300), ("medium", 8192, 20, 1000),
+                                                      ("sweep", 1024, 3, 400), ("paper_scale", 2048, 4, 600)])
+def test_embedded_hu_assignment_matches_oracle(name, n, n_iters, n_workers):
+    """NEXT row N2 (R39): with LGX_FLAG_HU_BALANCE the workers rebalance the HUs before
+    Algorithm 2; x_{i*} carries the HU sets it was scored with."""
+    from dataclasses import replace
+    inst = replace(wl.make(name), flags=2)
+    o, g = lgo.Oracle(inst), binding.Instance(inst)
+    p0 = o.init_plan()
+    w = check_move_eval(o, g, p0, 7, 0, n, f"{name}/hb/init")
+    check_move_eval(o, g, o.decode(inst.seed, 4242), 9, 1 << 33, min(n, 2048), f"{name}/hb/sampled")
+    base = lgo.Oracle(wl.make(name)).move_eval_batch(p0, 7, 0, n)
+    if name != "toy" and o.n_hu > o.n_t:                            # (paper_scale has one HU per tour: nothing can move)
+        assert not np.array_equal(base[2], w[2])                    # the flag changes makespans
+    for eps in (0, 0x66666666):
+        want_p, want_c, want_hc, want_hi = o.local_search(p0, 3, n_iters, n_workers, eps)
+        got_p, got_c, got_hc, got_hi = g.local_search(p0, 3, n_iters, n_workers, eps)
+        assert np.array_equal(got_hi, want_hi), f"{name}: winners differ (first at iteration {int(np.argmax(got_hi != want_hi))})"
+        assert_costs(got_hc, want_hc, f"{name}/hb/hist_cost")
+        assert got_c == want_c
+        assert_plan_equal(got_p, want_p, f"{name}/hb")
+    # n_iters = 0: x_0 takes the balanced HU sets
+    got_p, got_c, _, _ = g.local_search(p0, 1, 0, 64, 0)
+    r = o.score(p0, hu_balance=True)
+    assert (got_c == r["cost"] or (np.isinf(got_c) and not r["feasible"])) and np.array_equal(got_p["hu_tour"], r["hu_tour_final"])
+    g.close()
