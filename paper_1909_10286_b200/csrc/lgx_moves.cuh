@@ -63,8 +63,8 @@ struct MvHdr {
   uint32_t off_tst;     // f64 [7][n_t]   the incumbent's L_tour(g), E(g), T(g), T_wait(g), shuttle sum(g), route sum before the leg back to HQ, L_tour(g)/v_HU
   uint32_t off_thq;     // u32 [n_t]      H_q(g)
   uint32_t off_misc;    // u32 [16]       [0] BPs that miss their demand (eq. (2)); [4..9] the move being applied
-  uint32_t off_sort;    // u32 [kSortKeys + 1]  counting sort of a round's workers by the tours they touch
-  uint32_t off_order;   // u16 [blockDim.x]     sorted worker of every thread
+  uint32_t off_sort;    // u32 [kSortKeys + 2]  counting sort of the workers by the tours they touch; the warps' draw counter
+  uint32_t off_order;   // u16 [kSuper * 1024]  sorted workers: round << 10 | thread
   uint32_t off_plans;   // 3 plans (x*, x_old, scratch); the batch kernel uses the first
   uint32_t plan_bytes;  // one plan: bp_tour u8[n_b] | bp_pos u8[n_b] | field_bp u16[n_f] | field_pos u16[n_f] | SU masks u64[n_t*MW] | HU masks u64[n_t]
   uint32_t pl_bpos, pl_fbp, pl_fpos, pl_mask, pl_hmask;
@@ -722,44 +722,71 @@ __device__ __forceinline__ void mv_prologue(const MvParams &P, uint8_t *sm, St &
   __syncthreads();
 }
 
-// One round of a block = up to blockDim.x consecutive worker ids.  Which thread scores which worker is free, so the
-// round's workers are counting-sorted by the tours their moves touch: the lanes of a warp then walk the same tours
-// (equal trip counts, the same shared-memory words, BP boundaries at the same steps, similar Algorithm-2 paths).
-// Returns the worker (index within the round) this thread scores, or kNone.  Block-wide (barriers inside).
-__device__ __forceinline__ uint32_t mv_sort_round(const MvParams &P, uint8_t *sm, uint64_t id_base, uint32_t n_round, uint32_t tid, uint32_t T)
+// A block's share of n_total workers = rounds of blockDim.x consecutive indices, gridDim.x * blockDim.x apart.
+// Which lane scores which worker is free, so up to kSuper rounds at a time are counting-sorted by the tours their
+// moves touch — the lanes of a warp then walk the same tours (equal trip counts, the same shared-memory words,
+// similar Algorithm-2 paths) — and the warps DRAW chunks of 32 sorted workers from a shared counter, so a warp
+// stuck with expensive workers does not hold the others at a barrier.  eval(i) scores worker index i.
+constexpr uint32_t kSuper = 8;                  // rounds sorted and scheduled together (order: u16 [kSuper * 1024])
+
+template <class F>
+__device__ __forceinline__ void mv_for_workers(const MvParams &P, uint8_t *sm, uint64_t id0, uint64_t n_total,
+                                               uint32_t tid, uint32_t T, F &&eval)
 {
   const uint32_t n_t = P.H.n_t;
   const uint32_t nk = (n_t <= 16u) ? n_t * n_t : n_t;
-  uint32_t *hist = MV_TAB(uint32_t, P.M.off_sort);
+  uint32_t *hist = MV_TAB(uint32_t, P.M.off_sort);       // [nk + 2]: offsets per key, total, the warps' draw counter
   uint16_t *order = MV_TAB(uint16_t, P.M.off_order);
-  for (uint32_t k = tid; k <= nk; k += T) hist[k] = 0u;
-  __syncthreads();
-  uint32_t key = nk;
-  if (tid < n_round) {
-    const uint64_t id = id_base + tid;
-    uint32_t w[4];
-    philox_block(P, (uint32_t)id, (uint32_t)(id >> 32), 5u, 0u, w);
-    const Move mv = mv_derive(P, sm, w[0], w[1], w[2], nullptr);
-    const uint32_t ga = min(mv.g1, mv.g2), gb = max(mv.g1, mv.g2);
-    key = (n_t <= 16u) ? ga * n_t + gb : ga;
-  }
-  const uint32_t rank = atomicAdd(&hist[key], 1u);
-  __syncthreads();
-  if (tid < 32u) {                                   // exclusive scan of the histogram
-    const uint32_t per = (nk + 1u + 31u) / 32u, k0 = tid * per;
-    uint32_t sum = 0;
-    for (uint32_t k = k0; k < k0 + per && k <= nk; ++k) sum += hist[k];
-    uint32_t incl = sum;
+  const uint64_t stride = (uint64_t)gridDim.x * T;
+  const uint32_t lane = tid & 31u;
+  for (uint64_t base = (uint64_t)blockIdx.x * T; base < n_total; base += (uint64_t)kSuper * stride) {
+    for (uint32_t k = tid; k <= nk + 1u; k += T) hist[k] = 0u;
+    __syncthreads();
+    uint32_t key[kSuper], rank[kSuper];
 #pragma unroll
-    for (int off = 1; off < 32; off <<= 1) { const uint32_t o = __shfl_up_sync(0xFFFFFFFFu, incl, off); if ((int)tid >= off) incl += o; }
-    uint32_t run = incl - sum;
-    for (uint32_t k = k0; k < k0 + per && k <= nk; ++k) { const uint32_t h = hist[k]; hist[k] = run; run += h; }
+    for (uint32_t r = 0; r < kSuper; ++r) {
+      const uint64_t i = base + (uint64_t)r * stride + tid;
+      key[r] = kNone; rank[r] = 0u;
+      if (i < n_total) {
+        const uint64_t id = id0 + i;
+        uint32_t w[4];
+        philox_block(P, (uint32_t)id, (uint32_t)(id >> 32), 5u, 0u, w);
+        const Move mv = mv_derive(P, sm, w[0], w[1], w[2], nullptr);
+        const uint32_t ga = min(mv.g1, mv.g2), gb = max(mv.g1, mv.g2);
+        key[r] = (n_t <= 16u) ? ga * n_t + gb : ga;
+        rank[r] = atomicAdd(&hist[key[r]], 1u);
+      }
+    }
+    __syncthreads();
+    if (tid < 32u) {                                   // exclusive scan of the histogram; hist[nk] = number of workers
+      const uint32_t per = (nk + 1u + 31u) / 32u, k0 = tid * per;
+      uint32_t sum = 0;
+      for (uint32_t k = k0; k < k0 + per && k <= nk; ++k) sum += hist[k];
+      uint32_t incl = sum;
+#pragma unroll
+      for (int off = 1; off < 32; off <<= 1) { const uint32_t o = __shfl_up_sync(0xFFFFFFFFu, incl, off); if ((int)tid >= off) incl += o; }
+      uint32_t run = incl - sum;
+      for (uint32_t k = k0; k < k0 + per && k <= nk; ++k) { const uint32_t h = hist[k]; hist[k] = run; run += h; }
+    }
+    __syncthreads();
+#pragma unroll
+    for (uint32_t r = 0; r < kSuper; ++r)
+      if (key[r] != kNone) order[hist[key[r]] + rank[r]] = (uint16_t)((r << 10) | tid);
+    __syncthreads();
+    const uint32_t n_local = hist[nk];
+    for (;;) {
+      uint32_t c = 0;
+      if (lane == 0u) c = atomicAdd(&hist[nk + 1u], 32u);
+      c = __shfl_sync(0xFFFFFFFFu, c, 0);
+      if (c >= n_local) break;
+      if (c + lane < n_local) {
+        const uint32_t L = order[c + lane];
+        eval(base + (uint64_t)(L >> 10) * stride + (L & 1023u));
+      }
+      __syncwarp();
+    }
+    __syncthreads();
   }
-  __syncthreads();
-  order[hist[key] + rank] = (uint16_t)tid;
-  __syncthreads();
-  const uint32_t j = order[tid];
-  return j < n_round ? j : kNone;
 }
 
 // ================================================================== batch kernel (L163-165)
@@ -775,12 +802,8 @@ __global__ void __launch_bounds__(kMvThreads, 1) lgx_move_eval_k(const __grid_co
   uint8_t *plan = sm + P.M.off_plans;
   mv_load_plan<MASKW>(P, sm, plan, tid, T);
   mv_encode<MASKW>(P, sm, plan, tid, T);
-  const uint64_t stride = (uint64_t)gridDim.x * T;
-  for (uint64_t base = (uint64_t)blockIdx.x * T; base < P.n; base += stride) {
-    const uint32_t n_round = (uint32_t)min((uint64_t)T, P.n - base);
-    const uint32_t j = mv_sort_round(P, sm, P.first_id + base, n_round, tid, T);
-    if (j == kNone) continue;
-    const uint64_t i = base + j, id = P.first_id + i;
+  mv_for_workers(P, sm, P.first_id, P.n, tid, T, [&](uint64_t i) {
+    const uint64_t id = P.first_id + i;
     uint32_t w[4];
     philox_block(P, (uint32_t)id, (uint32_t)(id >> 32), 5u, 0u, w);
     const Move mv = mv_derive(P, sm, w[0], w[1], w[2], nullptr);
@@ -789,7 +812,7 @@ __global__ void __launch_bounds__(kMvThreads, 1) lgx_move_eval_k(const __grid_co
     if (P.path_km)    P.path_km[i] = r.path;
     if (P.makespan_h) P.makespan_h[i] = r.makespan;
     if (P.feasible)   P.feasible[i] = r.feasible ? 1 : 0;
-  }
+  });
 }
 
 // ================================================================== Algorithm 1 steps 4-16, persistent
@@ -841,11 +864,8 @@ __global__ void __launch_bounds__(kMvThreads, 1) lgx_local_search_k(const __grid
     // ---- steps 7-12: every worker moves x once and scores it; running (cost, id) minimum per thread
     unsigned long long best_bits = ~0ull, best_id = ~0ull;
     const uint64_t id0 = (uint64_t)k * P.n_workers;
-    for (uint64_t base = (uint64_t)blockIdx.x * T; base < P.n_workers; base += (uint64_t)gridDim.x * T) {
-      const uint32_t n_round = (uint32_t)min((uint64_t)T, (uint64_t)P.n_workers - base);
-      const uint32_t j = mv_sort_round(P, sm, id0 + base, n_round, tid, T);
-      if (j == kNone) continue;
-      const uint64_t id = id0 + base + j;
+    mv_for_workers(P, sm, id0, (uint64_t)P.n_workers, tid, T, [&](uint64_t i) {
+      const uint64_t id = id0 + i;
       uint32_t w[4];
       philox_block(P, (uint32_t)id, (uint32_t)(id >> 32), 5u, 0u, w);
       const Move mv = mv_derive(P, sm, w[0], w[1], w[2], nullptr);
@@ -858,7 +878,7 @@ __global__ void __launch_bounds__(kMvThreads, 1) lgx_local_search_k(const __grid
           if (HB) for (uint32_t g = 0; g < n_t; ++g) s.q(M.m64_bhmask + g) = s.q(M.m64_hmask + g);
         }
       }
-    }
+    });
     // ---- step 13 (L167): i* = arg min C_i.  warp -> block -> one slot per block -> grid barrier -> every block folds
     unsigned long long bb = best_bits, bi = best_id;
 #pragma unroll

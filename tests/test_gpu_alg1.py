@@ -116,10 +116,13 @@ def test_move_eval_degenerate_plans(ctxs):
     pm = om.init_plan()
     for n in (1, 31, 33, 511, 513):
         check_move_eval(om, gm, pm, 1, 3, n, f"medium/n{n}")
-    n = 148 * 512 + 1
-    got = gm.move_eval_batch(pm, 1, 3, n)[0].cpu().numpy()
-    want = om.move_eval_batch(pm, 1, 3 + n - 64, 64)[0]
-    assert np.array_equal(got[-64:], want)
+    for n in (148 * 512 + 1, 148 * 512 * 8 + 700):           # two rounds; more rounds than one sorted super-round
+        got = gm.move_eval_batch(pm, 1, 3, n)[0].cpu().numpy()
+        want = om.move_eval_batch(pm, 1, 3 + n - 64, 64)[0]
+        assert np.array_equal(got[-64:], want)
+        mid = n // 2
+        want = om.move_eval_batch(pm, 1, 3 + mid, 64)[0]
+        assert np.array_equal(got[mid:mid + 64], want)
 
 
 def test_invalid_plans_are_rejected(ctxs):
