@@ -44,6 +44,10 @@ def w_alg(inst, workload):
 
 
 SM_MAX_MHZ_FALLBACK = 1965.0
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE lgx_decode_walk launch (757 760 Medium candidates) from the
+# `ncu --set full` capture summarised in profiles/r01_v7_medium_ncu_full.md: 0.12 MB read + 4.08 MB written (the
+# queue records of the feasible candidates that do not stay in L2).  Per launch, like `achieved`.
+TRAFFIC_BYTES_DECODE_WALK_MEDIUM = 4.20e6
 
 
 def peaks():
@@ -138,7 +142,7 @@ def bench_alg1(args, torch, binding, wl):
         g.move_eval_batch(p0, 1, 0, n, out=out)
     b.record(stream); torch.cuda.synchronize()
     ms_batch = a.elapsed_time(b) / 3
-    n_workers, eps = sm * tmv, 0.4
+    n_workers, eps = sm * tmv * 8, 0.4        # 8 rounds per block and iteration: the warps balance them dynamically
     c0 = g.local_search(p0, inst.seed, 0, 1, 0, history=False)[1]
     g.local_search(p0, inst.seed, 10, n_workers, int(eps * 2**32), history=False)          # warm-up
     t0 = time.perf_counter()
@@ -204,7 +208,7 @@ def main():
     ap.add_argument("--batch-log2", type=int, default=None, help="candidates per GPU per step (default: config budget, capped 2^28)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--alg1-workload", default="paper_scale", help="instance of the Algorithm 1 leg (SURVEY §8(f) N1/N3)")
-    ap.add_argument("--alg1-iters", type=int, default=1000)
+    ap.add_argument("--alg1-iters", type=int, default=500)
     ap.add_argument("--no-alg1", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "lgx" else args.warmup
@@ -273,15 +277,21 @@ def main():
 
     # ---- e2e: host arrays -> lgx_instance_create (H2D image) -> lgx_search -> host result
     e2e_steps = max(2, min(args.steps, 3))
+
+    def e2e_step():
+        g2 = binding.Instance(inst)
+        if world == 1:
+            r = g2.search(inst.seed, per_gpu)
+        else:
+            r = sharding.search_sharded(lambda s, n, f: g2.search(s, n, first_id=f), inst.seed, total, rank, world)
+        g2.close()
+        return r
+
+    e2e_step()                                   # untimed warm-up of the create/destroy path
     barrier()
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
-        g2 = binding.Instance(inst)
-        if world == 1:
-            r2 = g2.search(inst.seed, per_gpu)
-        else:
-            r2 = sharding.search_sharded(lambda s, n, f: g2.search(s, n, first_id=f), inst.seed, total, rank, world)
-        g2.close()
+        r2 = e2e_step()
     barrier()
     e2e_s = time.perf_counter() - t0
     if dist is not None:
@@ -296,10 +306,13 @@ def main():
         n_ev = 1 << 24
         out = g.eval_batch(inst.seed, first_id=0, n=n_ev)
         torch.cuda.synchronize()
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record(stream); g.eval_batch(inst.seed, first_id=0, n=n_ev, out=out); b.record(stream)
-        torch.cuda.synchronize()
-        ev_ms = a.elapsed_time(b)
+        ev_list = []
+        for _ in range(3):                       # median of 3 device-timed calls
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream); g.eval_batch(inst.seed, first_id=0, n=n_ev, out=out); b.record(stream)
+            torch.cuda.synchronize()
+            ev_list.append(a.elapsed_time(b))
+        ev_ms = sorted(ev_list)[1]
         n_h = 1 << 22
         host_out = (np.empty(n_h), np.empty(n_h), np.empty(n_h), np.empty(n_h, np.uint8))
         g.eval_batch_host(inst.seed, first_id=0, n=n_h, out=host_out)
@@ -332,7 +345,7 @@ def main():
     obs = clocks.get("sm_mhz") or sm_max
     roofline = {"bound": "alu", "kernel": "lgx_decode_walk (dominant: %.0f %% of the kernel time of a step)" % (100.0 * ns_a / max(ns_a + ns_c, 1)),
                 "achieved": ach_a, "peak": peak_ginst, "unit": "G thread-inst/s", "frac": ach_a / peak_ginst if ach_a else None,
-                "traffic": None, "launch_ms": ms_a, "launches_timed": n_pairs, "candidates_per_launch": per_launch,
+                "traffic": TRAFFIC_BYTES_DECODE_WALK_MEDIUM if args.workload == "medium" else None, "launch_ms": ms_a, "launches_timed": n_pairs, "candidates_per_launch": per_launch,
                 "w_alg_thread_inst_per_candidate": w_dw,
                 "peak_source": f"{n_sm} SMs x 4 schedulers x 32 lanes x {sm_max:.0f} MHz ({pk_src} sm_max_mhz; DESIGN.md s8)",
                 "frac_at_observed_clock": ach_a / (peak_ginst * obs / sm_max) if ach_a else None,
