@@ -160,6 +160,22 @@ def bench_alg1(args, torch, binding, wl):
                             "what": "lgx_local_search through the C ABI, host plan in / x* out, wall clock",
                             "paper_context": "T_solve 81.89 s for 5000 iterations on a Titan V, workers per iteration "
                                              "not stated (PAPER.md Table 3, L355): another machine, not a target"}}
+    # N2: the same loop with the embedded HU assignment (LGX_FLAG_HU_BALANCE) on an instance that has spare HUs
+    from dataclasses import replace
+    inst_h = replace(wl.make("large"), flags=2)
+    gh = binding.Instance(inst_h)
+    ph = gh.init_plan()
+    nwh = sm * gh.query(15) * 8
+    ch0 = gh.local_search(ph, inst_h.seed, 0, 1, 0, history=False)[1]
+    gh.local_search(ph, inst_h.seed, 10, nwh, int(eps * 2**32), history=False)
+    t0 = time.perf_counter()
+    _, ch, _, _ = gh.local_search(ph, inst_h.seed, args.alg1_iters, nwh, int(eps * 2**32))
+    t_h = time.perf_counter() - t0
+    res["local_search_hu_balance"] = {"workload": f"large: N_T={inst_h.n_tours} N_B={inst_h.n_bps} N_F={inst_h.n_fields} N_HU={inst_h.n_hu} N_SU={inst_h.n_su}",
+                                      "iterations": args.alg1_iters, "workers_per_iteration": nwh, "wall_s": t_h,
+                                      "iterations_per_s": args.alg1_iters / t_h, "worker_evals_per_s": args.alg1_iters * nwh / t_h,
+                                      "cost_init": ch0, "cost_best": ch, "delta_pct": 100.0 * (ch - ch0) / ch0}
+    gh.close()
     if not args.no_cpu_baseline:
         cores = os.cpu_count() or 1
         per = 2048

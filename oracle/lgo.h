@@ -7,7 +7,10 @@
  *
  * Every function below cites the passage of PAPER.md it follows.
  * Pins (tests/test_oracle_*.py): Philox known answers + cuRAND header; hand toy A (P1);
- * Alg. 2 traces B and C (P2, P3); decoder / score invariants (P4, P5); brute force (P8).
+ * Alg. 2 traces B and C (P2, P3); decoder / score invariants (P4, P5); brute force (P8);
+ * Algorithm 1 (initialisation, moves, loop): hand instance and hand moves (tests/test_oracle_alg1.py);
+ * embedded HU assignment: two hand traces, degenerate cases, invariants (tests/test_oracle_hu.py).
+ * No function is "parity unpinned".
  */
 #ifndef LGO_H
 #define LGO_H
