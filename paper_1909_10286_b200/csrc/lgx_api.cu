@@ -377,6 +377,7 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
     M.off_trng = o;  o = align16(o + 8u * (uint32_t)nt);
     M.off_tst = o;   o = align16(o + 56u * (uint32_t)nt);
     M.off_thq = o;   o = align16(o + 4u * (uint32_t)nt);
+    M.off_sv = o;    o = align16(o + 16u * (uint32_t)nt * (uint32_t)nsu);
     M.off_misc = o;  o = align16(o + 64u);
     M.off_sort = o;  o = align16(o + 4u * (kSortKeys + 2u));
     M.off_order = o; o = align16(o + 2u * kSuper * 1024u);

@@ -62,6 +62,7 @@ struct MvHdr {
   uint32_t off_trng;    // u32x2 [n_t]    the tour's positions [begin, end) in plan order
   uint32_t off_tst;     // f64 [7][n_t]   the incumbent's L_tour(g), E(g), T(g), T_wait(g), shuttle sum(g), route sum before the leg back to HQ, L_tour(g)/v_HU
   uint32_t off_thq;     // u32 [n_t]      H_q(g)
+  uint32_t off_sv;      // f64 [n_t][2][n_su]  the tour's shuttle sum with one SU of capacity class r removed (0) / added (1)
   uint32_t off_misc;    // u32 [16]       [0] BPs that miss their demand (eq. (2)); [4..9] the move being applied
   uint32_t off_sort;    // u32 [kSortKeys + 2]  counting sort of the workers by the tours they touch; the warps' draw counter
   uint32_t off_order;   // u16 [kSuper * 1024]  sorted workers: round << 10 | thread
@@ -281,6 +282,25 @@ __device__ void mv_encode(const MvParams &P, uint8_t *sm, const uint8_t *plan, u
     uint32_t bad = 0;
     for (uint32_t b = 0; b < n_b; ++b) bad += (bsh[b].x < dq[b]) ? 1u : 0u;
     misc[0] = bad;
+  }
+  // Shuttle sums of every tour under the SU sets one Algorithm-2 move away (one unit of capacity class r removed or
+  // added): a worker whose Algorithm 2 changed an untouched tour that way looks the sum up instead of walking it.
+  // One thread per (tour, direction, class); a class is named by the first rank holding its capacity.
+  {
+    const uint32_t n_su = H.n_su;
+    double *sv = MV_TAB(double, M.off_sv);
+    for (uint32_t task = tid; task < n_t * 2u * n_su; task += T) {
+      const uint32_t r0 = task % n_su, dir = (task / n_su) & 1u, g = task / (2u * n_su);
+      if (r0 > 0u && cs[r0] == cs[r0 - 1u]) continue;
+      const uint2 sn = tsn[g];
+      if (dir == 0u && (sn.y < 2u || sn.x <= cs[r0])) continue;
+      const uint32_t n2 = dir ? sn.y + 1u : sn.y - 1u, C2 = dir ? sn.x + cs[r0] : sn.x - cs[r0];
+      const uint32_t magic = 0xFFFFFFFFu / C2;
+      const uint2 r = trng[g];
+      double shut = 0.0;
+      for (uint32_t p = r.x; p < r.y; ++p) shut = __dadd_rn(shut, __dmul_rn((double)shuttle_count(pos4[p].y, n2, C2, magic), leg2[p].y));
+      sv[task] = shut;
+    }
   }
   __syncthreads();
 }
@@ -645,8 +665,19 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
   for (uint32_t g = 0; g < n_t; ++g) {
     const uint2 sn = tsn[g];
     const bool same = (s.w(M.m32_s + g) == sn.x) && ((uint32_t)mask_count(mask_load<MASKW>(s, M.m64_mask + MASKW * g)) == sn.y);
-    if (g == ga || g == gb || !same) need |= 1ull << g;
-    else s.d(M.m64_w + g) = tst[4u * n_t + g];
+    if (g == ga || g == gb) { need |= 1ull << g; continue; }
+    if (same) { s.d(M.m64_w + g) = tst[4u * n_t + g]; continue; }
+    // an untouched tour one SU away from the incumbent's set: tabulated (mv_encode)
+    const uint32_t C2 = s.w(M.m32_s + g), n2 = (uint32_t)mask_count(mask_load<MASKW>(s, M.m64_mask + MASKW * g));
+    uint32_t dir = 2u, delta = 0u;
+    if (n2 == sn.y + 1u && C2 > sn.x) { dir = 1u; delta = C2 - sn.x; }
+    else if (n2 + 1u == sn.y && C2 < sn.x) { dir = 0u; delta = sn.x - C2; }
+    if (dir < 2u) {
+      uint32_t lo2 = 0, hi2 = n_su;                                            // first rank with capacity >= delta
+      while (lo2 < hi2) { const uint32_t mid = (lo2 + hi2) >> 1; if (cs[mid] < delta) lo2 = mid + 1u; else hi2 = mid; }
+      if (lo2 < n_su && cs[lo2] == delta) { s.d(M.m64_w + g) = MV_TAB(const double, M.off_sv)[(g * 2u + dir) * n_su + lo2]; continue; }
+    }
+    need |= 1ull << g;
   }
   while (need) {
     const uint32_t g = (uint32_t)__ffsll((long long)need) - 1u;
