@@ -380,7 +380,7 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
     M.off_sv = o;    o = align16(o + 16u * (uint32_t)nt * (uint32_t)nsu);
     M.off_misc = o;  o = align16(o + 64u);
     M.off_sort = o;  o = align16(o + 4u * (kSortKeys + 2u));
-    M.off_order = o; o = align16(o + 2u * kSuper * 1024u);
+    M.off_order = o; o = align16(o + 2u * kSuper * (uint32_t)kMvThreads);
     uint32_t q = 0;
     q += (uint32_t)nb; M.pl_bpos = q; q += (uint32_t)nb; q = (q + 1u) & ~1u;
     M.pl_fbp = q; q += 2u * (uint32_t)nf; M.pl_fpos = q; q += 2u * (uint32_t)nf; q = (q + 7u) & ~7u;

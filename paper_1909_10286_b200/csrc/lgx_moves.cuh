@@ -36,7 +36,7 @@ namespace cg = cooperative_groups;
 
 constexpr int      kMvThreads = 512;            // __launch_bounds__ of the move kernels
 constexpr uint32_t kNone      = 0xFFFFFFFFu;
-constexpr uint32_t kSortKeys  = 256;            // (source tour, target tour) pairs up to 16 tours, else the lower tour
+constexpr uint32_t kSortKeys  = 512;            // (tour pair, position bucket) keys of the worker sort
 
 // Shared-memory layout of the move kernels (byte offsets from the start of dynamic shared memory):
 //   vertex coordinates | demand quanta | tail of image C (from offc_cs) | incumbent tables | plan store | per-thread state rows
@@ -65,7 +65,7 @@ struct MvHdr {
   uint32_t off_sv;      // f64 [n_t][2][n_su]  the tour's shuttle sum with one SU of capacity class r removed (0) / added (1)
   uint32_t off_misc;    // u32 [16]       [0] BPs that miss their demand (eq. (2)); [4..9] the move being applied
   uint32_t off_sort;    // u32 [kSortKeys + 2]  counting sort of the workers by the tours they touch; the warps' draw counter
-  uint32_t off_order;   // u16 [kSuper * 1024]  sorted workers: round << 10 | thread
+  uint32_t off_order;   // u16 [kSuper * kMvThreads]  sorted workers: round << 10 | thread
   uint32_t off_plans;   // 3 plans (x*, x_old, scratch); the batch kernel uses the first
   uint32_t plan_bytes;  // one plan: bp_tour u8[n_b] | bp_pos u8[n_b] | field_bp u16[n_f] | field_pos u16[n_f] | SU masks u64[n_t*MW] | HU masks u64[n_t]
   uint32_t pl_bpos, pl_fbp, pl_fpos, pl_mask, pl_hmask;
@@ -765,7 +765,14 @@ __device__ __forceinline__ void mv_for_workers(const MvParams &P, uint8_t *sm, u
                                                uint32_t tid, uint32_t T, F &&eval)
 {
   const uint32_t n_t = P.H.n_t;
-  const uint32_t nk = (n_t <= 16u) ? n_t * n_t : n_t;
+  // key = (unordered pair of touched tours, bucket of the first changed position inside the lower tour): lanes of a
+  // warp then share the tours AND roughly the point from which their running sums must be re-added
+  const uint32_t n_pairs = n_t * (n_t + 1u) / 2u;
+  uint32_t nbk = 1u;
+  while (nbk < 16u && n_pairs * nbk * 2u <= kSortKeys) nbk *= 2u;
+  const bool by_pair = n_pairs <= kSortKeys;
+  const uint32_t nk = by_pair ? n_pairs * nbk : n_t;
+  const uint2 *trng = MV_TAB(const uint2, P.M.off_trng);
   uint32_t *hist = MV_TAB(uint32_t, P.M.off_sort);       // [nk + 2]: offsets per key, total, the warps' draw counter
   uint16_t *order = MV_TAB(uint16_t, P.M.off_order);
   const uint64_t stride = (uint64_t)gridDim.x * T;
@@ -784,7 +791,13 @@ __device__ __forceinline__ void mv_for_workers(const MvParams &P, uint8_t *sm, u
         philox_block(P, (uint32_t)id, (uint32_t)(id >> 32), 5u, 0u, w);
         const Move mv = mv_derive(P, sm, w[0], w[1], w[2], nullptr);
         const uint32_t ga = min(mv.g1, mv.g2), gb = max(mv.g1, mv.g2);
-        key[r] = (n_t <= 16u) ? ga * n_t + gb : ga;
+        if (by_pair) {
+          const uint2 rg = trng[ga];
+          const uint32_t pos = (mv.g1 == mv.g2) ? min(mv.a, mv.c) : ((mv.g1 == ga) ? mv.a : mv.c);
+          const uint32_t rel = pos > rg.x ? pos - rg.x : 0u;
+          const uint32_t bk = min(nbk - 1u, rel * nbk / (rg.y - rg.x + 1u));
+          key[r] = (ga * (2u * n_t - ga + 1u) / 2u + (gb - ga)) * nbk + bk;
+        } else key[r] = ga;
         rank[r] = atomicAdd(&hist[key[r]], 1u);
       }
     }
