@@ -207,3 +207,29 @@ def test_embedded_hu_assignment_matches_oracle(name, n, n_iters, n_workers):
     r = o.score(p0, hu_balance=True)
     assert (got_c == r["cost"] or (np.isinf(got_c) and not r["feasible"])) and np.array_equal(got_p["hu_tour"], r["hu_tour_final"])
     g.close()
+
+
+def test_local_search_at_bench_scale_is_self_consistent(ctxs):
+    """Beyond the oracle's reach (bench.py's launch configuration: 8 grid rounds of workers per iteration on the
+    paper's problem shape): x* re-scores in the oracle to exactly C* with no further Algorithm-2 move, C* is the
+    best winner of the history, every winner is one of its iteration's workers, and the run is reproducible."""
+    inst, o, g = ctxs("paper_scale")
+    p0 = o.init_plan()
+    n_workers = g.query(6) * g.query(15) * 8
+    n_iters = 30
+    best, c, hc, hi = g.local_search(p0, inst.seed, n_iters, n_workers, int(0.4 * 2**32))
+    r = o.score(best)
+    assert r["feasible"] and r["cost"] == c and r["moves"] == 0
+    c0 = o.score(p0)["cost"]
+    assert c == min(c0, hc.min()) and c < c0
+    assert np.all(hi // n_workers == np.arange(n_iters))
+    # the first iteration's winner, replayed by the oracle from x_0 (one worker)
+    p0s = dict(p0); p0s["su_tour"] = o.score(p0)["su_tour_final"]
+    w = o.move_eval_batch(p0s, inst.seed, int(hi[0]), 1)
+    assert w[0][0] == hc[0]
+    # sampled workers of iteration 0 are never better than its winner
+    ids = np.random.default_rng(1).integers(0, n_workers, 200)
+    for i in ids[:50]:
+        assert not (o.move_eval_batch(p0s, inst.seed, int(i), 1)[0][0] < hc[0])
+    again = g.local_search(p0, inst.seed, n_iters, n_workers, int(0.4 * 2**32))
+    assert again[1] == c and np.array_equal(again[3], hi) and np.array_equal(again[2], hc)
