@@ -58,3 +58,51 @@ def search_sharded(search_fn, seed: int, budget: int, rank: int, world: int, fir
         v, b, i = (int(x) for x in t.cpu())
         pairs.append((struct.unpack("<d", struct.pack("<Q", b % (1 << 64)))[0], i % (1 << 64)) if v else None)
     return combine(pairs)
+
+
+# ---- Algorithm 1 over several GPUs: the paper runs the loop for every eps of a uniform grid and returns the best
+# ("uniformly gridded for eps in {0, 0.25, ..., 1} ... before the lowest cost solution and
+# corresponding eps* is returned").  The runs are independent: grid point k goes to rank k mod world; ONE exchange of
+# (cost bits, grid index) follows, then the winning rank broadcasts x* (a few KB).  Ties: lowest grid index.
+
+def eps_grid_shares(n_eps: int, world: int, rank: int):
+    """Grid indices this rank runs."""
+    if n_eps < 1 or world < 1 or not (0 <= rank < world):
+        raise ValueError("bad shard arguments")
+    return list(range(rank, n_eps, world))
+
+
+def local_search_eps_grid(search_fn, plan, seed: int, n_iters: int, n_workers: int, eps_grid, rank: int, world: int):
+    """search_fn(plan, seed, n_iters, n_workers, eps_thresh) -> (x*, C*, ...) is the per-GPU call
+    (binding.Instance.local_search; the oracle's in the CPU test).  Returns (x*, C*, eps*) on every rank."""
+    import numpy as np
+    mine = None
+    for k in eps_grid_shares(len(eps_grid), world, rank):
+        thresh = min(int(eps_grid[k] * 2**32), 0xFFFFFFFF)
+        res = search_fn(plan, seed, n_iters, n_workers, thresh)
+        key = (cost_bits(res[1]), k)
+        if mine is None or key < mine[0]:
+            mine = (key, res[0])
+    if world == 1:
+        return mine[1], struct.unpack("<d", struct.pack("<Q", mine[0][0]))[0], eps_grid[mine[0][1]]
+    import torch
+    import torch.distributed as dist
+    dev = torch.device("cuda", torch.cuda.current_device()) if dist.get_backend() == "nccl" else torch.device("cpu")
+    s64 = lambda v: v - (1 << 64) if v >= (1 << 63) else v
+    t = torch.tensor([1 if mine else 0, s64(mine[0][0]) if mine else 0, mine[0][1] if mine else 0], dtype=torch.int64, device=dev)
+    allr = [torch.empty_like(t) for _ in range(world)]
+    dist.all_gather(allr, t)
+    best = None
+    for r, a in enumerate(allr):
+        v, b, k = (int(x) for x in a.cpu())
+        if v and (best is None or (b % (1 << 64), k) < best[0]):
+            best = ((b % (1 << 64), k), r)
+    (bits, k), owner = best
+    keys = sorted(plan.keys())
+    out = {}
+    for name in keys:                             # x* from its owner: one small broadcast per plan array
+        ref = np.asarray(plan[name])
+        buf = torch.from_numpy(np.ascontiguousarray(mine[1][name] if rank == owner else np.zeros_like(ref)).astype(np.int64)).to(dev)
+        dist.broadcast(buf, src=owner)
+        out[name] = buf.cpu().numpy().astype(ref.dtype)
+    return out, struct.unpack("<d", struct.pack("<Q", bits))[0], eps_grid[k]

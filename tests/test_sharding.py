@@ -53,3 +53,44 @@ def test_two_rank_search_equals_single_rank():
     want = o.search(0, budget); want1 = o.search(0, 1, first_id=5)
     for _, res, res1 in got:
         assert res == want and res1 == want1     # budget 1: rank 1 has no ids and passes None
+
+
+def _ls_worker(rank, world, port, q):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    from oracle import lgo
+    inst = wl.make("small"); o = lgo.Oracle(inst)
+    p0 = o.init_plan()
+    fn = lambda plan, seed, n_iters, n_workers, thresh: o.local_search(plan, seed, n_iters, n_workers, thresh)
+    x, c, eps = sharding.local_search_eps_grid(fn, p0, 3, 25, 64, [0.0, 0.25, 0.5, 0.75, 1.0], rank, world)
+    q.put((rank, {k: np.asarray(v).tolist() for k, v in x.items()}, c, eps))
+    dist.barrier(); dist.destroy_process_group()
+
+
+def test_eps_grid_shares_cover_the_grid():
+    for n in (1, 5, 8):
+        for world in (1, 2, 3, 8):
+            got = sorted(k for r in range(world) for k in sharding.eps_grid_shares(n, world, r))
+            assert got == list(range(n))
+
+
+def test_two_rank_eps_grid_equals_single_rank():
+    """the loop is run for eps in {0, 0.25, ..., 1} and the best is returned; ranks split the grid."""
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    ps = [ctx.Process(target=_ls_worker, args=(r, 2, port, q)) for r in range(2)]
+    [p.start() for p in ps]
+    got = [q.get(timeout=180) for _ in ps]
+    [p.join(60) for p in ps]
+    from oracle import lgo
+    inst = wl.make("small"); o = lgo.Oracle(inst)
+    p0 = o.init_plan()
+    fn = lambda plan, seed, n_iters, n_workers, thresh: o.local_search(plan, seed, n_iters, n_workers, thresh)
+    wx, wc, weps = sharding.local_search_eps_grid(fn, p0, 3, 25, 64, [0.0, 0.25, 0.5, 0.75, 1.0], 0, 1)
+    runs = [o.local_search(p0, 3, 25, 64, min(int(e * 2**32), 0xFFFFFFFF))[1] for e in (0.0, 0.25, 0.5, 0.75, 1.0)]
+    assert wc == min(runs)
+    for _, x, c, eps in got:
+        assert c == wc and eps == weps
+        for k in wx:
+            assert x[k] == np.asarray(wx[k]).tolist()
