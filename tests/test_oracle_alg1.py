@@ -136,3 +136,49 @@ def test_local_search_improves_and_is_consistent(eps):
     assert cost.min() == hc[0] and int(np.argmin(cost)) == int(hi[0])
     best2, c2, hc2, hi2 = o.local_search(p0, 3, 60, 256, eps)
     assert c2 == c and np.array_equal(hc2, hc) and np.array_equal(hi2, hi)   # deterministic
+
+
+def test_local_search_reaches_the_exhaustive_optimum():
+    """Brute force on the N_B = 2, N_F = 6 sub-instance (homogeneous units): every BP placement (incl. both BPs on one
+    tour: the other tour inactive, L184), every ordered field partition, every SU split, for the start plan's HU
+    split (the loop keeps the HU sets, R20).  From feasible sampled starts the loop must never beat that optimum and,
+    with 300 iterations of 512 workers, must reach it (to rounding: mirrored plans sum in another order)."""
+    import itertools
+    inst = wl.make("toy_brute"); o = lgo.Oracle(inst)
+
+    def brute(hu):
+        sc = np.zeros(8); fb = np.zeros(6, np.uint16); fp = np.zeros(6, np.uint16)
+        su_splits = [np.array([0] * a + [1] * (8 - a), np.uint8) for a in range(1, 8)]
+        placements = [(np.array([0, 1], np.uint8), np.zeros(2, np.uint8)), (np.array([1, 0], np.uint8), np.zeros(2, np.uint8))]
+        for g in (0, 1):
+            for first in (0, 1):
+                placements.append((np.array([g, g], np.uint8), np.array([0, 1] if first == 0 else [1, 0], np.uint8)))
+        best = np.inf
+        for bp_tour, bp_pos in placements:
+            for perm in itertools.permutations(range(6)):
+                for cut in range(7):
+                    for q, f in enumerate(perm):
+                        if q < cut: fb[f] = 0; fp[f] = q
+                        else:       fb[f] = 1; fp[f] = q - cut
+                    for su in su_splits:
+                        assert o.score_fast(bp_tour, bp_pos, fb, fp, hu, su, sc) == 0
+                        if sc[0] == 0.0:
+                            break
+                        best = min(best, sc[6])
+        return best
+
+    opts = {}
+    for pid in (0, 3):
+        p = o.decode(0, pid)
+        r = o.score(p)
+        assert r["feasible"]
+        hu = np.sort(p["hu_tour"]).astype(np.uint8)
+        key = tuple(np.bincount(hu, minlength=2))
+        if key not in opts and key[::-1] not in opts:
+            opts[key] = brute(hu)
+        opt = opts.get(key, opts.get(key[::-1]))
+        assert opt <= r["cost"]
+        for eps in (0, 0x66666666, 0xFFFFFFFF):
+            best, c, hc, hi = o.local_search(p, 3, 300, 512, eps)
+            assert c >= opt * (1 - 1e-12), "the loop beat the exhaustive optimum"
+            assert c <= opt * (1 + 1e-12), "the loop did not reach the exhaustive optimum"
