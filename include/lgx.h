@@ -127,8 +127,13 @@ int lgx_instance_set_timing(lgx_instance *inst, int enable);
  * h_field_bp/h_field_pos [N_F], h_hu_tour [N_HU], h_su_tour [N_SU].  A plan passed IN must be valid
  * (every BP on one tour at a unique position 0..len-1, every field on one BP likewise, every tour with
  * >= 1 HU and >= 1 SU; tours without BPs and BPs without fields are allowed, L184), else LGX_EINVAL.
- * LGX_ETOOBIG when the move kernels' state does not fit in shared memory (what = 15 reports 0).
- * Readings R31-R37 cover what the paper leaves open.                                 */
+ * LGX_ETOOBIG when the move kernels do not fit this instance (what = 15 reports 0): their tables (about 64 B per
+ * field + 16 B per tour and SU) and three plans live in shared memory next to >= 64 workers' rows, and the workers
+ * keep 64-bit sets of tours and of HUs (N_T <= 64, N_HU <= 64).
+ * With desc.flags & LGX_FLAG_HU_BALANCE the workers (and the scoring of x_0) first rebalance the HUs over the tours
+ * (R39): Algorithm 2's procedure on the completion times T(g), donor units by
+ * rising rate; x_{i*} and x* then carry the HU sets they were scored with (h_hu_tour is in/out).
+ * Readings R31-R39 cover what the paper leaves open.                                 */
 
 /* Steps 1-3 (L122-126, L171-173): the nearest-neighbour initialisation "a human scheduler may tacitly
  * conduct" (Case 1, L273).  HUs: floor(N_HU/N_T) per tour in index order, the residual on the last tour;
