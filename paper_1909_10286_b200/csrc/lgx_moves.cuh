@@ -476,16 +476,26 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
   if (fld) {
     const uint2 bA = bp[A], bT = bp[t];
     const uint32_t jA = bA.y & 0xFFu, jT = bT.y & 0xFFu;
-    auto mean_leg = [&](uint32_t ws, uint32_t k) -> double {
+    // the BP's k fields in the worker's order, straight from the incumbent's segment [start, ...): element `ra` of it is
+    // skipped when the moved field left this BP, and the moved field sits at offset q when it joined it
+    auto mean_leg = [&](uint32_t start, uint32_t k, bool has_rem, uint32_t ra, bool has_ins, uint32_t q) -> double {
       double sd = 0.0;
-      for (uint32_t p = ws; p < ws + k; ++p) sd = __dadd_rn(sd, (p == mv.c) ? xlb : leg2[map_idx(p)].y);
+      for (uint32_t i = 0; i < k; ++i) {
+        double leg = xlb;
+        if (!(has_ins && i == q)) {
+          const uint32_t j = i - ((has_ins && i > q) ? 1u : 0u);
+          leg = leg2[start + j + ((has_rem && j >= ra) ? 1u : 0u)].y;
+        }
+        sd = __dadd_rn(sd, leg);
+      }
       return div_small(sd, k, rcp);
     };
-    if (A == t) { kA = bA.x >> 16; qA = mean_leg(bA.x & 0xFFFFu, kA); }
+    const uint32_t sA = bA.x & 0xFFFFu, sT = bT.x & 0xFFFFu;
+    if (A == t) { kA = bA.x >> 16; qA = mean_leg(sA, kA, true, mv.a - sA, true, mv.c - sA); }
     else {
       kA = (bA.x >> 16) - 1u; kT = (bT.x >> 16) + 1u;
-      if (kA > 0u) qA = mean_leg((bA.x & 0xFFFFu) + (jT < jA ? 1u : 0u), kA);
-      qT = mean_leg((bT.x & 0xFFFFu) - (jA < jT ? 1u : 0u), kT);
+      if (kA > 0u) qA = mean_leg(sA, kA, true, mv.a - sA, false, 0u);
+      qT = mean_leg(sT, kT, false, 0u, true, mv.c - (sT - (jA < jT ? 1u : 0u)));
     }
   }
   // worker plan index -> incumbent plan index (a BP move relocates one BP in the plan order)
@@ -525,16 +535,21 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
       uint32_t P1 = Q1, J1 = K1, P2 = Q2, J2 = K2, P3 = Q3, J3 = K3;
       double Y1 = X1, Y2 = X2, Y3 = X3;
       while (P1 < p0) { P1 = P2; J1 = J2; Y1 = Y2; P2 = P3; J2 = J3; Y2 = Y3; P3 = kNone; }
-      uint32_t idx = 0;
-      for (uint32_t p = p0; p < we; ++p) {
+      uint32_t idx = 0, p = p0;
+      while (p < we) {
+        if (p + 4u <= we && p + 4u <= P1) {                                    // four table legs, no breakpoint among them
+          const double2 *lp = leg2 + idx;
+          Lt = __dadd_rn(Lt, lp[1].x); Lt = __dadd_rn(Lt, lp[2].x); Lt = __dadd_rn(Lt, lp[3].x); Lt = __dadd_rn(Lt, lp[4].x);
+          idx += 4u; p += 4u;
+          continue;
+        }
         ++idx;
-        if (__builtin_expect(p == P1, 0)) {
+        if (p == P1) {
           double lh = 0.0;
           do { idx = J1; lh = Y1; P1 = P2; J1 = J2; Y1 = Y2; P2 = P3; J2 = J3; Y2 = Y3; P3 = kNone; } while (p == P1);
           Lt = __dadd_rn(Lt, lh);
-          continue;
-        }
-        Lt = __dadd_rn(Lt, leg2[idx].x);                                       // field to field (L69)
+        } else Lt = __dadd_rn(Lt, leg2[idx].x);                                // field to field (L69)
+        ++p;
       }
     }
     if (we > wb) Lt = __dadd_rn(Lt, edge_from_xy(xy, 1u + n_b + (pos4[map_idx(we - 1u)].x & 0xFFFFu), 0u));   // back to HQ (L21; R2)
@@ -699,20 +714,28 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
     while (P1 < p) { P1 = P2; J1 = J2; P2 = P3; J2 = J3; P3 = kNone; }
     uint32_t idx = 0;
     bool inblk = false;
-    for (; p < pe; ++p) {
+    while (p < pe) {
+      if (!recount && !inblk && p + 4u <= pe && p + 4u <= P0) {                // four tabulated counts, no breakpoint among them
+        const uint4 *ep = pos4 + idx; const double2 *lp = leg2 + idx;
+        shut = __dadd_rn(shut, __dmul_rn((double)ep[1].w, lp[1].y)); shut = __dadd_rn(shut, __dmul_rn((double)ep[2].w, lp[2].y));
+        shut = __dadd_rn(shut, __dmul_rn((double)ep[3].w, lp[3].y)); shut = __dadd_rn(shut, __dmul_rn((double)ep[4].w, lp[4].y));
+        idx += 4u; p += 4u;
+        continue;
+      }
       ++idx;
-      if (__builtin_expect(p == P0, 0)) {
+      if (p == P0) {
         do { idx = J0; P0 = P1; J0 = J1; P1 = P2; J1 = J2; P2 = P3; J2 = J3; P3 = kNone; } while (p == P0);
         inblk = (p - mv.c) < L;                  // the moved block's counts were tabulated under another tour's SU set
       }
       const uint4 en = pos4[idx];
       double leg = leg2[idx].y;
       uint32_t N = en.w;
-      if (__builtin_expect(recount || inblk, 0)) {
+      if (recount || inblk) {
         if (inblk && fld) leg = xlb;
         N = shuttle_count(en.y, n_g, C_g, magic);
       }
       shut = __dadd_rn(shut, __dmul_rn((double)N, leg));
+      ++p;
     }
     s.d(M.m64_w + g) = shut;
   }
