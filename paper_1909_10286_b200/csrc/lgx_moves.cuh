@@ -715,10 +715,15 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
     uint32_t idx = 0;
     bool inblk = false;
     while (p < pe) {
-      if (!recount && !inblk && p + 4u <= pe && p + 4u <= P0) {                // four tabulated counts, no breakpoint among them
+      if (!inblk && p + 4u <= pe && p + 4u <= P0) {                            // four positions, no breakpoint among them
         const uint4 *ep = pos4 + idx; const double2 *lp = leg2 + idx;
-        shut = __dadd_rn(shut, __dmul_rn((double)ep[1].w, lp[1].y)); shut = __dadd_rn(shut, __dmul_rn((double)ep[2].w, lp[2].y));
-        shut = __dadd_rn(shut, __dmul_rn((double)ep[3].w, lp[3].y)); shut = __dadd_rn(shut, __dmul_rn((double)ep[4].w, lp[4].y));
+        uint32_t N1 = ep[1].w, N2 = ep[2].w, N3 = ep[3].w, N4 = ep[4].w;       // tabulated under the incumbent's SU set
+        if (recount) {
+          N1 = shuttle_count(ep[1].y, n_g, C_g, magic); N2 = shuttle_count(ep[2].y, n_g, C_g, magic);
+          N3 = shuttle_count(ep[3].y, n_g, C_g, magic); N4 = shuttle_count(ep[4].y, n_g, C_g, magic);
+        }
+        shut = __dadd_rn(shut, __dmul_rn((double)N1, lp[1].y)); shut = __dadd_rn(shut, __dmul_rn((double)N2, lp[2].y));
+        shut = __dadd_rn(shut, __dmul_rn((double)N3, lp[3].y)); shut = __dadd_rn(shut, __dmul_rn((double)N4, lp[4].y));
         idx += 4u; p += 4u;
         continue;
       }
