@@ -244,3 +244,14 @@ class Instance:
                                           C.byref(c), hc.ctypes.data if history else None,
                                           hi.ctypes.data if history else None, _stream_ptr(stream)))
         return dict(zip([k for k, _ in PLAN_KEYS], a)), c.value, hc, hi
+
+    def plan_of(self, seed, cand_id, stream=None):
+        """The plan of one sampled candidate (lgx_decode_batch, one row) as a dict of host arrays: the bridge from
+        lgx_search's winner to lgx_local_search's x_0 (SU sets as sampled; Algorithm 2 runs when x_0 is scored)."""
+        import torch
+        ids = torch.tensor([cand_id - (1 << 64) if cand_id >= (1 << 63) else cand_id], dtype=torch.int64, device="cuda")
+        d = self.decode_batch(seed, ids=ids, stream=stream)
+        torch.cuda.synchronize()
+        h = {k: v[0].cpu().numpy() for k, v in d.items()}
+        return dict(bp_tour=h["bp_tour"], bp_pos=h["bp_pos"], field_bp=h["field_bp"].view(np.uint16),
+                    field_pos=h["field_pos"].view(np.uint16), hu_tour=h["hu_tour"], su_tour=h["su_tour_init"])

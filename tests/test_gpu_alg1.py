@@ -233,3 +233,18 @@ def test_local_search_at_bench_scale_is_self_consistent(ctxs):
         assert not (o.move_eval_batch(p0s, inst.seed, int(i), 1)[0][0] < hc[0])
     again = g.local_search(p0, inst.seed, n_iters, n_workers, int(0.4 * 2**32))
     assert again[1] == c and np.array_equal(again[3], hi) and np.array_equal(again[2], hc)
+
+
+def test_search_winner_seeds_the_local_search(ctxs):
+    """The two halves compose through the C ABI: lgx_search's winner, decoded by lgx_decode_batch, is a valid x_0
+    whose score is the search's best cost, and Algorithm 1 improves on it (same result as the oracle's loop)."""
+    inst, o, g = ctxs("medium")
+    c, i = g.search(inst.seed, 1 << 20)
+    p = g.plan_of(inst.seed, i)
+    want = o.decode(inst.seed, i)
+    assert_plan_equal(p, want, "plan_of")
+    assert o.score(p)["cost"] == c
+    got = g.local_search(p, 5, 20, 2000, 0x66666666)
+    ref = o.local_search(p, 5, 20, 2000, 0x66666666)
+    assert got[1] == ref[1] and np.array_equal(got[3], ref[3]) and got[1] < c
+    assert_plan_equal(got[0], ref[0], "search -> local search")
