@@ -850,7 +850,9 @@ int lgo_apply_move(const lgo_instance *I, uint32_t w0, uint32_t w1, uint32_t w2,
 }
 
 /* One worker (L163-165): x_i = move(x), then constraint check and cost as in lgo_score. */
-static void worker_eval(const lgo_instance *I, const plan_buf *X, plan_buf *Y, uint64_t seed, uint64_t id, double *sc)
+/* t_best: the best-so-far maximum completion time; with LGO_FLAG_MAKESPAN_FILTER a feasible x_i whose makespan
+ * exceeds it is discarded by C_i = inf (reading R38). */
+static void worker_eval(const lgo_instance *I, const plan_buf *X, plan_buf *Y, uint64_t seed, uint64_t id, double t_best, double *sc)
 {
   uint32_t ctr[4] = { (uint32_t)id, (uint32_t)(id >> 32), 5u, 0u }, key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) }, w[4];
   lgo_philox4x32_10(ctr, key, w);
@@ -861,6 +863,7 @@ static void worker_eval(const lgo_instance *I, const plan_buf *X, plan_buf *Y, u
   lgo_apply_move(I, w[0], w[1], w[2], Y->bp_tour, Y->bp_pos, Y->field_bp, Y->field_pos);
   lgo_score_ex(I, Y->bp_tour, Y->bp_pos, Y->field_bp, Y->field_pos, Y->hu_tour, Y->su_init, (I->flags & LGO_FLAG_HU_BALANCE) != 0, sc,
                NULL, NULL, NULL, NULL, NULL, NULL, NULL, Y->su_final, Y->hu_final);
+  if ((I->flags & LGO_FLAG_MAKESPAN_FILTER) && sc[0] != 0.0 && sc[5] > t_best) sc[6] = INFINITY;
 }
 
 int lgo_move_eval_batch(const lgo_instance *I,
@@ -875,9 +878,15 @@ int lgo_move_eval_batch(const lgo_instance *I,
   memcpy(X.bp_tour, bp_tour, (size_t)I->n_b); memcpy(X.bp_pos, bp_pos, (size_t)I->n_b);
   memcpy(X.field_bp, field_bp, sizeof(uint16_t) * (size_t)I->n_f); memcpy(X.field_pos, field_pos, sizeof(uint16_t) * (size_t)I->n_f);
   memcpy(X.hu_tour, hu_tour, (size_t)I->n_hu); memcpy(X.su_init, su_tour, (size_t)I->n_su);
+  /* best-so-far makespan = that of x itself (scored like a worker's plan) */
+  double t_best = INFINITY;
+  { double s0[8];
+    lgo_score_ex(I, X.bp_tour, X.bp_pos, X.field_bp, X.field_pos, X.hu_tour, X.su_init, (I->flags & LGO_FLAG_HU_BALANCE) != 0, s0,
+                 NULL, NULL, NULL, NULL, NULL, NULL, NULL, NULL, NULL);
+    if (s0[0] != 0.0) t_best = s0[5]; }
   for (uint64_t i = 0; i < n; i++) {
     double sc[8];
-    worker_eval(I, &X, &Y, seed, first_id + i, sc);
+    worker_eval(I, &X, &Y, seed, first_id + i, t_best, sc);
     if (cost) cost[i] = sc[6];
     if (path_km) path_km[i] = sc[4];
     if (makespan_h) makespan_h[i] = sc[5];
@@ -917,19 +926,20 @@ int lgo_local_search(const lgo_instance *I,
   memcpy(best.su_init, best.su_final, (size_t)I->n_su);
   memcpy(best.hu_tour, best.hu_final, (size_t)I->n_hu);
   double c_star = sc[6];
+  double t_star = (sc[0] != 0.0) ? sc[5] : INFINITY;       /* best-so-far maximum completion time (L205; R38) */
   PLAN_COPY(old, best);
   for (uint32_t k = 0; k < n_iters; k++) {
     /* Step 6, eq. (5): x = x* if u < eps else x_old (on the host, L231). */
     uint32_t u = lgo_draw(seed, (uint64_t)k, 6u, 0u);
     if (u < eps_thresh) PLAN_COPY(cur, best); else PLAN_COPY(cur, old);
     /* Steps 9-13: every worker moves x once and evaluates; i* = arg min C_i (lowest id on ties). */
-    uint64_t bbits = 0, bid = 0; int have = 0;
+    uint64_t bbits = 0, bid = 0; int have = 0; double t_win = INFINITY;
     for (uint32_t i = 0; i < n_workers; i++) {
       uint64_t id = (uint64_t)k * n_workers + i;
-      worker_eval(I, &cur, &Y, seed, id, sc);
+      worker_eval(I, &cur, &Y, seed, id, t_star, sc);
       uint64_t bits; memcpy(&bits, &sc[6], 8);
       if (!have || bits < bbits) {
-        bbits = bits; bid = id; have = 1; PLAN_COPY(win, Y);
+        bbits = bits; bid = id; have = 1; t_win = sc[5]; PLAN_COPY(win, Y);
         memcpy(win.su_init, Y.su_final, (size_t)I->n_su); memcpy(win.hu_tour, Y.hu_final, (size_t)I->n_hu);
       }
     }
@@ -938,7 +948,7 @@ int lgo_local_search(const lgo_instance *I,
     if (hist_id) hist_id[k] = bid;
     /* Steps 14-15 (L169): update x*, C* if improving; x_old <- x_i*. */
     if (isfinite(c_win)) {
-      if (c_win < c_star) { c_star = c_win; PLAN_COPY(best, win); }
+      if (c_win < c_star) { c_star = c_win; t_star = t_win; PLAN_COPY(best, win); }
       PLAN_COPY(old, win);
     }
   }

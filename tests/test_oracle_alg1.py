@@ -182,3 +182,34 @@ def test_local_search_reaches_the_exhaustive_optimum():
             best, c, hc, hi = o.local_search(p, 3, 300, 512, eps)
             assert c >= opt * (1 - 1e-12), "the loop beat the exhaustive optimum"
             assert c <= opt * (1 + 1e-12), "the loop did not reach the exhaustive optimum"
+
+
+def test_makespan_filter_is_the_papers_selection_rule():
+    """PAPER.md:L205 (reading R38): the workers are ranked by the distance-based cost and "all candidate solutions x_i
+    that do not decrease the best-so-far maximum completion time ... are discarded by setting their cost C_i = inf".
+    With flag bit 2 a feasible worker whose makespan exceeds that of the best-so-far solution gets C_i = inf."""
+    from dataclasses import replace
+    base = replace(wl.make("small"), w_time=0.0)                 # rank by path length alone, as the paper does
+    filt = replace(base, flags=4)
+    o0, o1 = lgo.Oracle(base), lgo.Oracle(filt)
+    p0 = o0.init_plan()
+    t0 = o0.score(p0)["makespan"]
+    c0, path0, m0, f0 = o0.move_eval_batch(p0, 7, 0, 2000)
+    c1, path1, m1, f1 = o1.move_eval_batch(p0, 7, 0, 2000)
+    assert np.array_equal(f0, f1) and np.array_equal(m0, m1) and np.array_equal(path0, path1)
+    feas = f0.astype(bool)
+    worse = feas & (m0 > t0)
+    assert worse.any() and (feas & ~worse).any()
+    assert np.all(np.isinf(c1[worse])) and np.array_equal(c1[~worse], c0[~worse])
+    assert np.array_equal(c0[feas], path0[feas])                 # w_time = 0: the cost is the path length
+    # the loop: x*'s makespan never rises; without the filter the path gets shorter but the makespan may grow
+    b1, cst1, hc1, hi1 = o1.local_search(p0, 3, 80, 256, 0x66666666)
+    b0, cst0, hc0, hi0 = o0.local_search(p0, 3, 80, 256, 0x66666666)
+    r1, r0 = o1.score(b1), o0.score(b0)
+    assert r1["makespan"] <= t0 and r1["path"] == cst1 and cst1 < o0.score(p0)["path"]
+    assert cst0 <= cst1                                           # the filter only removes candidates
+    assert r0["makespan"] > r1["makespan"]                        # on this instance the unfiltered search trades makespan for path
+    # replay: the filtered loop's winners all respect the running best-so-far makespan
+    x = dict(p0); x["su_tour"] = o1.score(p0)["su_tour_final"]
+    w = o1.move_eval_batch(x, 3, 0, 256)
+    assert w[0].min() == hc1[0] and w[2][int(np.argmin(w[0]))] <= t0
