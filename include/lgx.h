@@ -31,6 +31,8 @@ extern "C" {
 
 /* lgx_instance_desc.flags */
 #define LGX_FLAG_HU_BALANCE 2u   /* lgx_move_eval_batch / lgx_local_search embed the HU assignment of PAPER.md:L190, L203 */
+#define LGX_FLAG_MAKESPAN_FILTER 4u /* ... and discard (C_i = +inf, feasible stays 1) every worker whose makespan exceeds the
+                                       best-so-far one = that of x* (of x in lgx_move_eval_batch): PAPER.md:L205, R38 */
 
 typedef struct lgx_instance lgx_instance;   /* opaque; owns host + device copies */
 
@@ -55,7 +57,7 @@ typedef struct {
   double   su_fill_h_per_t;                  /* kappa: t_SU^load = kappa * capacity (L96 (iii))  */
   double   w_path, w_time;                   /* cost = w_path*path_km + w_time*makespan_h (R1)   */
   uint32_t extra_field_thresh;               /* decoder knob: P(extra field) = thresh / 2^32     */
-  uint32_t flags;                            /* 0 or LGX_FLAG_HU_BALANCE (other bits: LGX_EINVAL) */
+  uint32_t flags;                            /* OR of LGX_FLAG_* (other bits: LGX_EINVAL)         */
 } lgx_instance_desc;
 
 /* Instance encoder.  Quantises supply/area/demand/rate/capacity to Q=1024

@@ -112,7 +112,7 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   if (!(std::isfinite(d->v_hu_road_kmh) && d->v_hu_road_kmh > 0.0)) return LGX_EINVAL;
   if (!(std::isfinite(d->v_su_road_kmh) && d->v_su_road_kmh > 0.0)) return LGX_EINVAL;
   if (!fin_nonneg(d->su_fill_h_per_t) || !fin_nonneg(d->w_path) || !fin_nonneg(d->w_time)) return LGX_EINVAL;
-  if ((d->flags & ~(uint32_t)LGX_FLAG_HU_BALANCE) != 0u) return LGX_EINVAL;
+  if ((d->flags & ~(uint32_t)(LGX_FLAG_HU_BALANCE | LGX_FLAG_MAKESPAN_FILTER)) != 0u) return LGX_EINVAL;
   const int nf = d->n_fields, nb = d->n_bps, nhu = d->n_hu_total, nsu = d->n_su_total, nt = d->n_tours;
   for (int f = 0; f < nf; ++f)
     if (!std::isfinite(d->field_x[f]) || !std::isfinite(d->field_y[f]) || !fin_nonneg(d->field_supply_t[f]) ||
@@ -399,7 +399,7 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
     M.m32_s = r; r += (uint32_t)nt;
     if (hb) { M.m32_r = r; r += (uint32_t)nt; }
     M.m32_rows = r;
-    M.slot_words = 2u + (uint32_t)nt * MW + (uint32_t)nt;
+    M.slot_words = 3u + (uint32_t)nt * MW + (uint32_t)nt;
     const int64_t mv_state = 8ll * M.m64_rows + 4ll * M.m32_rows;
     int64_t tm = (budget - 256 - (int64_t)M.off_state) / mv_state;      // static smem of the reductions
     tm = std::min<int64_t>(tm, kMvThreads) / 32 * 32;

@@ -874,12 +874,21 @@ __global__ void __launch_bounds__(kMvThreads, 1) lgx_move_eval_k(const __grid_co
   uint8_t *plan = sm + P.M.off_plans;
   mv_load_plan<MASKW>(P, sm, plan, tid, T);
   mv_encode<MASKW>(P, sm, plan, tid, T);
+  // the paper's selection rule (L205; R38), optional: the best-so-far maximum completion time is x's own
+  __shared__ double s_tbest;
+  const bool filter = (P.H.flags & 4u) != 0u;
+  if (filter) {
+    if (tid == 0) { const EvalOut r0 = mv_eval<MASKW, HB>(P, sm, s, mv_identity()); s_tbest = r0.makespan; }   // +inf if x is infeasible
+    __syncthreads();
+  }
+  const double t_best = filter ? s_tbest : 0.0;
   mv_for_workers(P, sm, P.first_id, P.n, tid, T, [&](uint64_t i) {
     const uint64_t id = P.first_id + i;
     uint32_t w[4];
     philox_block(P, (uint32_t)id, (uint32_t)(id >> 32), 5u, 0u, w);
     const Move mv = mv_derive(P, sm, w[0], w[1], w[2], nullptr);
-    const EvalOut r = mv_eval<MASKW, HB>(P, sm, s, mv);
+    EvalOut r = mv_eval<MASKW, HB>(P, sm, s, mv);
+    if (filter && r.feasible && r.makespan > t_best) r.cost = __longlong_as_double(0x7FF0000000000000ll);
     if (P.cost)       P.cost[i] = r.cost;
     if (P.path_km)    P.path_km[i] = r.path;
     if (P.makespan_h) P.makespan_h[i] = r.makespan;
@@ -901,6 +910,8 @@ __global__ void __launch_bounds__(kMvThreads, 1) lgx_local_search_k(const __grid
   __shared__ unsigned long long s_bits[kMvThreads / 32], s_id[kMvThreads / 32];
   __shared__ unsigned long long s_win[3];      // global winner of the iteration: cost bits, id, block
   __shared__ unsigned long long s_cstar;       // cost bits of x*
+  __shared__ double s_tstar;                   // makespan of x*: the best-so-far maximum completion time (L205; R38)
+  const bool filter = (H.flags & 4u) != 0u;
   St s;
   mv_prologue<MASKW>(P, sm, s, tid, T);
   uint8_t *x_best = sm + M.off_plans, *x_old = x_best + M.plan_bytes, *x_tmp = x_old + M.plan_bytes;
@@ -915,6 +926,7 @@ __global__ void __launch_bounds__(kMvThreads, 1) lgx_local_search_k(const __grid
   if (tid == 0) {
     const EvalOut r = mv_eval<MASKW, HB>(P, sm, s, mv_identity());
     s_cstar = (unsigned long long)__double_as_longlong(r.cost);
+    s_tstar = r.makespan;                                                      // +inf if x_0 is infeasible
     if (r.feasible) {
       uint64_t *mk = reinterpret_cast<uint64_t *>(x_best + M.pl_mask);
       for (uint32_t i = 0; i < n_t * MASKW; ++i) mk[i] = s.q(M.m64_mask + i);
@@ -935,6 +947,8 @@ __global__ void __launch_bounds__(kMvThreads, 1) lgx_local_search_k(const __grid
 
     // ---- steps 7-12: every worker moves x once and scores it; running (cost, id) minimum per thread
     unsigned long long best_bits = ~0ull, best_id = ~0ull;
+    double best_mk = 0.0;
+    const double t_star = s_tstar;
     const uint64_t id0 = (uint64_t)k * P.n_workers;
     mv_for_workers(P, sm, id0, (uint64_t)P.n_workers, tid, T, [&](uint64_t i) {
       const uint64_t id = id0 + i;
@@ -942,9 +956,10 @@ __global__ void __launch_bounds__(kMvThreads, 1) lgx_local_search_k(const __grid
       philox_block(P, (uint32_t)id, (uint32_t)(id >> 32), 5u, 0u, w);
       const Move mv = mv_derive(P, sm, w[0], w[1], w[2], nullptr);
       const EvalOut r = mv_eval<MASKW, HB>(P, sm, s, mv);
-      const unsigned long long bits = (unsigned long long)__double_as_longlong(r.cost);
+      unsigned long long bits = (unsigned long long)__double_as_longlong(r.cost);
+      if (filter && r.feasible && r.makespan > t_star) bits = 0x7FF0000000000000ull;   // discarded (L205; R38)
       if (bits < best_bits || (bits == best_bits && id < best_id)) {
-        best_bits = bits; best_id = id;
+        best_bits = bits; best_id = id; best_mk = r.makespan;
         if (r.feasible) {
           for (uint32_t q = 0; q < n_t * MASKW; ++q) s.q(M.m64_bmask + q) = s.q(M.m64_mask + q);
           if (HB) for (uint32_t g = 0; g < n_t; ++g) s.q(M.m64_bhmask + g) = s.q(M.m64_hmask + g);
@@ -977,6 +992,7 @@ __global__ void __launch_bounds__(kMvThreads, 1) lgx_local_search_k(const __grid
     {
       for (uint32_t q = 0; q < n_t * MASKW; ++q) slot[2 + q] = s.q(M.m64_bmask + q);
       if (HB) for (uint32_t g = 0; g < n_t; ++g) slot[2 + n_t * MASKW + g] = s.q(M.m64_bhmask + g);
+      slot[2 + n_t * MASKW + n_t] = (unsigned long long)__double_as_longlong(best_mk);
     }
     grid.sync();
     if (tid < 32u) {
@@ -1039,7 +1055,13 @@ __global__ void __launch_bounds__(kMvThreads, 1) lgx_local_search_k(const __grid
       __syncthreads();
       const bool improves = win_bits < s_cstar;
       __syncthreads();
-      if (improves) { copy_plan(x_best, x_tmp); if (tid == 0u) s_cstar = win_bits; }
+      if (improves) {
+        copy_plan(x_best, x_tmp);
+        if (tid == 0u) {
+          s_cstar = win_bits;
+          s_tstar = __longlong_as_double((long long)__ldcg(P.slots + ((size_t)(k & 1u) * gridDim.x + (size_t)s_win[2]) * SW + 2 + n_t * MASKW + n_t));
+        }
+      }
       copy_plan(x_old, x_tmp);
       __syncthreads();
     }

@@ -248,3 +248,22 @@ def test_search_winner_seeds_the_local_search(ctxs):
     ref = o.local_search(p, 5, 20, 2000, 0x66666666)
     assert got[1] == ref[1] and np.array_equal(got[3], ref[3]) and got[1] < c
     assert_plan_equal(got[0], ref[0], "search -> local search")
+
+
+@pytest.mark.parametrize("name,flags", [("small", 4), ("medium", 4), ("large", 6), ("paper_scale", 4)])
+def test_makespan_filter_matches_oracle(name, flags):
+    """The paper's selection rule (R38): rank by path length (w_time = 0), discard workers whose
+    makespan exceeds the best-so-far one; alone and together with the embedded HU assignment."""
+    from dataclasses import replace
+    inst = replace(wl.make(name), flags=flags, w_time=0.0)
+    o, g = lgo.Oracle(inst), binding.Instance(inst)
+    p0 = o.init_plan()
+    w = check_move_eval(o, g, p0, 7, 0, 4096, f"{name}/filter")
+    assert np.isinf(w[0][w[3] == 1]).any()                       # some feasible workers are discarded
+    for eps, n_iters, n_workers in ((0x66666666, 12, 700), (0xFFFFFFFF, 6, 1500)):
+        want = o.local_search(p0, 3, n_iters, n_workers, eps)
+        got = g.local_search(p0, 3, n_iters, n_workers, eps)
+        assert np.array_equal(got[3], want[3]) and got[1] == want[1]
+        assert_costs(got[2], want[2], f"{name}/filter/hist")
+        assert_plan_equal(got[0], want[0], f"{name}/filter")
+    g.close()
