@@ -31,6 +31,8 @@ extern "C" {
 
 /* lgx_instance_desc.flags */
 #define LGX_FLAG_HU_BALANCE 2u   /* lgx_move_eval_batch / lgx_local_search embed the HU assignment of PAPER.md:L190, L203 */
+#define LGX_FLAG_FIX_FIELD_BP 8u /* a moved field is reinserted into its own BP (the assignment of fields to BPs is fixed:
+                                    PAPER.md §2.6, Cases 2-3 L273); the target draw w1 is then unused for fields */
 #define LGX_FLAG_MAKESPAN_FILTER 4u /* ... and discard (C_i = +inf, feasible stays 1) every worker whose makespan exceeds the
                                        best-so-far one = that of x* (of x in lgx_move_eval_batch): PAPER.md:L205, R38 */
 

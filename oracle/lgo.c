@@ -834,6 +834,9 @@ int lgo_apply_move(const lgo_instance *I, uint32_t w0, uint32_t w1, uint32_t w2,
       int f = (int)v, a = field_bp[f];
       list_remove(L.bp_field + (size_t)a * nf, &L.bp_len[a], f);
       int t = (int)below(w1, (uint32_t)nb);
+      /* §2.6 (L249): with the field->BP assignment fixed, a removed field "must be reinserted into the same group of
+       * fields assigned to that given BP.  This is the only change."  (flag bit 3; the draw w1 is then unused) */
+      if (I->flags & LGO_FLAG_FIX_FIELD_BP) t = a;
       int q = (int)below(w2, (uint32_t)(L.bp_len[t] + 1));
       list_insert(L.bp_field + (size_t)t * nf, &L.bp_len[t], q, f);
     } else {

@@ -27,6 +27,7 @@ extern "C" {
 
 #define LGO_Q 1024   /* quanta per unit (t, ha, ha/h); R18 */
 #define LGO_FLAG_HU_BALANCE 2u   /* desc.flags bit 1: Algorithm 1's workers embed the HU assignment (N2; R39) */
+#define LGO_FLAG_FIX_FIELD_BP 8u   /* desc.flags bit 3: a moved field stays with its BP (§2.6; Cases 2-3 L273) */
 #define LGO_FLAG_MAKESPAN_FILTER 4u /* desc.flags bit 2: workers whose makespan exceeds the best-so-far one get C_i = inf (L205; R38) */
 
 /* Same field order as the product's lgx_instance_desc (restated, not shared). */

@@ -112,7 +112,7 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   if (!(std::isfinite(d->v_hu_road_kmh) && d->v_hu_road_kmh > 0.0)) return LGX_EINVAL;
   if (!(std::isfinite(d->v_su_road_kmh) && d->v_su_road_kmh > 0.0)) return LGX_EINVAL;
   if (!fin_nonneg(d->su_fill_h_per_t) || !fin_nonneg(d->w_path) || !fin_nonneg(d->w_time)) return LGX_EINVAL;
-  if ((d->flags & ~(uint32_t)(LGX_FLAG_HU_BALANCE | LGX_FLAG_MAKESPAN_FILTER)) != 0u) return LGX_EINVAL;
+  if ((d->flags & ~(uint32_t)(LGX_FLAG_HU_BALANCE | LGX_FLAG_MAKESPAN_FILTER | LGX_FLAG_FIX_FIELD_BP)) != 0u) return LGX_EINVAL;
   const int nf = d->n_fields, nb = d->n_bps, nhu = d->n_hu_total, nsu = d->n_su_total, nt = d->n_tours;
   for (int f = 0; f < nf; ++f)
     if (!std::isfinite(d->field_x[f]) || !std::isfinite(d->field_y[f]) || !fin_nonneg(d->field_supply_t[f]) ||

@@ -329,7 +329,8 @@ __device__ __forceinline__ Move mv_derive(const MvParams &P, const uint8_t *sm, 
   if (v < n_f) {
     const uint32_t a = MV_TAB(const uint16_t, M.off_posf)[v];
     const uint32_t A = MV_TAB(const uint4, M.off_pos4)[a].x >> 16;
-    const uint32_t t = __umulhi(w1, n_b);
+    // §2.6 (L249): with the field->BP assignment fixed (flag bit 3) the field is reinserted into its own BP
+    const uint32_t t = (H.flags & 8u) ? A : __umulhi(w1, n_b);
     const uint2 bt = bp[t], bA = bp[A];
     const uint32_t len_t = bt.x >> 16, start_t = bt.x & 0xFFFFu;
     const uint32_t q = __umulhi(w2, len_t - (A == t ? 1u : 0u) + 1u);

@@ -267,3 +267,19 @@ def test_makespan_filter_matches_oracle(name, flags):
         assert_costs(got[2], want[2], f"{name}/filter/hist")
         assert_plan_equal(got[0], want[0], f"{name}/filter")
     g.close()
+
+
+@pytest.mark.parametrize("name,flags", [("small", 8), ("medium", 8 | 2), ("paper_scale", 8 | 4)])
+def test_fixed_field_bp_assignment_matches_oracle(name, flags):
+    """PAPER.md §2.6 (L249), Cases 2-3: a moved field is reinserted into its own BP."""
+    from dataclasses import replace
+    inst = replace(wl.make(name), flags=flags)
+    o, g = lgo.Oracle(inst), binding.Instance(inst)
+    p0 = o.init_plan()
+    check_move_eval(o, g, p0, 7, 0, 4096, f"{name}/fixbp")
+    want = o.local_search(p0, 3, 10, 900, 0x66666666)
+    got = g.local_search(p0, 3, 10, 900, 0x66666666)
+    assert np.array_equal(got[3], want[3]) and got[1] == want[1]
+    assert_plan_equal(got[0], want[0], f"{name}/fixbp")
+    assert np.array_equal(got[0]["field_bp"], p0["field_bp"])
+    g.close()

@@ -213,3 +213,29 @@ def test_makespan_filter_is_the_papers_selection_rule():
     x = dict(p0); x["su_tour"] = o1.score(p0)["su_tour_final"]
     w = o1.move_eval_batch(x, 3, 0, 256)
     assert w[0].min() == hc1[0] and w[2][int(np.argmin(w[0]))] <= t0
+
+
+def test_fixed_field_to_bp_assignment():
+    """PAPER.md §2.6 (L249): "any field removed from x as part of Step 8 ... must be reinserted into the same group of
+    fields assigned to that given BP.  This is the only change."  (flag bit 3; Cases 2-3 of §3.2)"""
+    from dataclasses import replace
+    inst = replace(wl.make("small"), flags=8)
+    o, of = lgo.Oracle(inst), lgo.Oracle(wl.make("small"))
+    p = o.init_plan()
+    rng = np.random.default_rng(11)
+    n_field_moves = 0
+    for _ in range(400):
+        w = [int(x) for x in rng.integers(0, 2**32, 3)]
+        q = o.apply_move(p, *w)
+        assert np.array_equal(q["field_bp"], p["field_bp"])                      # no field ever changes its BP
+        v = (w[0] * (o.n_f + o.n_b)) >> 32
+        if v < o.n_f:
+            n_field_moves += 1
+            b = int(p["field_bp"][v]); k = int((p["field_bp"] == b).sum())
+            assert int(q["field_pos"][v]) == (w[2] * k) >> 32                     # position = below(w2, len after removal + 1)
+        else:                                                                     # BP moves are untouched by the flag
+            qf = of.apply_move(p, *w)
+            assert all(np.array_equal(q[k2], qf[k2]) for k2 in q)
+    assert n_field_moves > 300
+    best, c, hc, hi = o.local_search(p, 3, 60, 256, 0x66666666)
+    assert np.array_equal(best["field_bp"], p["field_bp"]) and c < o.score(p)["cost"]
