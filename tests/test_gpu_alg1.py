@@ -283,3 +283,20 @@ def test_fixed_field_bp_assignment_matches_oracle(name, flags):
     assert_plan_equal(got[0], want[0], f"{name}/fixbp")
     assert np.array_equal(got[0]["field_bp"], p0["field_bp"])
     g.close()
+
+
+def test_results_do_not_depend_on_the_launch_shape(ctxs, monkeypatch):
+    """Which thread scores which worker is free (sorted rounds, warps drawing chunks): the winners must not depend on it."""
+    inst, o, g = ctxs("medium")
+    p0 = o.init_plan()
+    ref = g.local_search(p0, 9, 15, 20000, 0x66666666)
+    refb = g.move_eval_batch(p0, 9, 0, 50000)[0].cpu().numpy()
+    for threads in ("64", "160", "384"):
+        monkeypatch.setenv("LGX_THREADS_MV", threads)
+        g2 = binding.Instance(inst)
+        assert g2.query(15) == int(threads)
+        got = g2.local_search(p0, 9, 15, 20000, 0x66666666)
+        assert got[1] == ref[1] and np.array_equal(got[3], ref[3]) and np.array_equal(got[2], ref[2])
+        assert_plan_equal(got[0], ref[0], f"threads {threads}")
+        assert np.array_equal(g2.move_eval_batch(p0, 9, 0, 50000)[0].cpu().numpy(), refb)
+        g2.close()
