@@ -10,20 +10,19 @@
 // takes the argmin there and rebuilds x_{i*} by replaying the random stream (L163-169, L233).  Here the
 // incumbent lives in the shared memory of every SM as a FLAT SEQUENCE: the fields in plan order (tour 0's
 // first BP's fields, ...), each entry carrying its BP.  A move (one field, or one BP with all its fields,
-// L184) is a rotation of one block of that sequence, so a worker never materialises x_i: it walks positions
-// s = 0..N_F-1 and maps s to an index of the incumbent's sequence with a handful of integer operations.
-// All workers of a warp therefore read (nearly) the same shared-memory words — broadcast, conflict-free —
-// and hit the BP / tour boundaries at (nearly) the same step, unlike the independently sampled plans of
-// lgx_decode_walk.  After the block/grid reduction of (cost bits, id) every block rebuilds x_{i*} ITSELF
-// from the winning id ("identical random process control", L233, taken one step further): the only
-// inter-SM traffic per iteration is one slot of (cost, id, SU sets) per block and one grid barrier.
+// L184) is a rotation of one block of that sequence, so a worker never materialises x_i: three breakpoints
+// (worker position -> incumbent index) describe it.  After the block/grid reduction of (cost bits, id) every
+// block rebuilds x_{i*} ITSELF from the winning id ("identical random process control", L233, taken one step
+// further): the only inter-SM traffic per iteration is one slot of (cost, id, SU / HU sets, makespan) per block
+// and one grid barrier.
 //
-// Because every worker walks the SAME sequence except around its one moved block, the two distances each
-// field contributes — the HU leg from its predecessor and the shuttle leg to its BP — are computed ONCE per
-// iteration per SM while the incumbent is encoded (leg2[p]) and merely read by the workers; a worker computes
-// a distance itself (from the vertex coordinates, same formula, same bits) only at the <= 3 positions where its
-// predecessor differs and for the moved field's new BP.  The per-field work of a worker is then two
-// shared-memory loads, two FP64 additions and the integer bookkeeping, whatever N_F is.
+// Evaluation is incremental and exact (mv_eval): per iteration and SM the encoder tabulates, for every position of
+// the incumbent, its two legs, its shuttle count and the tour's running sums before it, and per tour / per BP the
+// finished sums; a worker re-adds only what its move changes — the tail of the <= 2 touched tours from the first
+// changed position, the mean leg of the two BPs of a field move, the shuttle sums of tours whose SU set its
+// Algorithm 2 changed (tabulated too when the set is one unit away) — and reads the rest: same operands in the same
+// order, hence the same bits.  The workers of up to kSuper block rounds are sorted by (touched tours, first changed
+// position) so that a warp's lanes do the same work, and the warps draw sorted chunks from a shared counter.
 //
 // FP64 arithmetic follows DESIGN.md S4-S7 operation by operation (compiled with -fmad=false), in the
 // oracle's summation order, so costs are bit-equal.
