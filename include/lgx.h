@@ -9,7 +9,12 @@
  * argmin (L167).  DESIGN.md states every reading (R1..R30) the paper leaves open.
  *
  * Conventions
- *  - extern "C", no exceptions, no global state.  Return 0 (LGX_OK) or a negative code.
+ *  - extern "C", no exceptions.  Return 0 (LGX_OK) or a negative code.  No process-wide state: the library
+ *    reads no environment variables; every tuning knob is a flag of the descriptor or an lgx_instance_set_option
+ *    key; the only per-function CUDA state (the opt-in shared-memory size of a kernel) is set once, to the device
+ *    maximum, when an instance that uses the kernel is created.
+ *  - Every compute call must run with the CUDA device the instance was created on as the current device
+ *    (its images live there): otherwise LGX_EINVAL.
  *  - "d_" pointers are DEVICE pointers (caller-allocated, e.g. torch tensors' data_ptr());
  *    "h_" pointers and everything inside lgx_instance_desc are HOST pointers.
  *  - cuda_stream is a cudaStream_t passed as void* (NULL = default stream).
@@ -25,9 +30,17 @@ extern "C" {
 
 #define LGX_OK        0
 #define LGX_EINVAL   (-1)   /* bad argument / instance violates the documented ranges        */
-#define LGX_ETOOBIG  (-2)   /* instance image or per-candidate state does not fit on an SM   */
+#define LGX_ETOOBIG  (-2)   /* instance image or per-candidate state does not fit on an SM,
+                               or a kernel limit below is exceeded                           */
 #define LGX_ECUDA    (-3)   /* CUDA runtime error; text via lgx_strerror(LGX_ECUDA)          */
 #define LGX_ENOMEM   (-4)
+
+/* Kernel limits of this build (beyond them lgx_instance_create returns LGX_ETOOBIG; the move kernels'
+ * limits make lgx_move_eval_batch / lgx_local_search return LGX_ETOOBIG, the instance itself is still created). */
+#define LGX_MAX_BPS         127   /* N_B: 7-bit BP ids in the plan-order entries                                */
+#define LGX_MAX_SUS         128   /* N_SU: SU sets are 2 x 64-bit masks over capacity ranks                     */
+#define LGX_MAX_MOVE_TOURS   64   /* N_T of the Algorithm-1 entry points: 64-bit sets of tours                  */
+#define LGX_MAX_MOVE_HUS     64   /* N_HU of the Algorithm-1 entry points: 64-bit sets of HUs                   */
 
 /* lgx_instance_desc.flags */
 #define LGX_FLAG_HU_BALANCE 2u   /* lgx_move_eval_batch / lgx_local_search embed the HU assignment of PAPER.md:L190, L203 */
@@ -35,6 +48,22 @@ extern "C" {
                                     PAPER.md §2.6, Cases 2-3 L273); the target draw w1 is then unused for fields */
 #define LGX_FLAG_MAKESPAN_FILTER 4u /* ... and discard (C_i = +inf, feasible stays 1) every worker whose makespan exceeds the
                                        best-so-far one = that of x* (of x in lgx_move_eval_batch): PAPER.md:L205, R38 */
+
+/* Tuning flags: how the walk/finish kernel gets its distances.  Default: packed tables in shared memory while
+ * they fit next to >= 256 candidates per SM, else the field x BP table + coordinates while that table is <= 32 KB,
+ * else coordinates only.  D(u,v) is the same bit pattern in every mode (one rounding per operation, S0),
+ * so results do not depend on these flags.  Both set => LGX_EINVAL.                                             */
+#define LGX_FLAG_DIST_COORDS 16u /* vertex coordinates only, sqrt on the fly                                    */
+#define LGX_FLAG_DIST_MIXED  32u /* field x BP table + coordinates for the field-to-field legs (if it fits)     */
+
+/* lgx_instance_set_option keys: launch configuration only, never results.  Not to be called while a compute
+ * call on the same instance is in flight.  Values outside the stated range => LGX_EINVAL.                      */
+#define LGX_OPT_THREADS_A   1    /* threads per block of the decode/cut kernel: multiple of 32, 32 .. what fits */
+#define LGX_OPT_THREADS_B   2    /* threads per block of the walk/finish kernel: multiple of 32, 32 .. what fits */
+#define LGX_OPT_THREADS_MV  3    /* threads per block of the move kernels: multiple of 32, 64 .. what fits      */
+#define LGX_OPT_CHUNK_LOG2  4    /* log2 of the candidates per kernel pair, 10 .. 26 (queue memory = chunk * record bytes) */
+#define LGX_OPT_SQ_SHIFT    5    /* log2 of the replication of the s_q table in the decode/cut kernel's shared memory, 0 .. 5;
+                                    synchronises the device and re-uploads the image                            */
 
 typedef struct lgx_instance lgx_instance;   /* opaque; owns host + device copies */
 
@@ -46,12 +75,12 @@ typedef struct {
   const double *field_x, *field_y;           /* km, field centroids (Fig. 1, L21)                */
   const double *field_supply_t;              /* s_f, expected supply (t), eq. (2)/(3) L79-85     */
   const double *field_area_ha;               /* h_f (ha), L83                                    */
-  int32_t  n_bps;                            /* N_B, 1..255                                      */
+  int32_t  n_bps;                            /* N_B, 1..LGX_MAX_BPS (128..255: LGX_ETOOBIG)      */
   const double *bp_x, *bp_y;                 /* km                                               */
   const double *bp_demand_t;                 /* d_b^min (t), eq. (2)                         */
-  int32_t  n_hu_total;                       /* N_HU^total, eq. (1)                          */
+  int32_t  n_hu_total;                       /* N_HU^total, eq. (1); 1..255                  */
   const double *hu_rate_ha_per_h;            /* v_HU^area per unit (ha/h), L96 (ii), classes L75 */
-  int32_t  n_su_total;                       /* N_SU^total, eq. (1)                          */
+  int32_t  n_su_total;                       /* N_SU^total, eq. (1); 1..LGX_MAX_SUS (129..255: LGX_ETOOBIG) */
   const double *su_capacity_t;               /* l_SU^load per unit (t), L87                      */
   int32_t  n_tours;                          /* N_T <= min(N_B, N_HU^total, N_SU^total) (L69)    */
   double   v_hu_road_kmh, v_su_road_kmh;     /* v_HU^edge, v_SU^edge (Table 1: 40, 40)           */
@@ -63,12 +92,13 @@ typedef struct {
 } lgx_instance_desc;
 
 /* Instance encoder.  Quantises supply/area/demand/rate/capacity to Q=1024
- * quanta, builds the shared-memory image (distance tables or coordinates, unit tables) and
- * uploads it.  Errors: LGX_EINVAL (null pointer, n_tours out of range, non-finite or
- * negative input, zero rate/capacity/velocity, counts beyond the ranges above),
+ * quanta, builds the two shared-memory images (supply/demand quanta for the integer decode/cut kernel;
+ * distance tables or coordinates and the unit tables for the walk/finish kernel) and uploads them.
+ * Errors: LGX_EINVAL (null pointer, n_tours out of range, non-finite or negative input, zero
+ * rate/capacity/velocity, counts above 65535 fields / 255 BPs, tours, HUs, SUs, unknown flag bits),
  * LGX_ETOOBIG (integer ranges: max s_q*N_SU + sum c_q, sum s_q, sum h_q, sum r_q, d_q must
- * stay below 2^32; or the per-candidate state does not fit in 227 KB of shared memory),
- * LGX_ECUDA, LGX_ENOMEM.                                                                    */
+ * stay below 2^32; N_B > LGX_MAX_BPS or N_SU > LGX_MAX_SUS; or the per-candidate state does not fit in
+ * 227 KB of shared memory), LGX_ECUDA, LGX_ENOMEM.                                          */
 int lgx_instance_create (const lgx_instance_desc *desc, lgx_instance **out);
 int lgx_instance_destroy(lgx_instance *inst);
 
@@ -98,7 +128,8 @@ int lgx_search_range(const lgx_instance *inst, uint64_t seed, uint64_t first_id,
 int lgx_search(const lgx_instance *inst, uint64_t seed, uint64_t budget,
                double *h_best_cost, uint64_t *h_best_id, void *cuda_stream);
 
-/* Diagnostic export of decoded plans (needed for the "plans bit-exact" parity clause).
+/* Diagnostic export of decoded plans (needed for the "plans bit-exact" parity clause; SURVEY §8(b) lists it
+ * without first_id — added so that implicit id ranges work as in lgx_eval_batch).
  * Layouts: d_bp_tour/d_bp_pos [n][N_B] (tour of BP b, its position on that tour);
  * d_field_bp/d_field_pos [n][N_F] (BP of field f, its position in that BP's list);
  * d_hu_tour [n][N_HU]; d_su_tour_init / d_su_tour_final [n][N_SU] (before / after Alg. 2;
@@ -111,18 +142,23 @@ int lgx_decode_batch(const lgx_instance *inst, uint64_t seed,
                      void *cuda_stream);
 
 /* Introspection for bench.py / tests: what = 0 image bytes (both images), 1 threads per block
- * of the decode/walk kernel, 2 blocks in the persistent grid, 3 its dynamic shared memory
+ * of the decode/cut kernel, 2 blocks in the persistent grid, 3 its dynamic shared memory
  * bytes per block, 4 distance mode (0 = packed tables in smem, 1 = coordinates, 2 = field x BP table + coordinates),
- * 5 per-candidate state bytes of the decode/walk kernel, 6 SM count, 7 kernel launches issued
- * so far through this instance, 8 / 9 threads per block / shared memory bytes of the finish
+ * 5 per-candidate state bytes of the decode/cut kernel, 6 SM count, 7 kernel launches issued
+ * so far through this instance, 8 / 9 threads per block / shared memory bytes of the walk/finish
  * kernel, 10 candidates per kernel pair (chunk), 11 bytes per queue record, 15 / 16 threads per
- * block / shared memory bytes of the move kernels (Algorithm 1 entry points below).         */
+ * block / shared memory bytes of the move kernels (Algorithm 1 entry points below; 0 threads: they do not fit),
+ * 17 log2 of the s_q replication, 18 threads per block of the decode/cut kernel in lgx_decode_batch,
+ * 19 per-candidate state bytes of the walk/finish kernel, 20 the instance's CUDA device.    */
 int lgx_instance_query(const lgx_instance *inst, int what, int64_t *out);
+
+/* Launch-configuration knobs (LGX_OPT_* above).  Results never depend on them.              */
+int lgx_instance_set_option(lgx_instance *inst, int key, int64_t value);
 
 /* Per-kernel timing for bench.py's roofline: when enabled, every lgx_search(_range) call
  * brackets each kernel launch with CUDA events on the caller's stream and accumulates the
  * device time; lgx_instance_query what = 12 / 13 return the nanoseconds spent in the
- * decode/walk / finish kernels, 14 the number of kernel pairs timed.  Enabling or disabling
+ * decode/cut / walk/finish kernels, 14 the number of kernel pairs timed.  Enabling or disabling
  * resets the counters.                                                                     */
 int lgx_instance_set_timing(lgx_instance *inst, int enable);
 

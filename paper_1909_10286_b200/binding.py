@@ -15,6 +15,11 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "liblgx.so")
 
 LGX_OK, LGX_EINVAL, LGX_ETOOBIG, LGX_ECUDA, LGX_ENOMEM = 0, -1, -2, -3, -4
+# include/lgx.h: descriptor flags and lgx_instance_set_option keys
+LGX_FLAG_HU_BALANCE, LGX_FLAG_MAKESPAN_FILTER, LGX_FLAG_FIX_FIELD_BP = 2, 4, 8
+LGX_FLAG_DIST_COORDS, LGX_FLAG_DIST_MIXED = 16, 32
+LGX_OPT_THREADS_A, LGX_OPT_THREADS_B, LGX_OPT_THREADS_MV, LGX_OPT_CHUNK_LOG2, LGX_OPT_SQ_SHIFT = 1, 2, 3, 4, 5
+LGX_MAX_BPS, LGX_MAX_SUS, LGX_MAX_MOVE_TOURS, LGX_MAX_MOVE_HUS = 127, 128, 64, 64
 
 _dp = C.POINTER(C.c_double)
 
@@ -35,6 +40,7 @@ class lgx_instance_desc(C.Structure):
 
 EXPORTS = ("lgx_instance_create", "lgx_instance_destroy", "lgx_eval_batch", "lgx_eval_batch_host",
            "lgx_search_range", "lgx_search", "lgx_decode_batch", "lgx_instance_query", "lgx_instance_set_timing",
+           "lgx_instance_set_option",
            "lgx_init_plan", "lgx_move_eval_batch", "lgx_local_search", "lgx_strerror")
 
 _lib = None
@@ -60,6 +66,7 @@ def load(rebuild_if_stale: bool = True):
     lib.lgx_decode_batch.argtypes = [vp, u64, vp, u64, u64] + [vp] * 7 + [vp]
     lib.lgx_instance_query.argtypes = [vp, i32, C.POINTER(C.c_int64)]
     lib.lgx_instance_set_timing.argtypes = [vp, i32]
+    lib.lgx_instance_set_option.argtypes = [vp, i32, C.c_int64]
     lib.lgx_init_plan.argtypes = [vp] + [vp] * 6 + [vp]
     lib.lgx_move_eval_batch.argtypes = [vp] + [vp] * 6 + [u64, u64, u64, vp, vp, vp, vp, vp]
     lib.lgx_local_search.argtypes = [vp] + [vp] * 6 + [u64, C.c_uint32, C.c_uint32, C.c_uint32,
@@ -156,14 +163,21 @@ class Instance:
     def set_timing(self, enable: bool):
         _check(self._lib.lgx_instance_set_timing(self._h, 1 if enable else 0))
 
+    def set_option(self, key: int, value: int):
+        """lgx_instance_set_option: launch configuration only (LGX_OPT_*), never results."""
+        _check(self._lib.lgx_instance_set_option(self._h, key, value))
+
     def kernel_times(self):
-        """(ns in lgx_decode_walk, ns in lgx_finish, kernel pairs timed) since set_timing(True)."""
+        """(ns in lgx_decode_cut, ns in lgx_walk_finish, kernel pairs timed) since set_timing(True)."""
         return self.query(12), self.query(13), self.query(14)
 
     def info(self):
         keys = ["image_bytes", "threads", "grid", "smem_bytes", "coords", "state_bytes", "sm_count", "launches",
                 "threads_finish", "smem_bytes_finish", "chunk", "record_bytes"]
-        return {k: self.query(i) for i, k in enumerate(keys)}
+        d = {k: self.query(i) for i, k in enumerate(keys)}
+        d.update(threads_mv=self.query(15), sq_shift=self.query(17), threads_decode=self.query(18),
+                 state_bytes_finish=self.query(19), device=self.query(20))
+        return d
 
     # -- lgx_eval_batch: device tensors in/out (torch), asynchronous on `stream`
     def eval_batch(self, seed, ids=None, first_id=0, n=None, out=None, stream=None):

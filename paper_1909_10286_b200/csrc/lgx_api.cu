@@ -22,11 +22,16 @@ using namespace lgx;
 struct lgx_instance {
   ImgHdr hdr{};
   std::vector<uint8_t> image, image_c;       // host copies of the two images
+  std::vector<uint32_t> s_q, d_q;            // supply / demand quanta (image A is rebuilt when its replication changes)
   uint8_t *d_image = nullptr, *d_image_c = nullptr;
+  size_t d_image_cap = 0;                    // bytes allocated behind d_image
   int device = 0, sm_count = 0;
-  int threads_a = 0, threads_c = 0, grid = 0;  // launch configuration of the persistent kernels
-  size_t smem_a = 0, smem_c = 0;
+  int64_t smem_budget = 0;                   // dynamic shared memory one block may take
+  // launch configuration of the persistent kernels (lgx_decode_cut: a, its diagnostic decode mode: a_dec; lgx_walk_finish: b)
+  int threads_a = 0, threads_a_dec = 0, threads_b = 0, grid = 0;
+  uint64_t a_state = 0, a_state_dec = 0, b_state = 0;   // per-candidate shared-memory bytes
   uint64_t chunk = 0;                          // candidates per decode/finish kernel pair
+  cudaMemPool_t pool = nullptr;                // stream-ordered workspace allocations of this instance
   mutable std::atomic<long long> launches{0};
   // optional per-kernel timing (lgx_instance_set_timing): CUDA events around every launch of a search
   mutable std::atomic<int> timing{0};
@@ -34,7 +39,7 @@ struct lgx_instance {
   // move kernels (Algorithm 1: lgx_init_plan, lgx_move_eval_batch, lgx_local_search)
   MvHdr mv{};
   double2 *d_xy = nullptr;                     // vertex coordinates, every distance mode (lgx_init_plan)
-  int threads_mv = 0; size_t smem_mv = 0;
+  int threads_mv = 0, max_threads_mv = 0; size_t smem_mv = 0; int64_t mv_state = 0;
 };
 
 namespace {
@@ -65,12 +70,12 @@ inline double edge(double ax, double ay, double bx, double by)
 
 using KernelFn = void (*)(const KParams);
 
-template <int MODE> void pick_kernels(const ImgHdr &h, KernelFn &ka, KernelFn &kc)
+template <int MODE> void pick_kernels(const ImgHdr &h, KernelFn &ka, KernelFn &kb)
 {
   const bool p16 = h.perm16 != 0; const int dm = h.coords, mw = (int)h.mask_words;
-  ka = kc = nullptr;
-  // the finish kernel only distinguishes "field x BP table" (DM 0 / 2 -> 0) from coordinates (1)
-#define LGX_PICK(P, D, M) if (p16 == P && dm == D && mw == M) { ka = lgx_decode_walk<P, D, M, MODE>; kc = lgx_finish<P, (D == 1 ? 1 : 0), M, MODE>; }
+  ka = p16 ? lgx_decode_cut<true, MODE> : lgx_decode_cut<false, MODE>;
+  kb = nullptr;
+#define LGX_PICK(P, D, M) if (p16 == P && dm == D && mw == M) kb = lgx_walk_finish<P, D, M, MODE>;
   LGX_PICK(false, 0, 1) LGX_PICK(false, 0, 2) LGX_PICK(false, 1, 1) LGX_PICK(false, 1, 2) LGX_PICK(false, 2, 1) LGX_PICK(false, 2, 2)
   LGX_PICK(true,  0, 1) LGX_PICK(true,  0, 2) LGX_PICK(true,  1, 1) LGX_PICK(true,  1, 2) LGX_PICK(true,  2, 1) LGX_PICK(true,  2, 2)
 #undef LGX_PICK
@@ -82,6 +87,65 @@ void fill_round_keys(KParams &P, uint64_t seed)
   for (int r = 0; r < 10; ++r) { P.rk[2 * r] = k0; P.rk[2 * r + 1] = k1; k0 += kPhiloxW0; k1 += kPhiloxW1; }
 }
 
+// Every compute entry point runs on the device the instance was created on (its images live there).
+int check_device(const lgx_instance *I)
+{
+  int cur = -1;
+  CU(cudaGetDevice(&cur));
+  if (cur != I->device) { g_cuda_msg = "the current CUDA device is not the one the instance was created on"; return LGX_EINVAL; }
+  return LGX_OK;
+}
+
+// Image A: s_q replicated 2^sq_shift times (replica r of field f at (f << sq_shift) + r: lanes of a warp read
+// different banks whatever field they hold) and the demand quanta.  Uploads it.
+int build_image_a(lgx_instance *I, uint32_t sq_shift)
+{
+  ImgHdr &H = I->hdr;
+  const uint32_t nf = (uint32_t)H.n_f, nb = (uint32_t)H.n_b;
+  H.sq_shift = sq_shift;
+  uint32_t off = 0;
+  H.off_sq = off; off = align16(off + 4u * (nf << sq_shift));
+  H.off_dq = off; off = align16(off + 4u * nb);
+  H.image_bytes = off;
+  I->image.assign(H.image_bytes, 0);
+  uint32_t *sq = reinterpret_cast<uint32_t *>(I->image.data() + H.off_sq);
+  for (uint32_t f = 0; f < nf; ++f)
+    for (uint32_t r = 0; r < (1u << sq_shift); ++r) sq[(f << sq_shift) + r] = I->s_q[f];
+  uint32_t *dq = reinterpret_cast<uint32_t *>(I->image.data() + H.off_dq);
+  for (uint32_t b = 0; b < nb; ++b) dq[b] = I->d_q[b];
+  if (I->d_image && I->d_image_cap < H.image_bytes) { cudaFree(I->d_image); I->d_image = nullptr; }
+  if (!I->d_image) { CU(cudaMalloc((void **)&I->d_image, H.image_bytes)); I->d_image_cap = H.image_bytes; }
+  CU(cudaMemcpy(I->d_image, I->image.data(), H.image_bytes, cudaMemcpyHostToDevice));
+  return LGX_OK;
+}
+
+int64_t fit_threads(int64_t budget, int64_t image, int64_t state, int64_t cap)
+{
+  const int64_t t = (budget - image) / std::max<int64_t>(state, 1);
+  return std::min<int64_t>(t, cap) / 32 * 32;
+}
+
+void free_instance(lgx_instance *I)
+{
+  if (I->d_xy) cudaFree(I->d_xy);
+  if (I->d_image) cudaFree(I->d_image);
+  if (I->d_image_c) cudaFree(I->d_image_c);
+  if (I->pool) cudaMemPoolDestroy(I->pool);
+  delete I;
+}
+
+// The kernels take up to 227 KB of dynamic shared memory: the opt-in attribute is set ONCE per kernel, to the
+// device maximum, when an instance that uses the kernel is created — never per call, so concurrent calls on
+// instances of different sizes cannot race on it.
+int allow_max_smem(const void *fn, int smem_optin)
+{
+  CU(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, std::min(smem_optin, kMaxSmem)));
+  return LGX_OK;
+}
+
+using MvKernelFn = void (*)(const MvParams);
+void pick_move_kernels(const ImgHdr &h, MvKernelFn &kb, MvKernelFn &ks);
+
 }  // namespace
 
 extern "C" {
@@ -91,7 +155,7 @@ const char *lgx_strerror(int code)
   switch (code) {
     case LGX_OK:      return "ok";
     case LGX_EINVAL:  return "invalid argument or instance outside the documented ranges";
-    case LGX_ETOOBIG: return "instance image or per-candidate state does not fit (shared memory / 32-bit quanta)";
+    case LGX_ETOOBIG: return "instance image or per-candidate state does not fit (shared memory / 32-bit quanta / kernel limits)";
     case LGX_ECUDA:   return g_cuda_msg.c_str();
     case LGX_ENOMEM:  return "out of memory";
     default:          return "unknown lgx error code";
@@ -112,7 +176,10 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   if (!(std::isfinite(d->v_hu_road_kmh) && d->v_hu_road_kmh > 0.0)) return LGX_EINVAL;
   if (!(std::isfinite(d->v_su_road_kmh) && d->v_su_road_kmh > 0.0)) return LGX_EINVAL;
   if (!fin_nonneg(d->su_fill_h_per_t) || !fin_nonneg(d->w_path) || !fin_nonneg(d->w_time)) return LGX_EINVAL;
-  if ((d->flags & ~(uint32_t)(LGX_FLAG_HU_BALANCE | LGX_FLAG_MAKESPAN_FILTER | LGX_FLAG_FIX_FIELD_BP)) != 0u) return LGX_EINVAL;
+  const uint32_t known_flags = LGX_FLAG_HU_BALANCE | LGX_FLAG_MAKESPAN_FILTER | LGX_FLAG_FIX_FIELD_BP |
+                               LGX_FLAG_DIST_COORDS | LGX_FLAG_DIST_MIXED;
+  if ((d->flags & ~known_flags) != 0u) return LGX_EINVAL;
+  if ((d->flags & LGX_FLAG_DIST_COORDS) && (d->flags & LGX_FLAG_DIST_MIXED)) return LGX_EINVAL;
   const int nf = d->n_fields, nb = d->n_bps, nhu = d->n_hu_total, nsu = d->n_su_total, nt = d->n_tours;
   for (int f = 0; f < nf; ++f)
     if (!std::isfinite(d->field_x[f]) || !std::isfinite(d->field_y[f]) || !fin_nonneg(d->field_supply_t[f]) ||
@@ -135,8 +202,8 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   const int64_t lim = (int64_t)1 << 32;
   if (s_max * (int64_t)nsu + c_sum >= lim || s_sum >= lim || h_sum >= lim || r_sum >= lim) return LGX_ETOOBIG;
   for (int b = 0; b < nb; ++b) if (d_q[b] >= lim) return LGX_ETOOBIG;
-  // kernel limits of this build
-  if (nb > 127 || nsu > 128) return LGX_ETOOBIG;
+  // kernel limits of this build (include/lgx.h): 7-bit BP ids in the plan entries, SU sets of 2 x 64 bits
+  if (nb > LGX_MAX_BPS || nsu > LGX_MAX_SUS) return LGX_ETOOBIG;
 
   lgx_instance *I = new (std::nothrow) lgx_instance();
   if (!I) return LGX_ENOMEM;
@@ -151,6 +218,10 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   const uint32_t MW = H.mask_words;
   // stream-4 draws taken up front: (N_B-1) failures + geometric extras, with slack; <= 64
   H.n_extra_blocks = (uint32_t)std::min(16, ((nb - 1) * 4 / 3 + 8 + 3) / 4);
+  I->s_q.resize(nf); I->d_q.resize(nb);
+  for (int f = 0; f < nf; ++f) I->s_q[f] = (uint32_t)s_q[f];
+  H.zero_demand = 0u;
+  for (int b = 0; b < nb; ++b) { I->d_q[b] = (uint32_t)d_q[b]; if (d_q[b] == 0) H.zero_demand = 1u; }
 
   // ---- permutation array: right-aligned inside its words so that consumption position
   //      p = EPW*q + t always sits in a static lane of word row wtop - q
@@ -168,31 +239,27 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   H.n_bpseq_words  = cdiv((uint32_t)nb, 4u);
   H.n_segend_words = cdiv((uint32_t)nb, EPW);
 
-  // ---- state rows of the decode/walk kernel (BP partition + field loop only: the HU / SU
-  //      partitions run in the finish kernel, for the candidates that pass eq. (2))
+  // ---- state rows of the decode/cut kernel: 32-bit rows only (the kernel touches no FP64)
   const uint32_t n_units = (uint32_t)std::max(nhu, nsu);
   {
     uint32_t r = 0;
-    H.a64_sd = r; H.a64_ent = r; r += (uint32_t)nb;    // entry j is consumed before SD[j] is flushed: same rows
-    H.a64_lt = r; r += (uint32_t)nt;
-    H.a64_rows = r;
-    r = 0;
-    H.a32_perm = r;   r += H.n_perm_words;
-    H.a32_bpseq = r;  r += H.n_bpseq_words;
-    // partition scratch (dead once the field loop starts) shares its rows with the segment ends;
-    // the diagnostic decode mode also runs the unit partitions through scratch A
-    const uint32_t scra_words = ((uint32_t)std::max(nb, (int)n_units) + 3u) / 4u + 1u, scrb_words = cdiv((uint32_t)nb, 4u);
-    H.a32_scra = r; H.a32_segend = r; H.a32_scrb = r + scra_words;
-    r += std::max(scra_words + scrb_words, (uint32_t)nb);
-    H.a32_hq = r;     r += (uint32_t)nt;
+    H.a32_perm = r;  r += H.n_perm_words;
+    H.a32_bpseq = r; r += H.n_bpseq_words;
+    H.a32_ds = r;    r += (uint32_t)nb;                    // demands in plan order; cut j overwrites demand j once consumed
+    H.a32_scra = r;  r += ((uint32_t)nb + 3u) / 4u + 1u;   // BP partition: Fisher-Yates array
+    H.a32_scrb = r;  r += cdiv((uint32_t)nb, 4u);          // bin of consumption position p
+    H.a32_cnt = r;   r += cdiv((uint32_t)nt, 4u);          // counting sort cursors
     H.a32_rows = r;
+    H.a32_scru = r;  r += (n_units + 3u) / 4u + 1u;        // diagnostic decode mode only: unit partitions
+    H.a32_rows_dec = r;
   }
-  // ---- state rows of the finish kernel
+  // ---- state rows of the walk/finish kernel
   {
     uint32_t r = 0;
-    H.c64_w = r; r += (uint32_t)nt;
-    H.c64_e = r; r += (uint32_t)nt;
+    H.c64_w = r; r += (uint32_t)nt;                        // T_wait(g); then the shuttle sum
+    H.c64_e = r; r += (uint32_t)nt;                        // E(g)
     H.c64_mask = r; r += (uint32_t)nt * MW;
+    H.c64_sd = r; r += (uint32_t)nb;                       // SD per plan BP with fields; then L_tour(g) (N_T <= N_B)
     H.c64_rows = r;
     r = 0;
     H.c32_s = r; r += (uint32_t)nt;
@@ -200,54 +267,39 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
     H.c32_r = r; r += (uint32_t)nt;
     H.c32_ng = r; r += (uint32_t)nt;
     H.c32_magic = r; r += (uint32_t)nt;
-    H.c32_ent = r; r += (uint32_t)nb;
-    H.c32_scra = r; r += (n_units + 3u) / 4u + 1u;
+    H.c32_hq = r; r += (uint32_t)nt;
+    H.c32_ent = r; r += std::max((uint32_t)nb + 1u, (n_units + 3u) / 4u + 1u);   // walk entries + sentinel; partition scratch before
     H.c32_rows = r;
   }
   // ---- queue record
   {
     uint32_t w = 2;
-    H.rec_tw = 3u;
-    H.rec_tour = w;   w += (uint32_t)nt * H.rec_tw;
-    H.rec_sd = w;     w += 2u * (uint32_t)nb;
     H.rec_bpseq = w;  w += H.n_bpseq_words;
     H.rec_segend = w; w += H.n_segend_words;
     H.rec_perm = w;   w += H.n_perm_words;
     H.rec_words = w;
   }
-  const uint64_t a_state = 8ull * H.a64_rows + 4ull * H.a32_rows;
-  const uint64_t c_state = 8ull * H.c64_rows + 4ull * H.c32_rows;
+  I->a_state = 4ull * H.a32_rows;
+  I->a_state_dec = 4ull * H.a32_rows_dec;
+  I->b_state = 8ull * H.c64_rows + 4ull * H.c32_rows;
 
-  // ---- image AB: packed distance tables when they leave room for >= 256 candidates per SM,
-  //      else vertex coordinates
+  // ---- image C: packed distance tables when they leave room for >= 256 candidates per SM, else the
+  //      field x BP table + coordinates while the table is small, else coordinates only
   const uint64_t tri_bytes = (uint64_t)(nf + 1) * (uint64_t)nf / 2 * 8, dfb_bytes = (uint64_t)nf * nb * 8;
-  const uint64_t small_bytes = 8ull * nf + 4ull * nb + 64;
-  // distance mode: 0 = both tables, 2 = field x BP table + coordinates for the HU legs, 1 = coordinates only
   const uint64_t xy_bytes = 16ull * (1 + nb + nf), room = (uint64_t)kMaxSmem - 1024;
-  if (small_bytes + tri_bytes + dfb_bytes + 256ull * a_state <= room) H.coords = 0;
-  else {
-    // Measured on B200 (Large config): at the 8-9 resident warps per SM these sizes allow, the
-    // kernels are latency-bound and recomputing sqrt from coordinates (one conflict-prone
-    // LDS.128 shared by both legs) beats a second conflict-prone table look-up (1.4e8 vs 0.9e8
-    // cand/s), so mode 2 is never picked automatically; LGX_DIST_MODE=2 selects it for tuning.
-    H.coords = 1;
-  }
-  if (const char *ev = std::getenv("LGX_DIST_MODE")) { const int v = std::atoi(ev); if (v == 1 || v == 2) H.coords = v; }  // tuning knob
-  uint32_t off = 0;
-  H.off_dtri = H.off_dfb = H.off_xy = 0;
-  if (H.coords == 0) { H.off_dtri = off; off = align16(off + (uint32_t)tri_bytes); }
-  if (H.coords != 1) { H.off_dfb = off; off = align16(off + (uint32_t)dfb_bytes); }
-  if (H.coords != 0) { H.off_xy = off; off = align16(off + (uint32_t)xy_bytes); }
-  H.off_sh   = off; off = align16(off + 8u * (uint32_t)nf);
-  H.off_dq   = off; off = align16(off + 4u * (uint32_t)nb);
-  H.image_bytes = off;
-  // ---- image C
   const int n_rcp = std::max(nf, std::max(nb, nhu)) + 1;
-  off = 0;
-  H.offc_dfb = H.offc_xy = 0;
+  const uint64_t tail_bytes = 8ull * nf + 4ull * nsu + 8ull * n_rcp + 2ull * nsu + 8ull * nhu + 2ull * nhu + 256;
+  if (tail_bytes + tri_bytes + dfb_bytes + 256ull * I->b_state <= room) H.coords = 0;
+  else if (dfb_bytes <= 32ull * 1024 && tail_bytes + dfb_bytes + xy_bytes + 128ull * I->b_state <= room) H.coords = 2;
+  else H.coords = 1;
+  if (d->flags & LGX_FLAG_DIST_COORDS) H.coords = 1;      // tuning flags: same D(u,v) bit for bit
+  if ((d->flags & LGX_FLAG_DIST_MIXED) && tail_bytes + dfb_bytes + xy_bytes + 32ull * I->b_state <= room) H.coords = 2;
+  uint32_t off = 0;
+  H.offc_dtri = H.offc_dfb = H.offc_xy = 0;
+  if (H.coords == 0) { H.offc_dtri = off; off = align16(off + (uint32_t)tri_bytes); }
   if (H.coords != 1) { H.offc_dfb = off; off = align16(off + (uint32_t)dfb_bytes); }
-  else               { H.offc_xy = off; off = align16(off + (uint32_t)xy_bytes); }
-  H.offc_s    = off; off = align16(off + 4u * (uint32_t)nf);
+  if (H.coords != 0) { H.offc_xy = off; off = align16(off + (uint32_t)xy_bytes); }
+  H.offc_sh   = off; off = align16(off + 8u * (uint32_t)nf);
   H.offc_cs   = off; off = align16(off + 4u * (uint32_t)nsu);
   H.offc_rcp  = off; off = align16(off + 8u * (uint32_t)n_rcp);
   H.offc_unit = off; off = align16(off + (uint32_t)nsu);
@@ -258,12 +310,11 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   H.offc_hrank = off; off = align16(off + (uint32_t)nhu);
   H.imagec_bytes = off;
 
-  I->image.assign(H.image_bytes, 0);
   I->image_c.assign(H.imagec_bytes, 0);
-  uint8_t *img = I->image.data(), *imc = I->image_c.data();
+  uint8_t *imc = I->image_c.data();
   if (H.coords == 0) {
     // strict lower triangle over {HQ = 0, field f = f + 1}: entry (hi, lo) at hi(hi-1)/2 + lo
-    double *tri = reinterpret_cast<double *>(img + H.off_dtri);
+    double *tri = reinterpret_cast<double *>(imc + H.offc_dtri);
     for (int hi = 1; hi <= nf; ++hi)
       for (int lo = 0; lo < hi; ++lo) {
         const double ax = d->field_x[hi - 1], ay = d->field_y[hi - 1];
@@ -272,25 +323,18 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
       }
   }
   if (H.coords != 1) {
-    double *dfb = reinterpret_cast<double *>(img + H.off_dfb), *dfc = reinterpret_cast<double *>(imc + H.offc_dfb);
+    double *dfc = reinterpret_cast<double *>(imc + H.offc_dfb);
     for (int f = 0; f < nf; ++f)
       for (int b = 0; b < nb; ++b)
-        dfb[(size_t)f * nb + b] = dfc[(size_t)f * nb + b] = edge(d->field_x[f], d->field_y[f], d->bp_x[b], d->bp_y[b]);
+        dfc[(size_t)f * nb + b] = edge(d->field_x[f], d->field_y[f], d->bp_x[b], d->bp_y[b]);
   }
-  {
-    std::vector<double *> dst;
-    if (H.coords != 0) dst.push_back(reinterpret_cast<double *>(img + H.off_xy));
-    if (H.coords == 1) dst.push_back(reinterpret_cast<double *>(imc + H.offc_xy));
-    for (double *xy : dst) {
-      xy[0] = d->hq_x; xy[1] = d->hq_y;
-      for (int b = 0; b < nb; ++b) { xy[2 * (1 + b)] = d->bp_x[b]; xy[2 * (1 + b) + 1] = d->bp_y[b]; }
-      for (int f = 0; f < nf; ++f) { xy[2 * (1 + nb + f)] = d->field_x[f]; xy[2 * (1 + nb + f) + 1] = d->field_y[f]; }
-    }
-  }
-  uint32_t *sh = reinterpret_cast<uint32_t *>(img + H.off_sh), *sc = reinterpret_cast<uint32_t *>(imc + H.offc_s);
-  for (int f = 0; f < nf; ++f) { sh[2 * f] = sc[f] = (uint32_t)s_q[f]; sh[2 * f + 1] = (uint32_t)h_q[f]; }
-  uint32_t *dq = reinterpret_cast<uint32_t *>(img + H.off_dq);
-  for (int b = 0; b < nb; ++b) dq[b] = (uint32_t)d_q[b];
+  std::vector<double> xyv(2 * (size_t)(1 + nb + nf));
+  xyv[0] = d->hq_x; xyv[1] = d->hq_y;
+  for (int b = 0; b < nb; ++b) { xyv[2 * (1 + b)] = d->bp_x[b]; xyv[2 * (1 + b) + 1] = d->bp_y[b]; }
+  for (int f = 0; f < nf; ++f) { xyv[2 * (1 + nb + f)] = d->field_x[f]; xyv[2 * (1 + nb + f) + 1] = d->field_y[f]; }
+  if (H.coords != 0) std::memcpy(imc + H.offc_xy, xyv.data(), xyv.size() * 8);
+  uint32_t *shc = reinterpret_cast<uint32_t *>(imc + H.offc_sh);
+  for (int f = 0; f < nf; ++f) { shc[2 * f] = (uint32_t)s_q[f]; shc[2 * f + 1] = (uint32_t)h_q[f]; }
   uint32_t *rq = reinterpret_cast<uint32_t *>(imc + H.offc_rq);
   for (int u = 0; u < nhu; ++u) rq[u] = (uint32_t)r_q[u];
   // SUs ascending by (capacity quanta, unit index): "rising fill times" (R16, R17)
@@ -321,36 +365,47 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   int smem_optin = 0;
   cudaDeviceGetAttribute(&I->sm_count, cudaDevAttrMultiProcessorCount, I->device);
   cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, I->device);
-  const int64_t budget = std::min<int64_t>(smem_optin, kMaxSmem) - 1024;   // static smem of the reduction
-  int64_t ta = (budget - (int64_t)H.image_bytes) / (int64_t)a_state;
-  // finish kernel: kFinishBlocksPerSM blocks per SM (each with its own copy of image C)
-  int64_t tc = ((budget + 1024) / kFinishBlocksPerSM - 1024 - (int64_t)H.imagec_bytes) / (int64_t)c_state;
-  ta = std::min<int64_t>(ta, kMaxThreadsA) / 32 * 32;
-  tc = std::min<int64_t>(tc, kMaxThreads) / 32 * 32;
-  if (const char *ev = std::getenv("LGX_THREADS_A")) { const int v = std::atoi(ev); if (v >= 32 && v <= ta) ta = v / 32 * 32; }  // tuning knobs
-  if (const char *ev = std::getenv("LGX_THREADS_C")) { const int v = std::atoi(ev); if (v >= 32 && v <= tc) tc = v / 32 * 32; }
-  if (ta < 32 || tc < 32) { delete I; return LGX_ETOOBIG; }
-  I->threads_a = (int)ta; I->threads_c = (int)tc;
+  I->smem_budget = std::min<int64_t>(smem_optin, kMaxSmem) - 1024;   // static smem of the reduction
+  const int64_t budget = I->smem_budget;
+  // s_q replication of image A: as many replicas (<= 32, a power of two) as 16 KB hold
+  uint32_t sq_shift = 0;
+  while (sq_shift < 5u && 4ull * ((uint64_t)nf << (sq_shift + 1u)) <= 16ull * 1024) ++sq_shift;
+  int rc = build_image_a(I, sq_shift);
+  if (rc != LGX_OK) { free_instance(I); return rc; }
+  I->threads_a     = (int)fit_threads(budget, H.image_bytes, (int64_t)I->a_state, kMaxThreadsA);
+  I->threads_a_dec = (int)fit_threads(budget, H.image_bytes, (int64_t)I->a_state_dec, kMaxThreadsA);
+  I->threads_b     = (int)fit_threads(budget, H.imagec_bytes, (int64_t)I->b_state, kMaxThreadsB);
+  if (I->threads_a < 32 || I->threads_a_dec < 32 || I->threads_b < 32) { free_instance(I); return LGX_ETOOBIG; }
   I->grid = I->sm_count;                       // one persistent block per SM
-  I->smem_a = (size_t)H.image_bytes + a_state * (size_t)ta;
-  I->smem_c = (size_t)H.imagec_bytes + c_state * (size_t)tc;
-  // candidates per kernel pair: queue of at most 192 MiB, a whole number of grid rounds
+  // candidates per kernel pair: the queue holds a whole chunk (every candidate may pass eq. (2)); <= 512 MiB, <= 2^22
   {
-    const uint64_t round = (uint64_t)I->grid * (uint64_t)ta;
-    uint64_t cap = (192ull << 20) / (4ull * H.rec_words);
-    cap = std::min<uint64_t>(cap, 1ull << 21);
-    if (const char *ev = std::getenv("LGX_CHUNK_LOG2")) {      // tuning knob (bench sweeps); default above
-      const int lg = std::atoi(ev);
-      if (lg >= 10 && lg <= 26) cap = 1ull << lg;
-    }
-    cap = std::max<uint64_t>(cap / round, 1) * round;
-    I->chunk = cap;
+    uint64_t cap = (512ull << 20) / (4ull * H.rec_words);
+    cap = std::min<uint64_t>(cap, 1ull << 22);
+    I->chunk = std::max<uint64_t>(cap / 1024, 1) * 1024;
   }
-  if ((e = cudaMalloc((void **)&I->d_image, H.image_bytes)) != cudaSuccess) { delete I; return cuda_fail(e, "cudaMalloc(image)"); }
-  if ((e = cudaMalloc((void **)&I->d_image_c, H.imagec_bytes)) != cudaSuccess) { cudaFree(I->d_image); delete I; return cuda_fail(e, "cudaMalloc(image C)"); }
-  if ((e = cudaMemcpy(I->d_image, img, H.image_bytes, cudaMemcpyHostToDevice)) != cudaSuccess ||
-      (e = cudaMemcpy(I->d_image_c, imc, H.imagec_bytes, cudaMemcpyHostToDevice)) != cudaSuccess) {
-    cudaFree(I->d_image); cudaFree(I->d_image_c); delete I; return cuda_fail(e, "cudaMemcpy(image)");
+  if ((e = cudaMalloc((void **)&I->d_image_c, H.imagec_bytes)) != cudaSuccess) { free_instance(I); return cuda_fail(e, "cudaMalloc(image C)"); }
+  if ((e = cudaMemcpy(I->d_image_c, imc, H.imagec_bytes, cudaMemcpyHostToDevice)) != cudaSuccess) { free_instance(I); return cuda_fail(e, "cudaMemcpy(image C)"); }
+  {
+    // workspaces come from a pool of this instance that keeps its memory between calls
+    cudaMemPoolProps props{};
+    props.allocType = cudaMemAllocationTypePinned;
+    props.handleTypes = cudaMemHandleTypeNone;
+    props.location.type = cudaMemLocationTypeDevice;
+    props.location.id = I->device;
+    if ((e = cudaMemPoolCreate(&I->pool, &props)) != cudaSuccess) { I->pool = nullptr; free_instance(I); return cuda_fail(e, "cudaMemPoolCreate"); }
+    uint64_t keep = ~0ull;
+    cudaMemPoolSetAttribute(I->pool, cudaMemPoolAttrReleaseThreshold, &keep);
+  }
+  {
+    KernelFn ka, kb;
+    pick_kernels<MODE_EVAL>(H, ka, kb);
+    if (!kb) { free_instance(I); return LGX_EINVAL; }
+    rc = allow_max_smem((const void *)ka, smem_optin); if (rc == LGX_OK) rc = allow_max_smem((const void *)kb, smem_optin);
+    pick_kernels<MODE_SEARCH>(H, ka, kb);
+    if (rc == LGX_OK) rc = allow_max_smem((const void *)ka, smem_optin); if (rc == LGX_OK) rc = allow_max_smem((const void *)kb, smem_optin);
+    pick_kernels<MODE_DECODE>(H, ka, kb);
+    if (rc == LGX_OK) rc = allow_max_smem((const void *)ka, smem_optin); if (rc == LGX_OK) rc = allow_max_smem((const void *)kb, smem_optin);
+    if (rc != LGX_OK) { free_instance(I); return rc; }
   }
   // ---- move kernels: shared-memory layout (lgx_moves.cuh) and vertex coordinates for lgx_init_plan
   {
@@ -400,20 +455,21 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
     if (hb) { M.m32_r = r; r += (uint32_t)nt; }
     M.m32_rows = r;
     M.slot_words = 3u + (uint32_t)nt * MW + (uint32_t)nt;
-    const int64_t mv_state = 8ll * M.m64_rows + 4ll * M.m32_rows;
-    int64_t tm = (budget - 256 - (int64_t)M.off_state) / mv_state;      // static smem of the reductions
+    I->mv_state = 8ll * M.m64_rows + 4ll * M.m32_rows;
+    int64_t tm = (budget - 256 - (int64_t)M.off_state) / I->mv_state;      // static smem of the reductions
     tm = std::min<int64_t>(tm, kMvThreads) / 32 * 32;
-    if (const char *ev = std::getenv("LGX_THREADS_MV")) { const int v = std::atoi(ev); if (v >= 64 && v <= tm) tm = v / 32 * 32; }
-    if (nt > 64 || nhu > 64) tm = 0;                                      // 64-bit sets of tours and of HUs
-    I->threads_mv = tm >= 64 ? (int)tm : 0;                               // 0: the move kernels do not fit (LGX_ETOOBIG there)
-    I->smem_mv = (size_t)M.off_state + (size_t)mv_state * (size_t)std::max<int64_t>(tm, 0);
-    std::vector<double> xy(2 * (size_t)(1 + nb + nf));
-    xy[0] = d->hq_x; xy[1] = d->hq_y;
-    for (int b = 0; b < nb; ++b) { xy[2 * (1 + b)] = d->bp_x[b]; xy[2 * (1 + b) + 1] = d->bp_y[b]; }
-    for (int f = 0; f < nf; ++f) { xy[2 * (1 + nb + f)] = d->field_x[f]; xy[2 * (1 + nb + f) + 1] = d->field_y[f]; }
-    if ((e = cudaMalloc((void **)&I->d_xy, xy.size() * 8)) != cudaSuccess ||
-        (e = cudaMemcpy(I->d_xy, xy.data(), xy.size() * 8, cudaMemcpyHostToDevice)) != cudaSuccess) {
-      cudaFree(I->d_image); cudaFree(I->d_image_c); cudaFree(I->d_xy); delete I; return cuda_fail(e, "cudaMalloc/cudaMemcpy(xy)");
+    if (nt > LGX_MAX_MOVE_TOURS || nhu > LGX_MAX_MOVE_HUS) tm = 0;        // 64-bit sets of tours and of HUs
+    I->max_threads_mv = tm >= 64 ? (int)tm : 0;                           // 0: the move kernels do not fit (LGX_ETOOBIG there)
+    I->threads_mv = I->max_threads_mv;
+    I->smem_mv = (size_t)M.off_state + (size_t)I->mv_state * (size_t)I->threads_mv;
+    if ((e = cudaMalloc((void **)&I->d_xy, xyv.size() * 8)) != cudaSuccess ||
+        (e = cudaMemcpy(I->d_xy, xyv.data(), xyv.size() * 8, cudaMemcpyHostToDevice)) != cudaSuccess) {
+      free_instance(I); return cuda_fail(e, "cudaMalloc/cudaMemcpy(xy)");
+    }
+    if (I->threads_mv) {
+      MvKernelFn kb2, ks2; pick_move_kernels(H, kb2, ks2);
+      rc = allow_max_smem((const void *)kb2, smem_optin); if (rc == LGX_OK) rc = allow_max_smem((const void *)ks2, smem_optin);
+      if (rc != LGX_OK) { free_instance(I); return rc; }
     }
   }
   *out = I;
@@ -423,23 +479,65 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
 int lgx_instance_destroy(lgx_instance *I)
 {
   if (!I) return LGX_EINVAL;
-  if (I->d_xy) cudaFree(I->d_xy);
-  if (I->d_image) cudaFree(I->d_image);
-  if (I->d_image_c) cudaFree(I->d_image_c);
-  delete I;
+  free_instance(I);
   return LGX_OK;
+}
+
+int lgx_instance_set_option(lgx_instance *I, int key, int64_t value)
+{
+  if (!I) return LGX_EINVAL;
+  const ImgHdr &H = I->hdr;
+  const int64_t budget = I->smem_budget;
+  auto threads_ok = [](int64_t v, int64_t lo, int64_t hi) { return v >= lo && v <= hi && v % 32 == 0; };
+  switch (key) {
+    case LGX_OPT_THREADS_A: {
+      const int64_t hi = fit_threads(budget, H.image_bytes, (int64_t)I->a_state, kMaxThreadsA);
+      if (!threads_ok(value, 32, hi)) return LGX_EINVAL;
+      I->threads_a = (int)value; I->threads_a_dec = (int)std::min<int64_t>(value, fit_threads(budget, H.image_bytes, (int64_t)I->a_state_dec, kMaxThreadsA));
+      return LGX_OK;
+    }
+    case LGX_OPT_THREADS_B: {
+      const int64_t hi = fit_threads(budget, H.imagec_bytes, (int64_t)I->b_state, kMaxThreadsB);
+      if (!threads_ok(value, 32, hi)) return LGX_EINVAL;
+      I->threads_b = (int)value;
+      return LGX_OK;
+    }
+    case LGX_OPT_THREADS_MV: {
+      if (!threads_ok(value, 64, I->max_threads_mv)) return LGX_EINVAL;
+      I->threads_mv = (int)value;
+      I->smem_mv = (size_t)I->mv.off_state + (size_t)I->mv_state * (size_t)I->threads_mv;
+      return LGX_OK;
+    }
+    case LGX_OPT_CHUNK_LOG2: {
+      if (value < 10 || value > 26) return LGX_EINVAL;
+      I->chunk = 1ull << value;
+      return LGX_OK;
+    }
+    case LGX_OPT_SQ_SHIFT: {
+      if (value < 0 || value > 5) return LGX_EINVAL;
+      const int64_t img = 16 + 4ll * ((int64_t)H.n_f << value) + 16 + 4ll * H.n_b;
+      if (fit_threads(budget, img, (int64_t)I->a_state_dec, kMaxThreadsA) < 32) return LGX_ETOOBIG;
+      int rc = check_device(I);
+      if (rc == LGX_OK) { cudaDeviceSynchronize(); rc = build_image_a(I, (uint32_t)value); }
+      if (rc != LGX_OK) return rc;
+      I->threads_a     = (int)std::min<int64_t>(I->threads_a, fit_threads(budget, H.image_bytes, (int64_t)I->a_state, kMaxThreadsA));
+      I->threads_a_dec = (int)std::min<int64_t>(I->threads_a_dec, fit_threads(budget, H.image_bytes, (int64_t)I->a_state_dec, kMaxThreadsA));
+      return LGX_OK;
+    }
+    default: return LGX_EINVAL;
+  }
 }
 
 }  // extern "C"
 
 namespace {
 
-// One call = chunks of at most I->chunk candidates; per chunk the decode/walk kernel fills the
-// queue and the finish kernel drains it (same stream, so the pair is ordered).  The workspace
+// One call = chunks of at most I->chunk candidates; per chunk the decode/cut kernel fills the
+// queue and the walk/finish kernel drains it (same stream, so the pair is ordered).  The workspace
 // is allocated stream-ordered per call, so concurrent calls on different streams are legal.
 struct Workspace {
   uint8_t *base = nullptr;
-  unsigned int *q_count = nullptr, *done = nullptr;
+  unsigned int *q_count = nullptr, *done = nullptr, *ctr_a = nullptr, *ctr_b = nullptr;
   unsigned long long *result = nullptr, *block_best = nullptr;
   uint32_t *queue = nullptr;
   uint64_t cap = 0;
@@ -447,13 +545,13 @@ struct Workspace {
 
 int ws_alloc(const lgx_instance *I, uint64_t n, bool search, cudaStream_t st, Workspace &W)
 {
-  W.cap = std::min<uint64_t>(I->chunk, n);
-  const size_t head = 64 + 16ull * (size_t)I->grid * kFinishBlocksPerSM;
+  W.cap = std::min<uint64_t>(I->chunk, (n + 31) / 32 * 32);
+  const size_t head = 64 + 16ull * (size_t)I->grid;
   const size_t qoff = (head + 255) & ~(size_t)255;
   const size_t bytes = qoff + 4ull * I->hdr.rec_words * W.cap;
-  CU(cudaMallocAsync((void **)&W.base, bytes, st));
+  CU(cudaMallocFromPoolAsync((void **)&W.base, bytes, I->pool, st));
   W.q_count = reinterpret_cast<unsigned int *>(W.base);
-  W.done = W.q_count + 1;
+  W.done = W.q_count + 1; W.ctr_a = W.q_count + 2; W.ctr_b = W.q_count + 3;
   W.result = reinterpret_cast<unsigned long long *>(W.base + 16);
   W.block_best = reinterpret_cast<unsigned long long *>(W.base + 64);
   W.queue = reinterpret_cast<uint32_t *>(W.base + qoff);
@@ -463,27 +561,26 @@ int ws_alloc(const lgx_instance *I, uint64_t n, bool search, cudaStream_t st, Wo
   return LGX_OK;
 }
 
-int run_chunks(const lgx_instance *I, KernelFn ka, KernelFn kc, KParams &P, uint64_t n, const Workspace &W, cudaStream_t st,
-               std::vector<cudaEvent_t> *evs = nullptr)
+int run_chunks(const lgx_instance *I, KernelFn ka, KernelFn kb, KParams &P, uint64_t n, const Workspace &W, cudaStream_t st,
+               bool decode_mode, std::vector<cudaEvent_t> *evs = nullptr)
 {
-  if (!ka || !kc) return LGX_EINVAL;
-  CU(cudaFuncSetAttribute((const void *)ka, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)I->smem_a));
-  CU(cudaFuncSetAttribute((const void *)kc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)I->smem_c));
+  if (!ka || !kb) return LGX_EINVAL;
+  const uint64_t ta = (uint64_t)(decode_mode ? I->threads_a_dec : I->threads_a), tb = (uint64_t)I->threads_b;
+  const size_t smem_a = (size_t)I->hdr.image_bytes + (size_t)(decode_mode ? I->a_state_dec : I->a_state) * ta;
+  const size_t smem_b = (size_t)I->hdr.imagec_bytes + (size_t)I->b_state * tb;
   P.H = I->hdr; P.image = I->d_image; P.image_c = I->d_image_c;
-  P.queue = W.queue; P.cap = (uint32_t)W.cap; P.q_count = W.q_count;
+  P.queue = W.queue; P.cap = (uint32_t)W.cap; P.q_count = W.q_count; P.ctr_a = W.ctr_a; P.ctr_b = W.ctr_b;
   P.done_counter = W.done; P.block_best = W.block_best; P.result = W.result;
   void *args[] = { (void *)&P };
   for (uint64_t base = 0; base < n; base += W.cap) {
     P.base_i = base; P.n = std::min<uint64_t>(W.cap, n - base);
-    const uint64_t blocks_a = (P.n + (uint64_t)I->threads_a - 1) / (uint64_t)I->threads_a;
-    const unsigned grid_a = (unsigned)std::min<uint64_t>((uint64_t)I->grid, blocks_a);
-    const uint64_t blocks_c = (P.n + (uint64_t)I->threads_c - 1) / (uint64_t)I->threads_c;
-    const unsigned grid_c = (unsigned)std::min<uint64_t>((uint64_t)I->grid * kFinishBlocksPerSM, blocks_c);
+    const unsigned grid_a = (unsigned)std::min<uint64_t>((uint64_t)I->grid, (P.n + ta - 1) / ta);
+    const unsigned grid_b = (unsigned)std::min<uint64_t>((uint64_t)I->grid, (P.n + tb - 1) / tb);
     cudaEvent_t e3[3] = {nullptr, nullptr, nullptr};
     if (evs) { for (auto &e : e3) { CU(cudaEventCreate(&e)); evs->push_back(e); } CU(cudaEventRecord(e3[0], st)); }
-    CU(cudaLaunchKernel((const void *)ka, dim3(grid_a), dim3((unsigned)I->threads_a), args, I->smem_a, st));
+    CU(cudaLaunchKernel((const void *)ka, dim3(grid_a), dim3((unsigned)ta), args, smem_a, st));
     if (evs) CU(cudaEventRecord(e3[1], st));
-    CU(cudaLaunchKernel((const void *)kc, dim3(grid_c), dim3((unsigned)I->threads_c), args, I->smem_c, st));
+    CU(cudaLaunchKernel((const void *)kb, dim3(grid_b), dim3((unsigned)tb), args, smem_b, st));
     if (evs) CU(cudaEventRecord(e3[2], st));
     I->launches.fetch_add(2);
   }
@@ -501,13 +598,13 @@ int lgx_instance_query(const lgx_instance *I, int what, int64_t *out)
     case 0: *out = (int64_t)I->hdr.image_bytes + I->hdr.imagec_bytes; break;
     case 1: *out = I->threads_a; break;
     case 2: *out = I->grid; break;
-    case 3: *out = (int64_t)I->smem_a; break;
+    case 3: *out = (int64_t)I->hdr.image_bytes + (int64_t)I->a_state * I->threads_a; break;
     case 4: *out = I->hdr.coords; break;
-    case 5: *out = 8ll * I->hdr.a64_rows + 4ll * I->hdr.a32_rows; break;
+    case 5: *out = (int64_t)I->a_state; break;
     case 6: *out = I->sm_count; break;
     case 7: *out = I->launches.load(); break;
-    case 8: *out = I->threads_c; break;
-    case 9: *out = (int64_t)I->smem_c; break;
+    case 8: *out = I->threads_b; break;
+    case 9: *out = (int64_t)I->hdr.imagec_bytes + (int64_t)I->b_state * I->threads_b; break;
     case 10: *out = (int64_t)I->chunk; break;
     case 11: *out = 4ll * I->hdr.rec_words; break;
     case 12: *out = I->ns_a.load(); break;
@@ -515,6 +612,10 @@ int lgx_instance_query(const lgx_instance *I, int what, int64_t *out)
     case 14: *out = I->timed_pairs.load(); break;
     case 15: *out = I->threads_mv; break;
     case 16: *out = (int64_t)I->smem_mv; break;
+    case 17: *out = I->hdr.sq_shift; break;
+    case 18: *out = I->threads_a_dec; break;
+    case 19: *out = (int64_t)I->b_state; break;
+    case 20: *out = I->device; break;
     default: return LGX_EINVAL;
   }
   return LGX_OK;
@@ -533,16 +634,18 @@ int lgx_eval_batch(const lgx_instance *I, uint64_t seed, const uint64_t *d_ids, 
 {
   if (!I) return LGX_EINVAL;
   if (n == 0) return LGX_OK;
+  int rc = check_device(I);
+  if (rc != LGX_OK) return rc;
   cudaStream_t st = (cudaStream_t)stream;
   KParams P{};
   fill_round_keys(P, seed);
   P.ids = d_ids; P.first_id = first_id;
   P.cost = d_cost; P.path_km = d_path_km; P.makespan_h = d_makespan_h; P.feasible = d_feasible;
-  KernelFn ka, kc; pick_kernels<MODE_EVAL>(I->hdr, ka, kc);
+  KernelFn ka, kb; pick_kernels<MODE_EVAL>(I->hdr, ka, kb);
   Workspace W;
-  int rc = ws_alloc(I, n, false, st, W);
+  rc = ws_alloc(I, n, false, st, W);
   if (rc != LGX_OK) return rc;
-  rc = run_chunks(I, ka, kc, P, n, W, st);
+  rc = run_chunks(I, ka, kb, P, n, W, st, false);
   cudaFreeAsync(W.base, st);
   return rc;
 }
@@ -553,17 +656,19 @@ int lgx_decode_batch(const lgx_instance *I, uint64_t seed, const uint64_t *d_ids
 {
   if (!I) return LGX_EINVAL;
   if (n == 0) return LGX_OK;
+  int rc = check_device(I);
+  if (rc != LGX_OK) return rc;
   cudaStream_t st = (cudaStream_t)stream;
   KParams P{};
   fill_round_keys(P, seed);
   P.ids = d_ids; P.first_id = first_id;
   P.bp_tour = d_bp_tour; P.bp_pos = d_bp_pos; P.field_bp = d_field_bp; P.field_pos = d_field_pos;
   P.hu_tour = d_hu_tour; P.su_init = d_su_tour_init; P.su_final = d_su_tour_final;
-  KernelFn ka, kc; pick_kernels<MODE_DECODE>(I->hdr, ka, kc);
+  KernelFn ka, kb; pick_kernels<MODE_DECODE>(I->hdr, ka, kb);
   Workspace W;
-  int rc = ws_alloc(I, n, false, st, W);
+  rc = ws_alloc(I, n, false, st, W);
   if (rc != LGX_OK) return rc;
-  rc = run_chunks(I, ka, kc, P, n, W, st);
+  rc = run_chunks(I, ka, kb, P, n, W, st, true);
   cudaFreeAsync(W.base, st);
   return rc;
 }
@@ -572,17 +677,19 @@ int lgx_search_range(const lgx_instance *I, uint64_t seed, uint64_t first_id, ui
                      double *h_best_cost, uint64_t *h_best_id, void *stream)
 {
   if (!I || !h_best_cost || !h_best_id || n == 0) return LGX_EINVAL;
+  int rc = check_device(I);
+  if (rc != LGX_OK) return rc;
   cudaStream_t st = (cudaStream_t)stream;
   KParams P{};
   fill_round_keys(P, seed);
   P.ids = nullptr; P.first_id = first_id;
-  KernelFn ka, kc; pick_kernels<MODE_SEARCH>(I->hdr, ka, kc);
+  KernelFn ka, kb; pick_kernels<MODE_SEARCH>(I->hdr, ka, kb);
   Workspace W;
-  int rc = ws_alloc(I, n, true, st, W);
+  rc = ws_alloc(I, n, true, st, W);
   if (rc != LGX_OK) return rc;
   std::vector<cudaEvent_t> evs;
   const bool timed = I->timing.load() != 0;
-  rc = run_chunks(I, ka, kc, P, n, W, st, timed ? &evs : nullptr);
+  rc = run_chunks(I, ka, kb, P, n, W, st, false, timed ? &evs : nullptr);
   unsigned long long res[2] = {0, 0};
   if (rc == LGX_OK) {
     cudaError_t e = cudaMemcpyAsync(res, W.result, sizeof res, cudaMemcpyDeviceToHost, st);
@@ -619,9 +726,10 @@ int lgx_eval_batch_host(const lgx_instance *I, uint64_t seed, const uint64_t *h_
 {
   if (!I) return LGX_EINVAL;
   if (n == 0) return LGX_OK;
+  int rc = check_device(I);
+  if (rc != LGX_OK) return rc;
   const uint64_t chunk = std::min<uint64_t>(n, 1ull << 22);
   uint64_t *d_ids = nullptr; double *d_c = nullptr, *d_p = nullptr, *d_m = nullptr; uint8_t *d_f = nullptr;
-  int rc = LGX_OK;
   cudaError_t e = cudaSuccess;
   auto cleanup = [&]() { cudaFree(d_ids); cudaFree(d_c); cudaFree(d_p); cudaFree(d_m); cudaFree(d_f); };
   if (h_ids && (e = cudaMalloc((void **)&d_ids, chunk * 8)) != cudaSuccess) { cleanup(); return cuda_fail(e, "cudaMalloc"); }
@@ -742,10 +850,12 @@ int lgx_init_plan(const lgx_instance *I, uint8_t *h_bp_tour, uint8_t *h_bp_pos, 
                   uint8_t *h_hu_tour, uint8_t *h_su_tour, void *stream)
 {
   if (!I || !h_bp_tour || !h_bp_pos || !h_field_bp || !h_field_pos || !h_hu_tour || !h_su_tour) return LGX_EINVAL;
+  int rc = check_device(I);
+  if (rc != LGX_OK) return rc;
   cudaStream_t st = (cudaStream_t)stream;
   const ImgHdr &H = I->hdr;
   PlanDev D;
-  int rc = plan_dev_alloc(H, st, D);
+  rc = plan_dev_alloc(H, st, D);
   if (rc != LGX_OK) return rc;
   const size_t nb = H.n_b, nf = H.n_f;
   const size_t scratch_bytes = 4 * (3 * nb + 1) + 2 * (nf + (nf & 1)) + 2 * nb + 16;
@@ -755,14 +865,16 @@ int lgx_init_plan(const lgx_instance *I, uint8_t *h_bp_tour, uint8_t *h_bp_pos, 
   InitParams P{};
   P.n_f = H.n_f; P.n_b = H.n_b; P.n_t = H.n_t; P.n_hu = H.n_hu; P.n_su = H.n_su;
   P.xy = I->d_xy;
-  P.sq = reinterpret_cast<const uint32_t *>(I->d_image_c + H.offc_s);
+  P.sh = reinterpret_cast<const uint2 *>(I->d_image_c + H.offc_sh);
   P.dq = reinterpret_cast<const uint32_t *>(I->d_image + H.off_dq);
   P.unit_of = I->d_image_c + H.offc_unit;
   P.bp_tour = D.bt; P.bp_pos = D.bq; P.field_bp = D.fb; P.field_pos = D.fq; P.hu_tour = D.hu; P.su_tour = D.su;
   P.scratch = scratch;
-  lgx_init_plan_k<<<1, 256, 0, st>>>(P);
+  {
+    void *args[] = { (void *)&P };
+    e = cudaLaunchKernel((const void *)lgx_init_plan_k, dim3(1), dim3(256), args, 0, st);
+  }
   I->launches.fetch_add(1);
-  e = cudaGetLastError();
   if (e == cudaSuccess) rc = plan_download(H, D, h_bp_tour, h_bp_pos, h_field_bp, h_field_pos, h_hu_tour, h_su_tour, st);
   if (e == cudaSuccess && rc == LGX_OK) e = cudaStreamSynchronize(st);
   cudaFreeAsync(scratch, st); cudaFreeAsync(D.base, st);
@@ -781,11 +893,13 @@ int lgx_move_eval_batch(const lgx_instance *I,
   if (!plan_valid(H, h_bp_tour, h_bp_pos, h_field_bp, h_field_pos, h_hu_tour, h_su_tour)) return LGX_EINVAL;
   if (I->threads_mv < 64) return LGX_ETOOBIG;
   if (n == 0) return LGX_OK;
+  int rc = check_device(I);
+  if (rc != LGX_OK) return rc;
   cudaStream_t st = (cudaStream_t)stream;
   MvKernelFn kb, ks; pick_move_kernels(H, kb, ks);
   if (!kb) return LGX_EINVAL;
   PlanDev D;
-  int rc = plan_dev_alloc(H, st, D);
+  rc = plan_dev_alloc(H, st, D);
   if (rc != LGX_OK) return rc;
   rc = plan_upload(H, D, h_bp_tour, h_bp_pos, h_field_bp, h_field_pos, h_hu_tour, h_su_tour, st);
   if (rc == LGX_OK) {
@@ -793,8 +907,8 @@ int lgx_move_eval_batch(const lgx_instance *I,
     mv_fill(I, P, seed, D);
     P.first_id = first_id; P.n = n;
     P.cost = d_cost; P.path_km = d_path_km; P.makespan_h = d_makespan_h; P.feasible = d_feasible;
-    cudaError_t e = cudaFuncSetAttribute((const void *)kb, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)I->smem_mv);
-    if (e == cudaSuccess) {
+    cudaError_t e = cudaSuccess;
+    {
       const uint64_t blocks = (n + (uint64_t)I->threads_mv - 1) / (uint64_t)I->threads_mv;
       const unsigned grid = (unsigned)std::min<uint64_t>((uint64_t)I->grid, blocks);
       void *args[] = { (void *)&P };
@@ -818,13 +932,14 @@ int lgx_local_search(const lgx_instance *I,
   const ImgHdr &H = I->hdr;
   if (!plan_valid(H, h_bp_tour, h_bp_pos, h_field_bp, h_field_pos, h_hu_tour, h_su_tour)) return LGX_EINVAL;
   if (I->threads_mv < 64) return LGX_ETOOBIG;
+  int rc = check_device(I);
+  if (rc != LGX_OK) return rc;
   cudaStream_t st = (cudaStream_t)stream;
   MvKernelFn kb, ks; pick_move_kernels(H, kb, ks);
   if (!ks) return LGX_EINVAL;
   int coop = 0;
   cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, I->device);
   if (!coop) { g_cuda_msg = "device does not support cooperative launches"; return LGX_ECUDA; }
-  CU(cudaFuncSetAttribute((const void *)ks, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)I->smem_mv));
   int per_sm = 0;
   CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void *)ks, I->threads_mv, I->smem_mv));
   if (per_sm < 1) return LGX_ETOOBIG;
@@ -832,7 +947,7 @@ int lgx_local_search(const lgx_instance *I,
   const uint64_t blocks = ((uint64_t)n_workers + (uint64_t)I->threads_mv - 1) / (uint64_t)I->threads_mv;
   const unsigned grid = (unsigned)std::min<uint64_t>((uint64_t)I->sm_count, blocks);
   PlanDev D;
-  int rc = plan_dev_alloc(H, st, D);
+  rc = plan_dev_alloc(H, st, D);
   if (rc != LGX_OK) return rc;
   uint8_t *ws = nullptr;
   const size_t slots_bytes = 2ull * grid * I->mv.slot_words * 8ull;

@@ -1,11 +1,13 @@
 // lgx_image.h — layout of the instance images that live in shared memory,
 // of the per-candidate state rows, and of the queue record that carries a feasible
-// candidate from the decode/walk kernel to the finish kernel.
+// candidate from the decode/cut kernel to the walk/finish kernel.
 // Product code (CUDA path).  Shares nothing with oracle/.
 //
-// Image AB (decode + pass 1):   distance tables or coordinates | {s_q,h_q} per field | demand quanta
-// Image C  (Alg. 2 + pass 2):   field x BP table or coordinates | s_q per field | HU rate quanta |
-//                               SU capacities by rank | RN(1/k) table | unit<->rank maps
+// Image A (lgx_decode_cut: decode + eq. (2), integers only):
+//     s_q per field (replicated 2^sq_shift times so that lanes read different banks) | demand quanta
+// Image C (lgx_walk_finish: geometry, Algorithm 2, shuttles, cost):
+//     distance tables and/or coordinates | {s_q, h_q} per field | SU capacities by rank | RN(1/k) table |
+//     unit <-> rank maps | HU rate quanta
 // Both are contiguous, 16-byte aligned blobs built on the host by lgx_instance_create and
 // copied global -> shared once per (persistent) block.
 //
@@ -18,6 +20,15 @@
 #pragma once
 #include <stdint.h>
 
+// Dynamic shared memory of a kernel.  (The host-side single-lane emulation used by the CPU checks of the
+// kernel logic predefines this macro; the CUDA build always takes the declaration below.)
+#ifndef LGX_DYN_SMEM
+#define LGX_DYN_SMEM(name) extern __shared__ __align__(16) uint8_t name[]
+#endif
+#ifndef LGX_LANES
+#define LGX_LANES 32u            // lanes that draw work together (a warp)
+#endif
+
 namespace lgx {
 
 constexpr int      kQ           = 1024;          // quanta per t / ha / (ha/h)   (R18)
@@ -26,9 +37,9 @@ constexpr uint32_t kPhiloxM1    = 0xCD9E8D57u;
 constexpr uint32_t kPhiloxW0    = 0x9E3779B9u;   // key increments
 constexpr uint32_t kPhiloxW1    = 0xBB67AE85u;
 constexpr int      kMaxSmem     = 227 * 1024;    // opt-in dynamic shared memory per block, sm_100a
-constexpr int      kMaxThreads  = 512;           // __launch_bounds__ of the finish kernel
-constexpr int      kMaxThreadsA = 640;           // __launch_bounds__ of the decode/walk kernel (<= 96 registers)
-constexpr int      kFinishBlocksPerSM = 2;       // the finish kernel's image is small: two blocks share an SM
+constexpr int      kMaxThreadsA = 1024;          // __launch_bounds__ of the decode/cut kernel (<= 64 registers)
+constexpr int      kMaxThreadsB = 512;           // __launch_bounds__ of the walk/finish kernel (<= 128 registers)
+constexpr uint32_t kLanes       = LGX_LANES;
 
 struct ImgHdr {
   int32_t  n_f, n_b, n_hu, n_su, n_t;
@@ -40,37 +51,41 @@ struct ImgHdr {
   uint32_t n_extra_blocks;  // Philox blocks of stream 4 drawn up front (<= 16)
   uint32_t perm_pad;        // right-alignment of the permutation array inside its words
   uint32_t perm_w0;         // initial value of permutation word 0 (bytes below perm_pad unused)
+  uint32_t sq_shift;        // log2 of the replication factor of image A's s_q table
+  uint32_t zero_demand;     // some BP has zero demand: one field step may close several BPs (R21)
 
-  // ---- image AB (byte offsets)
-  uint32_t off_dtri;        // f64 [(n_f+1) n_f / 2]  strict lower triangle over {HQ, fields}
-  uint32_t off_dfb;         // f64 [n_f][n_b]         field -> BP legs
-  uint32_t off_xy;          // f64x2 [1 + n_b + n_f]  vertex coordinates (coords mode)
-  uint32_t off_sh;          // u32x2 [n_f]            {s_q, h_q}
+  // ---- image A (byte offsets)
+  uint32_t off_sq;          // u32 [n_f << sq_shift]  s_q; field f, replica r at (f << sq_shift) + r
   uint32_t off_dq;          // u32 [n_b]              demand quanta
   uint32_t image_bytes;
 
   // ---- image C (byte offsets inside image C)
-  uint32_t offc_dfb, offc_xy, offc_s, offc_cs, offc_rcp, offc_unit;
+  uint32_t offc_dtri;       // f64 [(n_f+1) n_f / 2]  strict lower triangle over {HQ, fields}      (mode 0)
+  uint32_t offc_dfb;        // f64 [n_f][n_b]         field -> BP legs                              (modes 0, 2)
+  uint32_t offc_xy;         // f64x2 [1 + n_b + n_f]  vertex coordinates                            (modes 1, 2)
+  uint32_t offc_sh;         // u32x2 [n_f]            {s_q, h_q}
+  uint32_t offc_cs;         // u32 [n_su]  SU capacity quanta by rank (ascending (capacity, unit)); the move kernels copy image C from here on
+  uint32_t offc_rcp;        // f64 [..]    RN(1/k)
+  uint32_t offc_unit;       // u8  [n_su]  rank -> SU
   uint32_t offc_rq;         // u32 [n_hu]  HU rate quanta
-  uint32_t offc_rank;       // u8  [n_su]  unit -> rank
+  uint32_t offc_rank;       // u8  [n_su]  SU -> rank
   uint32_t offc_hrs;        // u32 [n_hu]  HU rate quanta by rank (ascending (rate, unit)): the embedded HU assignment (N2)
   uint32_t offc_hunit;      // u8  [n_hu]  rank -> HU
   uint32_t offc_hrank;      // u8  [n_hu]  HU -> rank
-  uint32_t flags;           // lgx_instance_desc.flags (bit 1: Algorithm 1's workers embed the HU assignment)
+  uint32_t flags;           // lgx_instance_desc.flags
   uint32_t imagec_bytes;
 
-  // ---- state rows of the decode/walk kernel
-  uint32_t a64_sd, a64_lt, a64_ent, a64_rows;
-  uint32_t a32_perm, a32_bpseq, a32_segend, a32_scra, a32_scrb, a32_hq, a32_rows;
+  // ---- state rows of the decode/cut kernel (32-bit rows only)
+  uint32_t a32_perm, a32_bpseq, a32_ds, a32_scra, a32_scrb, a32_cnt, a32_rows;
+  uint32_t a32_scru, a32_rows_dec;      // diagnostic decode mode: scratch of the unit partitions, appended
 
-  // ---- state rows of the finish kernel
-  uint32_t c64_w, c64_e, c64_mask, c64_rows;
-  uint32_t c32_s, c32_nhu, c32_r, c32_ng, c32_magic, c32_ent, c32_scra, c32_rows;
+  // ---- state rows of the walk/finish kernel
+  uint32_t c64_w, c64_e, c64_mask, c64_sd, c64_rows;
+  uint32_t c32_s, c32_nhu, c32_r, c32_ng, c32_magic, c32_hq, c32_ent, c32_rows;
 
   // ---- queue record (32-bit words, stored transposed: word w of slot q at queue[w*cap + q])
-  //   0,1 index i | per tour g at rec_tour + g*rec_tw: LT lo,hi, H_q |
-  //   SD[j] lo,hi at rec_sd + 2j | bpseq words | segend words | perm words
-  uint32_t rec_tour, rec_tw, rec_sd, rec_bpseq, rec_segend, rec_perm, rec_words;
+  //   0,1 index i | bpseq words | segend words | perm words
+  uint32_t rec_bpseq, rec_segend, rec_perm, rec_words;
   uint32_t n_bpseq_words, n_segend_words, n_perm_words;
   uint32_t pad_[2];
 };

@@ -198,7 +198,7 @@ __device__ void mv_encode(const MvParams &P, uint8_t *sm, const uint8_t *plan, u
   __syncthreads();
   uint4 *pos4 = MV_TAB(uint4, M.off_pos4);
   uint16_t *posf = MV_TAB(uint16_t, M.off_posf);
-  const uint2 *sh = reinterpret_cast<const uint2 *>(P.image + H.off_sh);     // {s_q, h_q} per field (global, L2-resident)
+  const uint2 *sh = reinterpret_cast<const uint2 *>(P.image_c + H.offc_sh);  // {s_q, h_q} per field (global, L2-resident)
   for (uint32_t f = tid; f < n_f; f += T) {
     const uint32_t b = p_fb[f];
     const uint2 bb = bp[b];
@@ -866,7 +866,7 @@ __device__ __forceinline__ void mv_for_workers(const MvParams &P, uint8_t *sm, u
 template <int MASKW, bool HB>
 __global__ void __launch_bounds__(kMvThreads, 1) lgx_move_eval_k(const __grid_constant__ MvParams P)
 {
-  extern __shared__ __align__(16) uint8_t smem[];
+  LGX_DYN_SMEM(smem);
   uint8_t *sm = smem;
   const uint32_t tid = threadIdx.x, T = blockDim.x;
   St s;
@@ -901,7 +901,7 @@ __global__ void __launch_bounds__(kMvThreads, 1) lgx_move_eval_k(const __grid_co
 template <int MASKW, bool HB>
 __global__ void __launch_bounds__(kMvThreads, 1) lgx_local_search_k(const __grid_constant__ MvParams P)
 {
-  extern __shared__ __align__(16) uint8_t smem[];
+  LGX_DYN_SMEM(smem);
   uint8_t *sm = smem;
   cg::grid_group grid = cg::this_grid();
   const ImgHdr &H = P.H; const MvHdr &M = P.M;
@@ -1093,7 +1093,8 @@ __global__ void __launch_bounds__(kMvThreads, 1) lgx_local_search_k(const __grid
 struct InitParams {
   int32_t n_f, n_b, n_t, n_hu, n_su;
   const double2  *xy;        // [1 + n_b + n_f] vertex coordinates: HQ, BPs, fields
-  const uint32_t *sq, *dq;   // supply / demand quanta
+  const uint2    *sh;        // {s_q, h_q} per field
+  const uint32_t *dq;        // demand quanta
   const uint8_t  *unit_of;   // SU of capacity rank r (ascending (capacity, unit))
   uint8_t *bp_tour, *bp_pos; uint16_t *field_bp, *field_pos; uint8_t *hu_tour, *su_tour;
   uint32_t *scratch;         // [n_b] supplies | [n_b + 1] list offsets | [n_b] cursors | u16 [n_f] lists | u8 [n_b] chain, flags
@@ -1152,7 +1153,7 @@ __global__ void __launch_bounds__(256, 1) lgx_init_plan_k(const InitParams P)
       }
       warp_argmin(bd, best);
       if (best == kNone) { warp_argmin(ad, any); best = any; }
-      if (lane == 0u) { P.field_bp[f] = (uint16_t)best; Sq[best] += P.sq[f]; }
+      if (lane == 0u) { P.field_bp[f] = (uint16_t)best; Sq[best] += P.sh[f].x; }
       __syncwarp();
     }
   }

@@ -61,11 +61,38 @@ def test_create_validation_codes():
     assert _create(i) == binding.LGX_ETOOBIG
     i = toy(); i.bp_demand_t[0] = 5e6               # d_q >= 2^32
     assert _create(i) == binding.LGX_ETOOBIG
+    assert _create(toy(flags=binding.LGX_FLAG_DIST_COORDS | binding.LGX_FLAG_DIST_MIXED)) == binding.LGX_EINVAL
+    assert _create(toy(flags=64)) == binding.LGX_EINVAL
     # a valid instance reaches the device step: OK on a GPU box, LGX_ECUDA (never a CPU
     # fallback) without one
     import torch
     rc = _create(toy())
     assert rc == (binding.LGX_OK if torch.cuda.is_available() else binding.LGX_ECUDA)
+
+
+def _sized(n_f, n_b, n_hu, n_su, n_t):
+    rng = np.random.default_rng(5)
+    fields = [(rng.uniform(0, 50), rng.uniform(0, 50), 10.0, 1.0) for _ in range(n_f)]
+    bps = [(rng.uniform(0, 50), rng.uniform(0, 50), 1.0) for _ in range(n_b)]
+    return mk_instance((0, 0), fields, bps, [2.0] * n_hu, [10.0] * n_su, n_t)
+
+
+def test_documented_limits_return_documented_codes():
+    """include/lgx.h: counts above 65535 fields / 255 BPs, tours, HUs, SUs are LGX_EINVAL; N_B > LGX_MAX_BPS and
+    N_SU > LGX_MAX_SUS are LGX_ETOOBIG (kernel limits of this build); at the limits creation reaches the device step."""
+    import torch
+    hdr = open(os.path.join(ROOT, "include", "lgx.h")).read()
+    lim = {k: int(v) for k, v in re.findall(r"#define (LGX_MAX_[A-Z_]+)\s+(\d+)", hdr)}
+    assert lim == dict(LGX_MAX_BPS=binding.LGX_MAX_BPS, LGX_MAX_SUS=binding.LGX_MAX_SUS,
+                       LGX_MAX_MOVE_TOURS=binding.LGX_MAX_MOVE_TOURS, LGX_MAX_MOVE_HUS=binding.LGX_MAX_MOVE_HUS)
+    assert _create(_sized(300, 256, 4, 4, 2)) == binding.LGX_EINVAL
+    assert _create(_sized(300, 8, 256, 4, 2)) == binding.LGX_EINVAL
+    assert _create(_sized(300, 8, 4, 256, 2)) == binding.LGX_EINVAL
+    assert _create(_sized(300, binding.LGX_MAX_BPS + 1, 4, 4, 2)) == binding.LGX_ETOOBIG
+    assert _create(_sized(300, 8, 4, binding.LGX_MAX_SUS + 1, 2)) == binding.LGX_ETOOBIG
+    ok = binding.LGX_OK if torch.cuda.is_available() else binding.LGX_ECUDA
+    assert _create(_sized(300, binding.LGX_MAX_BPS, 4, 4, 2)) == ok
+    assert _create(_sized(300, 8, 4, binding.LGX_MAX_SUS, 2)) == ok
 
 
 def test_null_arguments():

@@ -285,16 +285,16 @@ def test_fixed_field_bp_assignment_matches_oracle(name, flags):
     g.close()
 
 
-def test_results_do_not_depend_on_the_launch_shape(ctxs, monkeypatch):
+def test_results_do_not_depend_on_the_launch_shape(ctxs):
     """Which thread scores which worker is free (sorted rounds, warps drawing chunks): the winners must not depend on it."""
     inst, o, g = ctxs("medium")
     p0 = o.init_plan()
     ref = g.local_search(p0, 9, 15, 20000, 0x66666666)
     refb = g.move_eval_batch(p0, 9, 0, 50000)[0].cpu().numpy()
-    for threads in ("64", "160", "384"):
-        monkeypatch.setenv("LGX_THREADS_MV", threads)
+    for threads in (64, 160, 384):
         g2 = binding.Instance(inst)
-        assert g2.query(15) == int(threads)
+        g2.set_option(binding.LGX_OPT_THREADS_MV, threads)
+        assert g2.query(15) == threads
         got = g2.local_search(p0, 9, 15, 20000, 0x66666666)
         assert got[1] == ref[1] and np.array_equal(got[3], ref[3]) and np.array_equal(got[2], ref[2])
         assert_plan_equal(got[0], ref[0], f"threads {threads}")
