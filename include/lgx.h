@@ -96,8 +96,8 @@ typedef struct {
  * distance tables or coordinates and the unit tables for the walk/finish kernel) and uploads them.
  * Errors: LGX_EINVAL (null pointer, n_tours out of range, non-finite or negative input, zero
  * rate/capacity/velocity, counts above 65535 fields / 255 BPs, tours, HUs, SUs, unknown flag bits),
- * LGX_ETOOBIG (integer ranges: max s_q*N_SU + sum c_q, sum s_q, sum h_q, sum r_q, d_q must
- * stay below 2^32; N_B > LGX_MAX_BPS or N_SU > LGX_MAX_SUS; or the per-candidate state does not fit in
+ * LGX_ETOOBIG (integer ranges: max s_q*N_SU + sum c_q, sum h_q, sum r_q, d_q must stay below 2^32
+ * and sum s_q below 2^32 - 1; N_B > LGX_MAX_BPS or N_SU > LGX_MAX_SUS; or the per-candidate state does not fit in
  * 227 KB of shared memory), LGX_ECUDA, LGX_ENOMEM.                                          */
 int lgx_instance_create (const lgx_instance_desc *desc, lgx_instance **out);
 int lgx_instance_destroy(lgx_instance *inst);
@@ -214,6 +214,13 @@ int lgx_local_search(const lgx_instance *inst,
                      uint8_t *h_hu_tour, uint8_t *h_su_tour,
                      uint64_t seed, uint32_t n_iters, uint32_t n_workers, uint32_t eps_thresh,
                      double *h_best_cost, double *h_hist_cost, uint64_t *h_hist_id, void *cuda_stream);
+
+/* Diagnostic self-test of a device routine against its library counterpart, on the current device's default stream
+ * (synchronous).  what = 0: the in-line correctly rounded square root of the walk/finish kernel against __dsqrt_rn
+ * on n pseudo-random arguments drawn from `seed` (squared coordinate differences, random mantissas over 120 binades,
+ * exact squares and their neighbours); h_out[0] = arguments checked, h_out[1] = mismatches (must be 0).
+ * Other `what`, n == 0 or a null pointer => LGX_EINVAL.                                                         */
+int lgx_selftest(int what, uint64_t n, uint64_t seed, uint64_t *h_out);
 
 const char *lgx_strerror(int code);
 

@@ -40,7 +40,7 @@ class lgx_instance_desc(C.Structure):
 
 EXPORTS = ("lgx_instance_create", "lgx_instance_destroy", "lgx_eval_batch", "lgx_eval_batch_host",
            "lgx_search_range", "lgx_search", "lgx_decode_batch", "lgx_instance_query", "lgx_instance_set_timing",
-           "lgx_instance_set_option",
+           "lgx_instance_set_option", "lgx_selftest",
            "lgx_init_plan", "lgx_move_eval_batch", "lgx_local_search", "lgx_strerror")
 
 _lib = None
@@ -67,6 +67,7 @@ def load(rebuild_if_stale: bool = True):
     lib.lgx_instance_query.argtypes = [vp, i32, C.POINTER(C.c_int64)]
     lib.lgx_instance_set_timing.argtypes = [vp, i32]
     lib.lgx_instance_set_option.argtypes = [vp, i32, C.c_int64]
+    lib.lgx_selftest.argtypes = [i32, u64, u64, C.POINTER(u64)]
     lib.lgx_init_plan.argtypes = [vp] + [vp] * 6 + [vp]
     lib.lgx_move_eval_batch.argtypes = [vp] + [vp] * 6 + [u64, u64, u64, vp, vp, vp, vp, vp]
     lib.lgx_local_search.argtypes = [vp] + [vp] * 6 + [u64, C.c_uint32, C.c_uint32, C.c_uint32,
@@ -134,6 +135,13 @@ PLAN_KEYS = (("bp_tour", np.uint8), ("bp_pos", np.uint8), ("field_bp", np.uint16
 def _plan_arrays(plan):
     """The six host arrays of a plan (copies, contiguous, typed) in the C ABI's order."""
     return [np.array(plan[k], dtype=dt, order="C", copy=True) for k, dt in PLAN_KEYS]
+
+
+def selftest(what: int, n: int, seed: int = 0):
+    """lgx_selftest: (arguments checked, mismatches) of a device routine against its library counterpart."""
+    out = (C.c_uint64 * 2)()
+    _check(load().lgx_selftest(what, n, seed, out))
+    return int(out[0]), int(out[1])
 
 
 class Instance:

@@ -73,8 +73,12 @@ using KernelFn = void (*)(const KParams);
 template <int MODE> void pick_kernels(const ImgHdr &h, KernelFn &ka, KernelFn &kb)
 {
   const bool p16 = h.perm16 != 0; const int dm = h.coords, mw = (int)h.mask_words;
-  ka = p16 ? lgx_decode_cut<true, MODE> : lgx_decode_cut<false, MODE>;
-  kb = nullptr;
+  const bool zd = h.zero_demand != 0u, x64 = h.n_extra_blocks > 7u;
+  ka = nullptr; kb = nullptr;
+#define LGX_PICK_A(P, Z, X) if (p16 == P && zd == Z && x64 == X) ka = lgx_decode_cut<P, Z, X, MODE>;
+  LGX_PICK_A(false, false, false) LGX_PICK_A(false, false, true) LGX_PICK_A(false, true, false) LGX_PICK_A(false, true, true)
+  LGX_PICK_A(true,  false, false) LGX_PICK_A(true,  false, true) LGX_PICK_A(true,  true, false) LGX_PICK_A(true,  true, true)
+#undef LGX_PICK_A
 #define LGX_PICK(P, D, M) if (p16 == P && dm == D && mw == M) kb = lgx_walk_finish<P, D, M, MODE>;
   LGX_PICK(false, 0, 1) LGX_PICK(false, 0, 2) LGX_PICK(false, 1, 1) LGX_PICK(false, 1, 2) LGX_PICK(false, 2, 1) LGX_PICK(false, 2, 2)
   LGX_PICK(true,  0, 1) LGX_PICK(true,  0, 2) LGX_PICK(true,  1, 1) LGX_PICK(true,  1, 2) LGX_PICK(true,  2, 1) LGX_PICK(true,  2, 2)
@@ -139,7 +143,9 @@ void free_instance(lgx_instance *I)
 // instances of different sizes cannot race on it.
 int allow_max_smem(const void *fn, int smem_optin)
 {
-  CU(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, std::min(smem_optin, kMaxSmem)));
+  cudaFuncAttributes fa{};
+  CU(cudaFuncGetAttributes(&fa, fn));                      // the kernel's static shared memory counts against the limit
+  CU(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, std::min(smem_optin, kMaxSmem) - (int)fa.sharedSizeBytes));
   return LGX_OK;
 }
 
@@ -200,7 +206,8 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   for (int u = 0; u < nhu; ++u) { r_q[u] = quantise(d->hu_rate_ha_per_h[u]); if (r_q[u] <= 0) return LGX_EINVAL; r_sum += r_q[u]; }
   for (int u = 0; u < nsu; ++u) { c_q[u] = quantise(d->su_capacity_t[u]); if (c_q[u] <= 0) return LGX_EINVAL; c_sum += c_q[u]; }
   const int64_t lim = (int64_t)1 << 32;
-  if (s_max * (int64_t)nsu + c_sum >= lim || s_sum >= lim || h_sum >= lim || r_sum >= lim) return LGX_ETOOBIG;
+  // (sum s_q stays below 2^32 - 1: the decode/cut kernel marks the last BP of a plan with the demand 2^32 - 1)
+  if (s_max * (int64_t)nsu + c_sum >= lim || s_sum >= lim - 1 || h_sum >= lim || r_sum >= lim) return LGX_ETOOBIG;
   for (int b = 0; b < nb; ++b) if (d_q[b] >= lim) return LGX_ETOOBIG;
   // kernel limits of this build (include/lgx.h): 7-bit BP ids in the plan entries, SU sets of 2 x 64 bits
   if (nb > LGX_MAX_BPS || nsu > LGX_MAX_SUS) return LGX_ETOOBIG;
@@ -216,8 +223,8 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   H.perm16 = nf > 255 ? 1 : 0;
   H.mask_words = nsu > 64 ? 2u : 1u;
   const uint32_t MW = H.mask_words;
-  // stream-4 draws taken up front: (N_B-1) failures + geometric extras, with slack; <= 64
-  H.n_extra_blocks = (uint32_t)std::min(16, ((nb - 1) * 4 / 3 + 8 + 3) / 4);
+  // stream-4 draws taken up front: (N_B-1) failures + geometric extras, with slack; <= 60 (+ a sentinel bit)
+  H.n_extra_blocks = (uint32_t)std::min(15, ((nb - 1) * 4 / 3 + 8 + 3) / 4);
   I->s_q.resize(nf); I->d_q.resize(nb);
   for (int f = 0; f < nf; ++f) I->s_q[f] = (uint32_t)s_q[f];
   H.zero_demand = 0u;
@@ -253,22 +260,24 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
     H.a32_scru = r;  r += (n_units + 3u) / 4u + 1u;        // diagnostic decode mode only: unit partitions
     H.a32_rows_dec = r;
   }
-  // ---- state rows of the walk/finish kernel
+  // ---- state rows of the walk/finish kernel.  Rows are reused as their contents die (lgx_kernels.cuh): one block of
+  //      64-bit rows holds SD per plan BP, then T_wait(g) | the walk's tour parameters; the 32-bit rows of H_q(g) and of
+  //      the walk entries are the unit partitions' scratch before (a thread only ever aliases its OWN cells: warps of a
+  //      block are in different phases).
   {
+    const uint32_t scratch_rows = (n_units + 3u) / 4u + 1u;
+    const uint32_t blk = std::max((uint32_t)nb, 2u * (uint32_t)nt);
     uint32_t r = 0;
-    H.c64_w = r; r += (uint32_t)nt;                        // T_wait(g); then the shuttle sum
-    H.c64_e = r; r += (uint32_t)nt;                        // E(g)
+    H.c64_w = r; H.c64_sd = r; H.c64_tp = r + (uint32_t)nt; r += blk;
+    H.c64_e = r; r += (uint32_t)nt;                        // sumE(g), E(g); then L_tour(g)
     H.c64_mask = r; r += (uint32_t)nt * MW;
-    H.c64_sd = r; r += (uint32_t)nb;                       // SD per plan BP with fields; then L_tour(g) (N_T <= N_B)
     H.c64_rows = r;
     r = 0;
     H.c32_s = r; r += (uint32_t)nt;
-    H.c32_nhu = r; r += (uint32_t)nt;
+    H.c32_hn = r; r += (uint32_t)nt;                       // n_HU(g) | n_SU(g) << 8 | m(g) << 16
     H.c32_r = r; r += (uint32_t)nt;
-    H.c32_ng = r; r += (uint32_t)nt;
-    H.c32_magic = r; r += (uint32_t)nt;
-    H.c32_hq = r; r += (uint32_t)nt;
-    H.c32_ent = r; r += std::max((uint32_t)nb + 1u, (n_units + 3u) / 4u + 1u);   // walk entries + sentinel; partition scratch before
+    H.c32_hq = r; H.c32_ent = r + (uint32_t)nt;            // H_q(g); walk entries + sentinel
+    r += std::max((uint32_t)nt + (uint32_t)nb + 1u, scratch_rows);
     H.c32_rows = r;
   }
   // ---- queue record
@@ -288,7 +297,7 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   const uint64_t tri_bytes = (uint64_t)(nf + 1) * (uint64_t)nf / 2 * 8, dfb_bytes = (uint64_t)nf * nb * 8;
   const uint64_t xy_bytes = 16ull * (1 + nb + nf), room = (uint64_t)kMaxSmem - 1024;
   const int n_rcp = std::max(nf, std::max(nb, nhu)) + 1;
-  const uint64_t tail_bytes = 8ull * nf + 4ull * nsu + 8ull * n_rcp + 2ull * nsu + 8ull * nhu + 2ull * nhu + 256;
+  const uint64_t tail_bytes = 8ull * nf + 8ull * nf + 6ull * nsu + 8ull * n_rcp + 2ull * nsu + 8ull * nhu + 2ull * nhu + 320;
   if (tail_bytes + tri_bytes + dfb_bytes + 256ull * I->b_state <= room) H.coords = 0;
   else if (dfb_bytes <= 32ull * 1024 && tail_bytes + dfb_bytes + xy_bytes + 128ull * I->b_state <= room) H.coords = 2;
   else H.coords = 1;
@@ -299,7 +308,10 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   if (H.coords == 0) { H.offc_dtri = off; off = align16(off + (uint32_t)tri_bytes); }
   if (H.coords != 1) { H.offc_dfb = off; off = align16(off + (uint32_t)dfb_bytes); }
   if (H.coords != 0) { H.offc_xy = off; off = align16(off + (uint32_t)xy_bytes); }
+  H.offc_dhq = 0;
+  if (H.coords != 0) { H.offc_dhq = off; off = align16(off + 8u * (uint32_t)nf); }
   H.offc_sh   = off; off = align16(off + 8u * (uint32_t)nf);
+  H.offc_suinit = off; off = align16(off + 4u * (((uint32_t)nsu + 3u) / 4u));
   H.offc_cs   = off; off = align16(off + 4u * (uint32_t)nsu);
   H.offc_rcp  = off; off = align16(off + 8u * (uint32_t)n_rcp);
   H.offc_unit = off; off = align16(off + (uint32_t)nsu);
@@ -332,7 +344,11 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   xyv[0] = d->hq_x; xyv[1] = d->hq_y;
   for (int b = 0; b < nb; ++b) { xyv[2 * (1 + b)] = d->bp_x[b]; xyv[2 * (1 + b) + 1] = d->bp_y[b]; }
   for (int f = 0; f < nf; ++f) { xyv[2 * (1 + nb + f)] = d->field_x[f]; xyv[2 * (1 + nb + f) + 1] = d->field_y[f]; }
-  if (H.coords != 0) std::memcpy(imc + H.offc_xy, xyv.data(), xyv.size() * 8);
+  if (H.coords != 0) {
+    std::memcpy(imc + H.offc_xy, xyv.data(), xyv.size() * 8);
+    double *dh = reinterpret_cast<double *>(imc + H.offc_dhq);
+    for (int f = 0; f < nf; ++f) dh[f] = edge(d->field_x[f], d->field_y[f], d->hq_x, d->hq_y);
+  }
   uint32_t *shc = reinterpret_cast<uint32_t *>(imc + H.offc_sh);
   for (int f = 0; f < nf; ++f) { shc[2 * f] = (uint32_t)s_q[f]; shc[2 * f + 1] = (uint32_t)h_q[f]; }
   uint32_t *rq = reinterpret_cast<uint32_t *>(imc + H.offc_rq);
@@ -345,6 +361,10 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   for (int r = 0; r < nsu; ++r) {
     cc[r] = (uint32_t)c_q[order[r]];
     imc[H.offc_unit + r] = (uint8_t)order[r]; imc[H.offc_rank + order[r]] = (uint8_t)r;
+  }
+  {   // initial Fisher-Yates array of the SU partition: element i (byte i + pad of the right-aligned words) = rank of unit i
+    const uint32_t padu = (4u - ((uint32_t)nsu & 3u)) & 3u;
+    for (int u = 0; u < nsu; ++u) imc[H.offc_suinit + (uint32_t)u + padu] = imc[H.offc_rank + u];
   }
   {   // HUs ascending by (rate quanta, unit index): "sorted according to rising in-field working rates"
     std::vector<int> ho(nhu);
@@ -618,6 +638,24 @@ int lgx_instance_query(const lgx_instance *I, int what, int64_t *out)
     case 20: *out = I->device; break;
     default: return LGX_EINVAL;
   }
+  return LGX_OK;
+}
+
+int lgx_selftest(int what, uint64_t n, uint64_t seed, uint64_t *h_out)
+{
+  if (what != 0 || !h_out || n == 0) return LGX_EINVAL;
+  unsigned long long *d = nullptr;
+  CU(cudaMalloc((void **)&d, 16));
+  cudaError_t e = cudaMemset(d, 0, 16);
+  if (e == cudaSuccess) {
+    void *args[] = { (void *)&n, (void *)&seed, (void *)&d };
+    e = cudaLaunchKernel((const void *)lgx_selftest_sqrt_k, dim3(592), dim3(256), args, 0, nullptr);
+  }
+  unsigned long long r[2] = {0, 0};
+  if (e == cudaSuccess) e = cudaMemcpy(r, d, 16, cudaMemcpyDeviceToHost);
+  cudaFree(d);
+  if (e != cudaSuccess) return cuda_fail(e, "lgx_selftest");
+  h_out[0] = r[0]; h_out[1] = r[1];
   return LGX_OK;
 }
 

@@ -38,7 +38,7 @@ constexpr uint32_t kPhiloxW0    = 0x9E3779B9u;   // key increments
 constexpr uint32_t kPhiloxW1    = 0xBB67AE85u;
 constexpr int      kMaxSmem     = 227 * 1024;    // opt-in dynamic shared memory per block, sm_100a
 constexpr int      kMaxThreadsA = 1024;          // __launch_bounds__ of the decode/cut kernel (<= 64 registers)
-constexpr int      kMaxThreadsB = 512;           // __launch_bounds__ of the walk/finish kernel (<= 128 registers)
+constexpr int      kMaxThreadsB = 640;           // __launch_bounds__ of the walk/finish kernel (<= 96 registers)
 constexpr uint32_t kLanes       = LGX_LANES;
 
 struct ImgHdr {
@@ -63,7 +63,9 @@ struct ImgHdr {
   uint32_t offc_dtri;       // f64 [(n_f+1) n_f / 2]  strict lower triangle over {HQ, fields}      (mode 0)
   uint32_t offc_dfb;        // f64 [n_f][n_b]         field -> BP legs                              (modes 0, 2)
   uint32_t offc_xy;         // f64x2 [1 + n_b + n_f]  vertex coordinates                            (modes 1, 2)
+  uint32_t offc_dhq;        // f64 [n_f]              field -> HQ legs (the closing leg of a tour)  (modes 1, 2)
   uint32_t offc_sh;         // u32x2 [n_f]            {s_q, h_q}
+  uint32_t offc_suinit;     // u32 [..]    initial array of the SU partition: capacity ranks of units 0.., right-aligned bytes
   uint32_t offc_cs;         // u32 [n_su]  SU capacity quanta by rank (ascending (capacity, unit)); the move kernels copy image C from here on
   uint32_t offc_rcp;        // f64 [..]    RN(1/k)
   uint32_t offc_unit;       // u8  [n_su]  rank -> SU
@@ -80,14 +82,14 @@ struct ImgHdr {
   uint32_t a32_scru, a32_rows_dec;      // diagnostic decode mode: scratch of the unit partitions, appended
 
   // ---- state rows of the walk/finish kernel
-  uint32_t c64_w, c64_e, c64_mask, c64_sd, c64_rows;
-  uint32_t c32_s, c32_nhu, c32_r, c32_ng, c32_magic, c32_hq, c32_ent, c32_rows;
+  uint32_t c64_w, c64_e, c64_mask, c64_sd, c64_tp, c64_rows;
+  uint32_t c32_s, c32_hn, c32_r, c32_hq, c32_ent, c32_rows;
 
   // ---- queue record (32-bit words, stored transposed: word w of slot q at queue[w*cap + q])
   //   0,1 index i | bpseq words | segend words | perm words
   uint32_t rec_bpseq, rec_segend, rec_perm, rec_words;
   uint32_t n_bpseq_words, n_segend_words, n_perm_words;
-  uint32_t pad_[2];
+  uint32_t pad_[1];
 };
 static_assert(sizeof(ImgHdr) % 16 == 0, "image header must keep 16-byte alignment");
 

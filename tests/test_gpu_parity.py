@@ -224,6 +224,14 @@ def test_concurrent_streams_share_an_instance(ctxs):
     assert np.array_equal(got, want[0])
 
 
+def test_inline_sqrt_equals_library_sqrt():
+    """The walk/finish kernel's in-line square root (two independent chains per field instead of two subroutine
+    calls) must be __dsqrt_rn bit for bit: 2^26 arguments per seed, structured and random (include/lgx.h)."""
+    for seed in (0, 0xC0FFEE, 2**63 + 17):
+        checked, bad = binding.selftest(0, 1 << 26, seed)
+        assert checked > (1 << 25) and bad == 0, (seed, checked, bad)
+
+
 @pytest.mark.parametrize("mode", [1, 2])
 def test_distance_modes_agree(ctxs, mode):
     """The three distance modes (tables / coordinates / mixed; tuning flags of the descriptor) compute the same
