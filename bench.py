@@ -222,6 +222,9 @@ def main():
     ap.add_argument("--impl", default="lgx", choices=["lgx", "reference"])
     ap.add_argument("--workload", default="medium")
     ap.add_argument("--batch-log2", type=int, default=None, help="candidates per GPU per step (default: config budget, capped 2^28)")
+    ap.add_argument("--chunk-log2", type=int, default=None, help="candidates per kernel pair (LGX_OPT_CHUNK_LOG2; profiling)")
+    ap.add_argument("--threads-a", type=int, default=None, help="LGX_OPT_THREADS_A (tuning)")
+    ap.add_argument("--threads-b", type=int, default=None, help="LGX_OPT_THREADS_B (tuning)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--alg1-workload", default="paper_scale", help="instance of the Algorithm 1 leg (SURVEY §8(f) N1/N3)")
     ap.add_argument("--alg1-iters", type=int, default=500)
@@ -249,6 +252,9 @@ def main():
     per_gpu = 1 << (args.batch_log2 if args.batch_log2 is not None else min(28, inst.budget.bit_length() - 1))
     total = per_gpu * world                      # weak scaling: fixed ids per GPU
     g = binding.Instance(inst)
+    for key, val in ((4, args.chunk_log2), (1, args.threads_a), (2, args.threads_b)):
+        if val is not None:
+            g.set_option(key, val)
     info = g.info()
     stream = torch.cuda.current_stream()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
@@ -296,6 +302,9 @@ def main():
 
     def e2e_step():
         g2 = binding.Instance(inst)
+        for key, val in ((4, args.chunk_log2), (1, args.threads_a), (2, args.threads_b)):
+            if val is not None:
+                g2.set_option(key, val)
         if world == 1:
             r = g2.search(inst.seed, per_gpu)
         else:

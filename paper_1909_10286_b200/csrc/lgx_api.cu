@@ -3,7 +3,7 @@
 // entry point fails with LGX_ECUDA when there is no usable CUDA device.
 #include "../../include/lgx.h"
 #include "lgx_image.h"
-#include "lgx_kernels.cuh"
+#include "lgx_dispatch.h"
 #include "lgx_moves.cuh"
 
 #include <algorithm>
@@ -68,21 +68,10 @@ inline double edge(double ax, double ay, double bx, double by)
   return std::sqrt(ss);
 }
 
-using KernelFn = void (*)(const KParams);
-
 template <int MODE> void pick_kernels(const ImgHdr &h, KernelFn &ka, KernelFn &kb)
 {
-  const bool p16 = h.perm16 != 0; const int dm = h.coords, mw = (int)h.mask_words;
-  const bool zd = h.zero_demand != 0u, x64 = h.n_extra_blocks > 7u;
-  ka = nullptr; kb = nullptr;
-#define LGX_PICK_A(P, Z, X) if (p16 == P && zd == Z && x64 == X) ka = lgx_decode_cut<P, Z, X, MODE>;
-  LGX_PICK_A(false, false, false) LGX_PICK_A(false, false, true) LGX_PICK_A(false, true, false) LGX_PICK_A(false, true, true)
-  LGX_PICK_A(true,  false, false) LGX_PICK_A(true,  false, true) LGX_PICK_A(true,  true, false) LGX_PICK_A(true,  true, true)
-#undef LGX_PICK_A
-#define LGX_PICK(P, D, M) if (p16 == P && dm == D && mw == M) kb = lgx_walk_finish<P, D, M, MODE>;
-  LGX_PICK(false, 0, 1) LGX_PICK(false, 0, 2) LGX_PICK(false, 1, 1) LGX_PICK(false, 1, 2) LGX_PICK(false, 2, 1) LGX_PICK(false, 2, 2)
-  LGX_PICK(true,  0, 1) LGX_PICK(true,  0, 2) LGX_PICK(true,  1, 1) LGX_PICK(true,  1, 2) LGX_PICK(true,  2, 1) LGX_PICK(true,  2, 2)
-#undef LGX_PICK
+  ka = pick_decode_cut(h, MODE);
+  kb = h.coords == 0 ? pick_walk_finish_dm0(h, MODE) : (h.coords == 1 ? pick_walk_finish_dm1(h, MODE) : pick_walk_finish_dm2(h, MODE));
 }
 
 void fill_round_keys(KParams &P, uint64_t seed)
@@ -149,7 +138,6 @@ int allow_max_smem(const void *fn, int smem_optin)
   return LGX_OK;
 }
 
-using MvKernelFn = void (*)(const MvParams);
 void pick_move_kernels(const ImgHdr &h, MvKernelFn &kb, MvKernelFn &ks);
 
 }  // namespace
@@ -392,9 +380,9 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   while (sq_shift < 5u && 4ull * ((uint64_t)nf << (sq_shift + 1u)) <= 16ull * 1024) ++sq_shift;
   int rc = build_image_a(I, sq_shift);
   if (rc != LGX_OK) { free_instance(I); return rc; }
-  I->threads_a     = (int)fit_threads(budget, H.image_bytes, (int64_t)I->a_state, kMaxThreadsA);
-  I->threads_a_dec = (int)fit_threads(budget, H.image_bytes, (int64_t)I->a_state_dec, kMaxThreadsA);
-  I->threads_b     = (int)fit_threads(budget, H.imagec_bytes, (int64_t)I->b_state, kMaxThreadsB);
+  I->threads_a     = (int)fit_threads(budget, H.image_bytes, (int64_t)I->a_state, H.perm16 ? kMaxThreadsA16 : kMaxThreadsA);
+  I->threads_a_dec = (int)fit_threads(budget, H.image_bytes, (int64_t)I->a_state_dec, H.perm16 ? kMaxThreadsA16 : kMaxThreadsA);
+  I->threads_b     = (int)fit_threads(budget, H.imagec_bytes, (int64_t)I->b_state, H.coords == 0 ? kMaxThreadsB : kMaxThreadsBC);
   if (I->threads_a < 32 || I->threads_a_dec < 32 || I->threads_b < 32) { free_instance(I); return LGX_ETOOBIG; }
   I->grid = I->sm_count;                       // one persistent block per SM
   // candidates per kernel pair: the queue holds a whole chunk (every candidate may pass eq. (2)); <= 512 MiB, <= 2^22
@@ -511,13 +499,13 @@ int lgx_instance_set_option(lgx_instance *I, int key, int64_t value)
   auto threads_ok = [](int64_t v, int64_t lo, int64_t hi) { return v >= lo && v <= hi && v % 32 == 0; };
   switch (key) {
     case LGX_OPT_THREADS_A: {
-      const int64_t hi = fit_threads(budget, H.image_bytes, (int64_t)I->a_state, kMaxThreadsA);
+      const int64_t hi = fit_threads(budget, H.image_bytes, (int64_t)I->a_state, H.perm16 ? kMaxThreadsA16 : kMaxThreadsA);
       if (!threads_ok(value, 32, hi)) return LGX_EINVAL;
-      I->threads_a = (int)value; I->threads_a_dec = (int)std::min<int64_t>(value, fit_threads(budget, H.image_bytes, (int64_t)I->a_state_dec, kMaxThreadsA));
+      I->threads_a = (int)value; I->threads_a_dec = (int)std::min<int64_t>(value, fit_threads(budget, H.image_bytes, (int64_t)I->a_state_dec, H.perm16 ? kMaxThreadsA16 : kMaxThreadsA));
       return LGX_OK;
     }
     case LGX_OPT_THREADS_B: {
-      const int64_t hi = fit_threads(budget, H.imagec_bytes, (int64_t)I->b_state, kMaxThreadsB);
+      const int64_t hi = fit_threads(budget, H.imagec_bytes, (int64_t)I->b_state, H.coords == 0 ? kMaxThreadsB : kMaxThreadsBC);
       if (!threads_ok(value, 32, hi)) return LGX_EINVAL;
       I->threads_b = (int)value;
       return LGX_OK;
@@ -536,12 +524,12 @@ int lgx_instance_set_option(lgx_instance *I, int key, int64_t value)
     case LGX_OPT_SQ_SHIFT: {
       if (value < 0 || value > 5) return LGX_EINVAL;
       const int64_t img = 16 + 4ll * ((int64_t)H.n_f << value) + 16 + 4ll * H.n_b;
-      if (fit_threads(budget, img, (int64_t)I->a_state_dec, kMaxThreadsA) < 32) return LGX_ETOOBIG;
+      if (fit_threads(budget, img, (int64_t)I->a_state_dec, H.perm16 ? kMaxThreadsA16 : kMaxThreadsA) < 32) return LGX_ETOOBIG;
       int rc = check_device(I);
       if (rc == LGX_OK) { cudaDeviceSynchronize(); rc = build_image_a(I, (uint32_t)value); }
       if (rc != LGX_OK) return rc;
-      I->threads_a     = (int)std::min<int64_t>(I->threads_a, fit_threads(budget, H.image_bytes, (int64_t)I->a_state, kMaxThreadsA));
-      I->threads_a_dec = (int)std::min<int64_t>(I->threads_a_dec, fit_threads(budget, H.image_bytes, (int64_t)I->a_state_dec, kMaxThreadsA));
+      I->threads_a     = (int)std::min<int64_t>(I->threads_a, fit_threads(budget, H.image_bytes, (int64_t)I->a_state, H.perm16 ? kMaxThreadsA16 : kMaxThreadsA));
+      I->threads_a_dec = (int)std::min<int64_t>(I->threads_a_dec, fit_threads(budget, H.image_bytes, (int64_t)I->a_state_dec, H.perm16 ? kMaxThreadsA16 : kMaxThreadsA));
       return LGX_OK;
     }
     default: return LGX_EINVAL;
@@ -649,7 +637,7 @@ int lgx_selftest(int what, uint64_t n, uint64_t seed, uint64_t *h_out)
   cudaError_t e = cudaMemset(d, 0, 16);
   if (e == cudaSuccess) {
     void *args[] = { (void *)&n, (void *)&seed, (void *)&d };
-    e = cudaLaunchKernel((const void *)lgx_selftest_sqrt_k, dim3(592), dim3(256), args, 0, nullptr);
+    e = cudaLaunchKernel(selftest_sqrt_kernel(), dim3(592), dim3(256), args, 0, nullptr);
   }
   unsigned long long r[2] = {0, 0};
   if (e == cudaSuccess) e = cudaMemcpy(r, d, 16, cudaMemcpyDeviceToHost);
@@ -796,16 +784,9 @@ int lgx_eval_batch_host(const lgx_instance *I, uint64_t seed, const uint64_t *h_
 
 namespace {
 
-using MvKernelFn = void (*)(const MvParams);
-
 void pick_move_kernels(const ImgHdr &h, MvKernelFn &kb, MvKernelFn &ks)
 {
-  kb = ks = nullptr;
-  const bool hb = (h.flags & LGX_FLAG_HU_BALANCE) != 0u;
-  if (h.mask_words == 1u && !hb) { kb = lgx_move_eval_k<1, false>; ks = lgx_local_search_k<1, false>; }
-  if (h.mask_words == 2u && !hb) { kb = lgx_move_eval_k<2, false>; ks = lgx_local_search_k<2, false>; }
-  if (h.mask_words == 1u && hb)  { kb = lgx_move_eval_k<1, true>;  ks = lgx_local_search_k<1, true>; }
-  if (h.mask_words == 2u && hb)  { kb = lgx_move_eval_k<2, true>;  ks = lgx_local_search_k<2, true>; }
+  if (h.mask_words == 1u) pick_move_kernels_mw1(h, kb, ks); else pick_move_kernels_mw2(h, kb, ks);
 }
 
 // A plan is valid when every BP sits on exactly one tour at a unique position 0..len-1, every field on exactly
@@ -910,7 +891,7 @@ int lgx_init_plan(const lgx_instance *I, uint8_t *h_bp_tour, uint8_t *h_bp_pos, 
   P.scratch = scratch;
   {
     void *args[] = { (void *)&P };
-    e = cudaLaunchKernel((const void *)lgx_init_plan_k, dim3(1), dim3(256), args, 0, st);
+    e = cudaLaunchKernel(init_plan_kernel(), dim3(1), dim3(256), args, 0, st);
   }
   I->launches.fetch_add(1);
   if (e == cudaSuccess) rc = plan_download(H, D, h_bp_tour, h_bp_pos, h_field_bp, h_field_pos, h_hu_tour, h_su_tour, st);

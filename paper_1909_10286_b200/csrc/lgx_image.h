@@ -38,7 +38,9 @@ constexpr uint32_t kPhiloxW0    = 0x9E3779B9u;   // key increments
 constexpr uint32_t kPhiloxW1    = 0xBB67AE85u;
 constexpr int      kMaxSmem     = 227 * 1024;    // opt-in dynamic shared memory per block, sm_100a
 constexpr int      kMaxThreadsA = 1024;          // __launch_bounds__ of the decode/cut kernel (<= 64 registers)
-constexpr int      kMaxThreadsB = 640;           // __launch_bounds__ of the walk/finish kernel (<= 96 registers)
+constexpr int      kMaxThreadsA16 = 384;         // ... with 16-bit field ids (N_F > 255: the permutation caps the residency anyway; <= 168 registers)
+constexpr int      kMaxThreadsB = 640;           // __launch_bounds__ of the walk/finish kernel with distance tables (<= 96 registers)
+constexpr int      kMaxThreadsBC = 448;          // ... with coordinates (<= 144 registers: several square-root chains in flight)
 constexpr uint32_t kLanes       = LGX_LANES;
 
 struct ImgHdr {

@@ -1116,6 +1116,7 @@ __device__ __forceinline__ void warp_argmin(double &d, uint32_t &i)
 // nearest-neighbour chain over the BPs from HQ, cut into N_T consecutive runs (R32).  Step 2 (L124): fields in
 // identification order (L173) to their closest BP not yet supplied, else to their closest BP.  Step 3 (L126,
 // L171): per BP a nearest-neighbour order starting from HQ.
+#ifdef LGX_INSTANTIATE_INIT_PLAN      // non-template kernel: compiled by one translation unit (lgx_inst_moves.cu)
 __global__ void __launch_bounds__(256, 1) lgx_init_plan_k(const InitParams P)
 {
   const uint32_t tid = threadIdx.x, T = blockDim.x, lane = tid & 31u, warp = tid >> 5, n_warps = T >> 5;
@@ -1189,5 +1190,6 @@ __global__ void __launch_bounds__(256, 1) lgx_init_plan_k(const InitParams P)
 
 #undef MV_TAB
 #undef MV_CTAB
+#endif
 
 }  // namespace lgx
