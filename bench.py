@@ -2,11 +2,14 @@
 """bench.py — candidates/s of the lgx hot path on B200 (BASELINE.json metric).
 
 A "step" is one pass of the whole hot path (the persistent kernel
-pair lgx_decode_walk + lgx_finish per chunk, over the shared-memory images built by a1) over
+pair lgx_decode_cut + lgx_walk_finish per chunk, over the shared-memory images built by a1) over
 one batch of candidates:
 `lgx_search` over the Medium config's full budget (2^28 ids, 100 fields / 8 BPs / 5 tours;
 the config the north_star target of >= 1e9 cand/s is quoted on).  Synthetic, seeded
 instance (paper_1909_10286_b200/workloads.py); nothing is read from /root/reference.
+Beside the headline the line carries `configs` (lgx_search and lgx_eval_batch timed separately on toy, small,
+medium, large, sweep and paper_scale, each with its roofline fractions) and `best_vs_oracle` (the GPU's (cost, id)
+over an id prefix against the oracle's, bit for bit: the second half of BASELINE.json's metric).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload medium]
 
@@ -23,31 +26,41 @@ sys.path.insert(0, ROOT)
 
 METRIC = "candidate plans evaluated/sec"
 UNIT = "candidates/s"
-# Algorithmic thread-instructions per candidate: what the method itself needs,
-# split into the part every candidate pays (decode + pass 1: kernel lgx_decode_walk) and the part
-# only feasible candidates pay (tour statistics, Algorithm 2, pass 2, cost: kernel lgx_finish).
-ALG2_ITERS = {"toy": 2.3, "small": 5.6, "medium": 9.9, "large": 12.7, "sweep": 19.5}   # oracle-measured means
+ALL_CONFIGS = ("toy", "small", "medium", "large", "sweep", "paper_scale")
+# log2 of the ids per lgx_search step / per lgx_eval_batch call of the `configs` leg (about 0.3-1 s of GPU time each),
+# and of the id prefix [0, 2^k) the oracle scans for `best_vs_oracle` (about 1 s on the host cores each)
+CONFIG_SEARCH_LOG2 = {"toy": 30, "small": 30, "medium": 29, "large": 28, "sweep": 26, "paper_scale": 25}
+CONFIG_EVAL_LOG2   = {"toy": 24, "small": 24, "medium": 24, "large": 24, "sweep": 23, "paper_scale": 22}
+ORACLE_PREFIX_LOG2 = {"toy": 21, "small": 21, "medium": 21, "large": 19, "sweep": 18, "paper_scale": 17}
 
 
-def w_alg(inst, workload):
+def w_alg(inst, a2_iters):
+    """MODEL, not a measurement: thread-instructions the method itself needs per candidate.
+    Returns (round-1 model: decode + pass 1 for every candidate, the rest for feasible ones;
+             strict model of the round-2 kernel split: (every candidate, feasible candidate))."""
     nf, nb, nt, nhu, nsu = inst.n_fields, inst.n_bps, inst.n_tours, inst.n_hu, inst.n_su
     cd = lambda a, b: -(-a // b)
     part_blocks = lambda n: cd(n, 4) + cd(n - nt, 4)            # Philox blocks of one ordered partition
-    # every candidate: BP partition, field permutation + extras, pass 1  (kernel lgx_decode_walk)
     blocks_a = cd(nf, 4) + part_blocks(nb) + cd((nb - 1) * 4 // 3 + 8, 4)
-    decode_walk = 40 * blocks_a + 7 * (nf + nb) + 2 * (nb - nt) + 6 * nb + 14 * nf + 10 * (nb + nt)
-    # feasible candidates only: HU / SU partitions, tour statistics, Algorithm 2, pass 2, cost  (lgx_finish)
+    decode = 40 * blocks_a + 7 * (nf + nb) + 2 * (nb - nt) + 6 * nb
+    pass1 = 14 * nf + 10 * (nb + nt)
     blocks_c = part_blocks(nhu) + part_blocks(nsu)
     finish = (40 * blocks_c + 7 * (nhu + nsu) + 2 * (nhu + nsu - 2 * nt) + 6 * nhu + 10 * nsu
-              + 6 * nb + 92 * nt + 110 * ALG2_ITERS.get(workload, 10.0) + 18 * nf + 10 * (nb + nt) + 9 * nt + 5)
-    return decode_walk, finish
+              + 6 * nb + 92 * nt + 110 * a2_iters + 18 * nf + 10 * (nb + nt) + 9 * nt + 5)
+    # round 2: lgx_decode_cut decides the cuts and eq. (2) on quanta alone (s_q look-up, add, compare, extras bit:
+    # 6 per field, 4 per BP); the geometry of pass 1 (8 per field + the flushes) is paid by feasible candidates only
+    cut = 6 * nf + 4 * nb
+    geo1 = 8 * nf + 10 * (nb + nt)
+    return (decode + pass1, finish), (decode + cut, geo1 + finish)
 
 
 SM_MAX_MHZ_FALLBACK = 1965.0
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE lgx_decode_walk launch (757 760 Medium candidates) from the
-# `ncu --set full` capture summarised in profiles/r01_v7_medium_ncu_full.md: 0.12 MB read + 4.08 MB written (the
-# queue records of the feasible candidates that do not stay in L2).  Per launch, like `achieved`.
-TRAFFIC_BYTES_DECODE_WALK_MEDIUM = 4.20e6
+# PROFILE CONSTANTS (not measured in this run): dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the
+# config's dominant kernel from the `ncu --set full` captures summarised under profiles/ (file named per entry),
+# with the candidates that launch covered.  The path's algorithmic HBM bytes are 0 per candidate in lgx_search
+# (everything lives in shared memory and the L2-resident queue); these numbers show the real traffic is negligible.
+TRAFFIC = {
+}
 
 
 def peaks():
@@ -96,7 +109,8 @@ class ClockSampler:
 
 def oracle_rate(name, n_ids, procs):
     """The oracle as it stands (single-threaded by design), run as `procs` independent
-    processes over disjoint contiguous id ranges on the host cores."""
+    processes over disjoint contiguous id ranges on the host cores.  Returns (ids/s, seconds, (cost, id) of the
+    ordered minimum over ids [0, n_ids // procs * procs))."""
     import multiprocessing as mp
     ctx = mp.get_context("fork")
     per = max(1, n_ids // procs)
@@ -114,6 +128,34 @@ def _oracle_chunk(name, first, n):
     inst = wl.make(name)
     o = lgo.Oracle(inst)
     return o.search(inst.seed, n, first_id=first)
+
+
+def _oracle_a2_chunk(name, first, n):
+    """Accepted Algorithm-2 moves (scalars[7] of lgo_score) of the feasible candidates among ids [first, first+n)."""
+    import numpy as np
+    from oracle import lgo
+    from paper_1909_10286_b200 import workloads as wl
+    inst = wl.make(name)
+    o = lgo.Oracle(inst)
+    sc = np.zeros(8)
+    moves = feas = 0
+    for i in range(first, first + n):
+        pl = o.decode(inst.seed, i)
+        o.score_fast(pl["bp_tour"], pl["bp_pos"], pl["field_bp"], pl["field_pos"], pl["hu_tour"], pl["su_tour"], sc)
+        if sc[0] != 0.0:
+            feas += 1; moves += int(sc[7])
+    return moves, feas
+
+
+def oracle_alg2_iters(name, n_ids, procs):
+    """Mean number of accepted Algorithm-2 moves per feasible candidate, measured with the oracle on ids [0, n_ids):
+    the `A2` of the work model."""
+    import multiprocessing as mp
+    per = max(1, n_ids // procs)
+    with mp.get_context("fork").Pool(procs) as pool:
+        res = pool.starmap(_oracle_a2_chunk, [(name, r * per, per) for r in range(procs)])
+    moves = sum(r[0] for r in res); feas = sum(r[1] for r in res)
+    return (moves / feas if feas else 0.0), feas, per * procs
 
 
 def _oracle_moves_chunk(name, first, n):
@@ -229,6 +271,7 @@ def main():
     ap.add_argument("--alg1-workload", default="paper_scale", help="instance of the Algorithm 1 leg (SURVEY §8(f) N1/N3)")
     ap.add_argument("--alg1-iters", type=int, default=500)
     ap.add_argument("--no-alg1", action="store_true")
+    ap.add_argument("--no-configs", action="store_true", help="skip the per-config leg (toy .. paper_scale)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "lgx" else args.warmup
     if args.impl == "reference":
@@ -251,10 +294,16 @@ def main():
     inst = wl.make(args.workload)
     per_gpu = 1 << (args.batch_log2 if args.batch_log2 is not None else min(28, inst.budget.bit_length() - 1))
     total = per_gpu * world                      # weak scaling: fixed ids per GPU
-    g = binding.Instance(inst)
-    for key, val in ((4, args.chunk_log2), (1, args.threads_a), (2, args.threads_b)):
-        if val is not None:
-            g.set_option(key, val)
+    opts = ((4, args.chunk_log2), (1, args.threads_a), (2, args.threads_b))
+
+    def new_instance(ins):
+        gi = binding.Instance(ins)
+        for key, val in opts:
+            if val is not None:
+                gi.set_option(key, val)
+        return gi
+
+    g = new_instance(inst)
     info = g.info()
     stream = torch.cuda.current_stream()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
@@ -265,7 +314,7 @@ def main():
         torch.cuda.synchronize()
 
     def step(first_total=0):
-        # this rank's contiguous share of [0, total); one 16-byte exchange when world > 1
+        # this rank's contiguous share of [0, total); one 24-byte exchange when world > 1
         if world == 1:
             return g.search(inst.seed, per_gpu, first_id=first_total)
         return sharding.search_sharded(lambda s, n, f: g.search(s, n, first_id=f), inst.seed, total, rank, world, first_total)
@@ -301,10 +350,7 @@ def main():
     e2e_steps = max(2, min(args.steps, 3))
 
     def e2e_step():
-        g2 = binding.Instance(inst)
-        for key, val in ((4, args.chunk_log2), (1, args.threads_a), (2, args.threads_b)):
-            if val is not None:
-                g2.set_option(key, val)
+        g2 = new_instance(inst)
         if world == 1:
             r = g2.search(inst.seed, per_gpu)
         else:
@@ -325,27 +371,29 @@ def main():
     e2e_value = total * e2e_steps / e2e_s
     assert r2 == best, "e2e result differs from the device-timed result"
 
-    # ---- eval_batch (per-candidate outputs) timed separately, device and host buffers
-    extra = {}
-    if rank == 0:
-        n_ev = 1 << 24
-        out = g.eval_batch(inst.seed, first_id=0, n=n_ev)
+    def time_eval_batch(gi, ins, n_ev, n_h):
+        """lgx_eval_batch (per-candidate outputs): median of 3 device-timed calls, plus one call with host buffers."""
+        out = gi.eval_batch(ins.seed, first_id=0, n=n_ev)
         torch.cuda.synchronize()
         ev_list = []
-        for _ in range(3):                       # median of 3 device-timed calls
+        for _ in range(3):
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record(stream); g.eval_batch(inst.seed, first_id=0, n=n_ev, out=out); b.record(stream)
+            a.record(stream); gi.eval_batch(ins.seed, first_id=0, n=n_ev, out=out); b.record(stream)
             torch.cuda.synchronize()
             ev_list.append(a.elapsed_time(b))
         ev_ms = sorted(ev_list)[1]
-        n_h = 1 << 22
-        host_out = (np.empty(n_h), np.empty(n_h), np.empty(n_h), np.empty(n_h, np.uint8))
-        g.eval_batch_host(inst.seed, first_id=0, n=n_h, out=host_out)
-        t0 = time.perf_counter(); g.eval_batch_host(inst.seed, first_id=0, n=n_h, out=host_out); th = time.perf_counter() - t0
-        extra["eval_batch"] = {"value": n_ev / ev_ms * 1e3, "unit": UNIT, "ids": n_ev,
-                               "feasible_fraction": float(out[3].float().mean().item()),
-                               "e2e_host_buffers": {"value": n_h / th, "unit": UNIT, "ids": n_h,
-                                                    "d2h_bytes": 25 * n_h, "h2d_bytes": 0}}
+        res = {"value": n_ev / ev_ms * 1e3, "unit": UNIT, "ids": n_ev,
+               "feasible_fraction": float(out[3].float().mean().item())}
+        if n_h:
+            host_out = (np.empty(n_h), np.empty(n_h), np.empty(n_h), np.empty(n_h, np.uint8))
+            gi.eval_batch_host(ins.seed, first_id=0, n=n_h, out=host_out)
+            t0 = time.perf_counter(); gi.eval_batch_host(ins.seed, first_id=0, n=n_h, out=host_out); th = time.perf_counter() - t0
+            res["e2e_host_buffers"] = {"value": n_h / th, "unit": UNIT, "ids": n_h, "d2h_bytes": 25 * n_h, "h2d_bytes": 0}
+        return res
+
+    extra = {}
+    if rank == 0:
+        extra["eval_batch"] = time_eval_batch(g, inst, 1 << 24, 1 << 22)
 
     if rank == 0 and world == 1 and not args.no_alg1:
         extra["alg1"] = bench_alg1(args, torch, binding, wl)
@@ -359,35 +407,99 @@ def main():
     sm_max = float(pk.get("sm_max_mhz", SM_MAX_MHZ_FALLBACK))
     n_sm = info["sm_count"]
     peak_ginst = n_sm * 4 * 32 * sm_max * 1e6 / 1e9          # thread-instructions/s at max clock
-    feas = extra.get("eval_batch", {}).get("feasible_fraction", 1.0)
-    w_dw, w_fin = w_alg(inst, args.workload)
-    cand_timed = per_gpu * args.steps                         # this rank's candidates in the timed region
-    per_launch = cand_timed / max(n_pairs, 1)                 # candidates per launch of each kernel
-    ms_a = ns_a * 1e-6 / max(n_pairs, 1); ms_c = ns_c * 1e-6 / max(n_pairs, 1)
-    ach_a = per_launch * w_dw / (ms_a * 1e-3) / 1e9 if ms_a > 0 else None
-    ach_c = per_launch * feas * w_fin / (ms_c * 1e-3) / 1e9 if ms_c > 0 else None
-    ach_all = (w_dw + feas * w_fin) * value / world / 1e9
-    obs = clocks.get("sm_mhz") or sm_max
-    roofline = {"bound": "alu", "kernel": "lgx_decode_walk (dominant: %.0f %% of the kernel time of a step)" % (100.0 * ns_a / max(ns_a + ns_c, 1)),
-                "achieved": ach_a, "peak": peak_ginst, "unit": "G thread-inst/s", "frac": ach_a / peak_ginst if ach_a else None,
-                "traffic": TRAFFIC_BYTES_DECODE_WALK_MEDIUM if args.workload == "medium" else None, "launch_ms": ms_a, "launches_timed": n_pairs, "candidates_per_launch": per_launch,
-                "w_alg_thread_inst_per_candidate": w_dw,
-                "peak_source": f"{n_sm} SMs x 4 schedulers x 32 lanes x {sm_max:.0f} MHz ({pk_src} sm_max_mhz; DESIGN.md s8)",
-                "frac_at_observed_clock": ach_a / (peak_ginst * obs / sm_max) if ach_a else None,
-                "other_kernels": [{"kernel": "lgx_finish", "launch_ms": ms_c, "achieved": ach_c,
-                                   "frac": ach_c / peak_ginst if ach_c else None,
-                                   "w_alg_thread_inst_per_feasible_candidate": w_fin, "feasible_fraction": feas}],
-                "whole_step": {"w_alg_thread_inst_per_candidate": w_dw + feas * w_fin, "achieved": ach_all,
-                               "frac": ach_all / peak_ginst},
-                "hbm_note": "queue traffic ~%.0f B per candidate; dram bytes per launch in profiles/ (negligible)" % (feas * info["record_bytes"])}
+    cores = os.cpu_count() or 1
 
+    def roofline_of(ins, name, feas, a2, rate_per_gpu, ns_a_, ns_b_, pairs, cand_timed, rec_bytes):
+        """Issue roofline of one config from the work MODEL w_alg (a model) and the measured kernel times."""
+        (w_dw, w_fin), (w_a, w_b) = w_alg(ins, a2)
+        per_launch = cand_timed / max(pairs, 1)
+        ms_a_ = ns_a_ * 1e-6 / max(pairs, 1); ms_b_ = ns_b_ * 1e-6 / max(pairs, 1)
+        ach_a = per_launch * w_a / (ms_a_ * 1e-3) / 1e9 if ms_a_ > 0 else None
+        ach_b = per_launch * feas * w_b / (ms_b_ * 1e-3) / 1e9 if ms_b_ > 0 else None
+        a_dominant = ns_a_ >= ns_b_
+        ach_d, ms_d = (ach_a, ms_a_) if a_dominant else (ach_b, ms_b_)
+        ach_r1 = (w_dw + feas * w_fin) * rate_per_gpu / 1e9
+        ach_strict = (w_a + feas * w_b) * rate_per_gpu / 1e9
+        tr = TRAFFIC.get(name)
+        return {"bound": "alu",
+                "kernel": "%s (dominant: %.0f %% of the kernel time of a step)" % ("lgx_decode_cut" if a_dominant else "lgx_walk_finish", 100.0 * max(ns_a_, ns_b_) / max(ns_a_ + ns_b_, 1)),
+                "achieved": ach_d, "peak": peak_ginst, "unit": "G thread-inst/s", "frac": ach_d / peak_ginst if ach_d else None,
+                "traffic": tr["bytes_per_launch"] if tr else None,
+                "traffic_source": ("profile constant: %s, %d candidates per launch" % (tr["file"], tr["candidates_per_launch"])) if tr else None,
+                "launch_ms": ms_d, "launches_timed": pairs, "candidates_per_launch": per_launch,
+                "work_model": "w_alg (bench.py; DESIGN.md s8): a hand model of the thread-instructions the method needs, not a measured count; "
+                              "A2 = mean accepted Algorithm-2 moves, oracle-measured in this run",
+                "alg2_moves_mean": a2,
+                "peak_source": f"{n_sm} SMs x 4 schedulers x 32 lanes x {sm_max:.0f} MHz ({pk_src} sm_max_mhz; DESIGN.md s8)",
+                "kernels": [{"kernel": "lgx_decode_cut", "launch_ms": ms_a_, "achieved": ach_a, "frac": ach_a / peak_ginst if ach_a else None,
+                             "w_alg_thread_inst_per_candidate": w_a},
+                            {"kernel": "lgx_walk_finish", "launch_ms": ms_b_, "achieved": ach_b, "frac": ach_b / peak_ginst if ach_b else None,
+                             "w_alg_thread_inst_per_feasible_candidate": w_b, "feasible_fraction": feas}],
+                "whole_step": {"w_alg_thread_inst_per_candidate": w_dw + feas * w_fin, "achieved": ach_r1, "frac": ach_r1 / peak_ginst,
+                               "model": "round-1 model (unchanged): decode + pass 1 charged to every candidate"},
+                "whole_step_strict": {"w_alg_thread_inst_per_candidate": w_a + feas * w_b, "achieved": ach_strict, "frac": ach_strict / peak_ginst,
+                                      "model": "round-2 kernel split: pass-1 geometry charged to feasible candidates only (PAPER.md L186)"},
+                "kernel_time_share_of_step": (ns_a_ + ns_b_) * 1e-6 / max(cand_timed / rate_per_gpu * 1e3, 1e-9),
+                "hbm_note": "queue traffic ~%.0f B per candidate, L2-resident in practice; algorithmic HBM bytes of lgx_search: 0" % (feas * rec_bytes)}
+
+    def best_vs_oracle(gi, ins, name):
+        """The second half of the metric: the GPU's (cost, id) over an id prefix must equal the oracle's, bit for bit."""
+        n_pre = 1 << ORACLE_PREFIX_LOG2.get(name, 18)
+        rate, dt, cbest = oracle_rate(name, n_pre, cores)
+        n_scanned = n_pre // cores * cores
+        gbest = gi.search(ins.seed, n_scanned)
+        return {"ids": n_scanned, "oracle": {"cost": cbest[0], "id": cbest[1]}, "lgx": {"cost": gbest[0], "id": gbest[1]},
+                "match": bool(gbest[0] == cbest[0] and gbest[1] == cbest[1])}, rate, dt
+
+    feas = extra.get("eval_batch", {}).get("feasible_fraction", 1.0)
+    a2_main = 0.0
     cpu = None
+    bvo = None
     if not args.no_cpu_baseline:
-        cores = os.cpu_count() or 1
-        n_cpu = 1 << 21 if args.workload in ("toy", "small", "medium") else 1 << 18
-        rate, dt, cbest = oracle_rate(args.workload, n_cpu, cores)
+        a2_main, _, _ = oracle_alg2_iters(args.workload, 2048 if inst.n_fields <= 250 else 512, cores)
+        bvo, rate, dt = best_vs_oracle(g, inst, args.workload)
+        n_cpu = 1 << 23 if args.workload in ("toy", "small", "medium") else 1 << 19
+        rate, dt, _ = oracle_rate(args.workload, n_cpu, cores)
         cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": f"ids [0, {n_cpu // cores * cores}) of the {args.workload} budget, {cores} processes, {dt:.1f} s wall"}
+    else:
+        a2_main = {"toy": 2.3, "small": 5.5, "medium": 9.8, "large": 12.9, "sweep": 18.5, "paper_scale": 8.4}.get(args.workload, 10.0)
+    roofline = roofline_of(inst, args.workload, feas, a2_main, value / world, ns_a, ns_c, n_pairs, per_gpu * args.steps, info["record_bytes"])
+
+    # ---- every config (BASELINE.json: "on all five configs", config 5: lgx_eval_batch and lgx_search timed separately)
+    configs = {}
+    if world == 1 and not args.no_configs:
+        for name in ALL_CONFIGS:
+            ins = wl.make(name)
+            gi = g if name == args.workload and not any(v is not None for _, v in opts) else binding.Instance(ins)
+            n_s = 1 << CONFIG_SEARCH_LOG2[name]
+            gi.search(ins.seed, n_s // 4); gi.search(ins.seed, n_s // 4); gi.search(ins.seed, n_s // 4)      # W = 3 warm-up calls
+            gi.set_timing(True)
+            l0 = gi.query(7)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            flush.fill_(1); a.record(stream)
+            cbest = gi.search(ins.seed, n_s)
+            b.record(stream); torch.cuda.synchronize()
+            ka, kb, kp = gi.kernel_times(); gi.set_timing(False)
+            ms = a.elapsed_time(b)
+            evb = time_eval_batch(gi, ins, 1 << CONFIG_EVAL_LOG2[name], 0)
+            c = {"workload": f"N_T={ins.n_tours} N_B={ins.n_bps} N_F={ins.n_fields} N_HU={ins.n_hu} N_SU={ins.n_su}",
+                 "lgx_search": {"value": n_s / ms * 1e3, "unit": UNIT, "ids": n_s, "ms": ms, "gpu_launches": gi.query(7) - l0,
+                                "best": {"cost": cbest[0], "id": cbest[1]}},
+                 "lgx_eval_batch": evb, "threads_per_block": [gi.query(1), gi.query(8)], "distance_mode": gi.query(4)}
+            if not args.no_cpu_baseline:
+                a2, _, _ = oracle_alg2_iters(name, 1024 if ins.n_fields <= 250 else 256, cores)
+                c["best_vs_oracle"], orate, odt = best_vs_oracle(gi, ins, name)
+                c["cpu_baseline"] = {"value": orate, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                     "sample": f"ids [0, {c['best_vs_oracle']['ids']}), {odt:.1f} s wall"}
+            else:
+                a2 = {"toy": 2.3, "small": 5.5, "medium": 9.8, "large": 12.9, "sweep": 18.5, "paper_scale": 8.4}[name]
+            r = roofline_of(ins, name, evb["feasible_fraction"], a2, n_s / ms * 1e3, ka, kb, kp, n_s, gi.query(11))
+            c["roofline"] = {k: r[k] for k in ("kernel", "frac", "launch_ms", "candidates_per_launch", "alg2_moves_mean", "kernels",
+                                               "whole_step", "whole_step_strict", "kernel_time_share_of_step", "traffic", "traffic_source")}
+            configs[name] = c
+            if gi is not g:
+                gi.close()
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": dev_ms / args.steps, "higher_is_better": True,
@@ -396,15 +508,17 @@ def main():
                                    f"N_HU={inst.n_hu} N_SU={inst.n_su}",
                        "candidates_per_gpu_per_step": per_gpu, "seed": inst.seed,
                        "l2": "flushed between timed iterations (256 MiB write)",
-                       "parallelism": f"id-range shards x{world}", "threads_per_block": info["threads"],
-                       "grid": info["grid"], "smem_bytes": info["smem_bytes"]},
-            "best": {"cost": best[0], "id": best[1]},
+                       "parallelism": f"id-range shards x{world}", "threads_per_block": [info["threads"], info["threads_finish"]],
+                       "grid": info["grid"], "smem_bytes": [info["smem_bytes"], info["smem_bytes_finish"]]},
+            "best": {"cost": best[0], "id": best[1]}, "best_vs_oracle": bvo,
             "clocks": clocks, "gpu_launches": launches,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": info["image_bytes"],
                     "d2h_bytes_per_step": 16, "steps": e2e_steps,
                     "what": "lgx_instance_create(host arrays) + lgx_search + lgx_instance_destroy, wall clock"},
             "wall_s_timed_region": t_wall, "roofline": roofline, "cpu_baseline": cpu}
     line.update(extra)
+    if configs:
+        line["configs"] = configs
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
