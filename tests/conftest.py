@@ -8,3 +8,5 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
+    # the multi-process oracle helpers fork after torch started its threads; the children only run the C oracle
+    config.addinivalue_line("filterwarnings", "ignore:.*multi-threaded.*fork.*:DeprecationWarning")

@@ -11,10 +11,12 @@ pytestmark = pytest.mark.gpu
 
 from oracle import lgo
 from paper_1909_10286_b200 import binding, workloads as wl
-from helpers import mk_instance
+from helpers import mk_instance, oracle_eval_mp, oracle_search_mp
 
 RTOL = 1e-9
-N_ORACLE = {"toy": 1 << 16, "small": 1 << 15, "medium": 1 << 14, "large": 1 << 12, "sweep": 3 << 10, "paper_scale": 1 << 9}
+# SURVEY s8(d) parity protocol: 2^16 ids per id set on every config (2^12 on paper_scale); the oracle runs as it is,
+# one process per host core over disjoint chunks of the ids (helpers.oracle_eval_mp)
+N_ORACLE = {"toy": 1 << 16, "small": 1 << 16, "medium": 1 << 16, "large": 1 << 16, "sweep": 1 << 16, "paper_scale": 1 << 12}
 
 
 @pytest.fixture(scope="module")
@@ -53,7 +55,7 @@ def test_eval_batch_matches_oracle(ctxs, name):
     inst, o, g = ctxs(name)
     n = N_ORACLE[name]
     for label, ids, first in id_sets(inst, n):
-        want = o.eval_batch(inst.seed, ids=ids, first_id=first, n=n)
+        want = oracle_eval_mp(name, inst.seed, ids=ids, first_id=first, n=n)
         d_ids = torch.from_numpy(ids.astype(np.int64)).cuda() if ids is not None else None
         got = [t.cpu().numpy() for t in g.eval_batch(inst.seed, ids=d_ids, first_id=first, n=n)]
         assert np.array_equal(got[3], want[3]), f"{name}/{label}: feasibility flags differ"
@@ -65,7 +67,7 @@ def test_eval_batch_matches_oracle(ctxs, name):
 @pytest.mark.parametrize("name", ["toy", "small", "medium", "large", "sweep"])
 def test_decode_batch_matches_oracle(ctxs, name):
     inst, o, g = ctxs(name)
-    n = max(256, N_ORACLE[name] // 8)
+    n = 2048 if name in ("toy", "small", "medium") else 512
     for label, ids, first in id_sets(inst, n):
         want = o.decode_batch(inst.seed, ids=ids, first_id=first, n=n)
         d_ids = torch.from_numpy(ids.astype(np.int64)).cuda() if ids is not None else None
@@ -77,18 +79,34 @@ def test_decode_batch_matches_oracle(ctxs, name):
             assert np.array_equal(a, want[key]), f"{name}/{label}: plan array {key} differs"
 
 
-@pytest.mark.parametrize("name,budget", [("toy", 1 << 16), ("small", 1 << 17), ("medium", 1 << 16),
-                                         ("large", 1 << 13), ("sweep", 1 << 12)])
+@pytest.mark.parametrize("name,budget", [("toy", 1 << 16), ("small", 1 << 24), ("medium", 1 << 24),
+                                         ("large", 1 << 20), ("sweep", 1 << 20), ("paper_scale", 1 << 17)])
 def test_search_matches_oracle_argmin(ctxs, name, budget):
+    """lgx_search against the oracle's full scan of Toy and Small (2^24) and of id prefixes of the
+    others (Medium 2^24, Large / Sweep 2^20), the oracle spread over the host cores."""
     inst, o, g = ctxs(name)
-    want_c, want_i = o.search(inst.seed, budget)
+    want_c, want_i = oracle_search_mp(name, inst.seed, budget)
     got_c, got_i = g.search(inst.seed, budget)
     assert got_i == want_i and got_c == want_c
     # a window that does not start at 0 (multi-GPU shards use these)
-    first = inst.budget - budget
-    want_c, want_i = o.search(inst.seed, budget // 4, first_id=first)
-    got_c, got_i = g.search(inst.seed, budget // 4, first_id=first)
+    first = inst.budget - budget // 16
+    want_c, want_i = oracle_search_mp(name, inst.seed, budget // 16, first_id=first)
+    got_c, got_i = g.search(inst.seed, budget // 16, first_id=first)
     assert got_i == want_i and got_c == want_c
+
+
+def test_eight_shard_windows_combine_to_one_search(ctxs):
+    """SURVEY s4 / s8(e) on one GPU: eight disjoint lgx_search_range windows (sharding.split_range), min-combined by
+    sharding.combine, equal one lgx_search over the whole range — ties and all."""
+    from paper_1909_10286_b200 import sharding
+    for name, budget in (("medium", (1 << 24) + 12345), ("toy", 1 << 16), ("sweep", 1 << 18)):
+        inst, o, g = ctxs(name)
+        whole = g.search(inst.seed, budget, first_id=77)
+        parts = []
+        for r in range(8):
+            first, n = sharding.split_range(budget, 8, r, first_id=77)
+            parts.append(g.search(inst.seed, n, first_id=first) if n else None)
+        assert sharding.combine(parts) == whole
 
 
 def test_search_equals_min_of_eval_batch_at_scale(ctxs):
@@ -185,9 +203,18 @@ def test_paper_scale_workload(ctxs):
     """NEXT row N4: the paper's own problem shape (1200 fields, 20 BPs, 7 tours; L267)."""
     inst, o, g = ctxs("paper_scale")
     n = N_ORACLE["paper_scale"]
-    want = o.eval_batch(inst.seed, first_id=0, n=n)
-    got = [t.cpu().numpy() for t in g.eval_batch(inst.seed, first_id=0, n=n)]
-    assert np.array_equal(got[3], want[3]) and np.array_equal(got[0], want[0])
+    for label, ids, first in id_sets(inst, n):
+        want = oracle_eval_mp("paper_scale", inst.seed, ids=ids, first_id=first, n=n)
+        d_ids = torch.from_numpy(ids.astype(np.int64)).cuda() if ids is not None else None
+        got = [t.cpu().numpy() for t in g.eval_batch(inst.seed, ids=d_ids, first_id=first, n=n)]
+        assert np.array_equal(got[3], want[3]), label
+        for k in range(3):
+            assert np.array_equal(got[k], want[k]), (label, k)
+    wd = o.decode_batch(inst.seed, first_id=0, n=128); gd = g.decode_batch(inst.seed, first_id=0, n=128)
+    for key in wd:
+        a_ = gd[key].cpu().numpy()
+        if a_.dtype == np.int16: a_ = a_.view(np.uint16)
+        assert np.array_equal(a_, wd[key]), key
 
 
 def test_timing_hook_and_query(ctxs):

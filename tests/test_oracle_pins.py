@@ -143,8 +143,11 @@ def test_alg2_degenerate_cases():
     moves, su, W = lgo.su_local_min([0.5, 0.49], [1, 1], cap, [0, 1, 1], 0.01)
     assert moves == 1 and list(su) == [0, 1, 0] and W == pytest.approx([0.4, 0.49], abs=1e-12)
     # HU count divides the fill-time term (eq. (6), R7)
+    # by hand: W = (0.5 - 0.01*(40-30)/4, 0 - 0.01*(20-10)/1) = (0.475, -0.1); neither 10 t unit of tour 1 brings
+    # tour 0 below -0.1 (0.5 - 0.01*20/4 = 0.45), so the largest by (capacity, unit) = unit 3 moves: (0.45, 0.0),
+    # maximum 0.475 -> 0.45, kept; then the donor is down to one SU.  With n_HU = 1 the waits would be 0.4 -> 0.3.
     moves, su, W = lgo.su_local_min([0.5, 0.0], [4, 1], np.array([10, 30, 10, 10]) * 1024, [0, 0, 1, 1], 0.01)
-    assert moves == 0 or W.max() < 0.5
+    assert moves == 1 and list(su) == [0, 0, 1, 0] and W == pytest.approx([0.45, 0.0], abs=1e-12)
     W0 = lgo.su_local_min([0.5], [4], np.array([10, 30]) * 1024, [0, 0], 0.01)[2][0]
     assert W0 == pytest.approx(0.5 - 0.01 * 10 / 4)
 
