@@ -573,7 +573,7 @@ int run_chunks(const lgx_instance *I, KernelFn ka, KernelFn kb, KParams &P, uint
                bool decode_mode, std::vector<cudaEvent_t> *evs = nullptr)
 {
   if (!ka || !kb) return LGX_EINVAL;
-  const uint64_t ta = (uint64_t)(decode_mode ? I->threads_a_dec : I->threads_a), tb = (uint64_t)I->threads_b;
+  const uint64_t ta = LGX_BLOCK_THREADS((uint64_t)(decode_mode ? I->threads_a_dec : I->threads_a)), tb = LGX_BLOCK_THREADS((uint64_t)I->threads_b);
   const size_t smem_a = (size_t)I->hdr.image_bytes + (size_t)(decode_mode ? I->a_state_dec : I->a_state) * ta;
   const size_t smem_b = (size_t)I->hdr.imagec_bytes + (size_t)I->b_state * tb;
   P.H = I->hdr; P.image = I->d_image; P.image_c = I->d_image_c;

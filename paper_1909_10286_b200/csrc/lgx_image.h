@@ -20,13 +20,16 @@
 #pragma once
 #include <stdint.h>
 
-// Dynamic shared memory of a kernel.  (The host-side single-lane emulation used by the CPU checks of the
-// kernel logic predefines this macro; the CUDA build always takes the declaration below.)
+// Dynamic shared memory of a kernel.  (tests/emu compiles the kernels for the host, single lane, to check their
+// indexing under AddressSanitizer; it predefines the three macros below.  The CUDA build always takes these defaults.)
 #ifndef LGX_DYN_SMEM
 #define LGX_DYN_SMEM(name) extern __shared__ __align__(16) uint8_t name[]
 #endif
 #ifndef LGX_LANES
 #define LGX_LANES 32u            // lanes that draw work together (a warp)
+#endif
+#ifndef LGX_BLOCK_THREADS
+#define LGX_BLOCK_THREADS(t) (t) // threads a launch of the sampling kernels uses (the host-side check of tests/emu runs one)
 #endif
 
 namespace lgx {
