@@ -422,9 +422,14 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
     M.off_xy = o;    o = align16(o + 16u * (uint32_t)(1 + nb + nf));
     M.off_dq = o;    o = align16(o + 4u * (uint32_t)nb);
     M.off_c = o;     o = align16(o + (H.imagec_bytes - H.offc_cs));
-    M.off_pos4 = o;  o = align16(o + 16u * (uint32_t)nf);
-    M.off_leg2 = o;  o = align16(o + 16u * (uint32_t)nf);
-    M.off_pre2 = o;  o = align16(o + 16u * (uint32_t)nf);
+    M.off_pfb = o;   o = align16(o + 4u * (uint32_t)nf);
+    M.off_psq = o;   o = align16(o + 4u * (uint32_t)nf);
+    M.off_phq = o;   o = align16(o + 4u * (uint32_t)nf);
+    M.off_term = o;  o = align16(o + 8u * (uint32_t)nf);
+    M.off_legx = o;  o = align16(o + 8u * (uint32_t)nf);
+    M.off_legy = o;  o = align16(o + 8u * (uint32_t)nf);
+    M.off_prex = o;  o = align16(o + 8u * (uint32_t)nf);
+    M.off_prey = o;  o = align16(o + 8u * (uint32_t)nf);
     M.off_posf = o;  o = align16(o + 2u * (uint32_t)nf);
     M.off_bp = o;    o = align16(o + 8u * (uint32_t)nb);
     M.off_bsh = o;   o = align16(o + 8u * (uint32_t)nb);

@@ -35,7 +35,7 @@ namespace cg = cooperative_groups;
 
 constexpr int      kMvThreads = 512;            // __launch_bounds__ of the move kernels
 constexpr uint32_t kNone      = 0xFFFFFFFFu;
-constexpr uint32_t kSortKeys  = 512;            // (tour pair, position bucket) keys of the worker sort
+constexpr uint32_t kSortKeys  = 1024;           // (tour pair, position bucket | BP move) keys of the worker sort
 
 // Shared-memory layout of the move kernels (byte offsets from the start of dynamic shared memory):
 //   vertex coordinates | demand quanta | tail of image C (from offc_cs) | incumbent tables | plan store | per-thread state rows
@@ -43,9 +43,15 @@ struct MvHdr {
   uint32_t off_xy;      // f64x2 [1 + n_b + n_f]  vertex coordinates: HQ, BPs, fields
   uint32_t off_dq;      // u32 [n_b]      demand quanta
   uint32_t off_c;       // tail of image C: byte x of image C (x >= offc_cs) sits at off_c + x - offc_cs
-  uint32_t off_pos4;    // u32x4 [n_f]    plan order: f | b << 16, s_q[f], h_q[f], shuttle count N under the incumbent's SU sets
-  uint32_t off_leg2;    // f64x2 [n_f]    plan order: D(predecessor on the tour or HQ, f), D(f, b)
-  uint32_t off_pre2;    // f64x2 [n_f]    plan order: the tour's running route sum / shuttle sum BEFORE this position
+  // the incumbent's positions in plan order, one array per quantity (the walks read 4 or 8 bytes per position and lane)
+  uint32_t off_pfb;     // u32 [n_f]      f | b << 16
+  uint32_t off_psq;     // u32 [n_f]      s_q[f]
+  uint32_t off_phq;     // u32 [n_f]      h_q[f]
+  uint32_t off_term;    // f64 [n_f]      N * D(f, b): the position's shuttle term under the incumbent's SU sets (N = eq. (4) count)
+  uint32_t off_legx;    // f64 [n_f]      D(predecessor on the tour or HQ, f)
+  uint32_t off_legy;    // f64 [n_f]      D(f, b)
+  uint32_t off_prex;    // f64 [n_f]      the tour's running route sum BEFORE this position
+  uint32_t off_prey;    // f64 [n_f]      the tour's running shuttle sum BEFORE this position
   uint32_t off_posf;    // u16 [n_f]      position of field f in plan order
   uint32_t off_bp;      // u32x2 [n_b]    x = start | len << 16;  y = plan index | tour << 8 | pos << 16
   uint32_t off_bsh;     // u32x2 [n_b]    S_q(b), area quanta of b's fields
@@ -196,32 +202,34 @@ __device__ void mv_encode(const MvParams &P, uint8_t *sm, const uint8_t *plan, u
     }
   }
   __syncthreads();
-  uint4 *pos4 = MV_TAB(uint4, M.off_pos4);
+  uint32_t *pfb = MV_TAB(uint32_t, M.off_pfb), *psq = MV_TAB(uint32_t, M.off_psq), *phq = MV_TAB(uint32_t, M.off_phq);
   uint16_t *posf = MV_TAB(uint16_t, M.off_posf);
   const uint2 *sh = reinterpret_cast<const uint2 *>(P.image_c + H.offc_sh);  // {s_q, h_q} per field (global, L2-resident)
   for (uint32_t f = tid; f < n_f; f += T) {
     const uint32_t b = p_fb[f];
-    const uint2 bb = bp[b];
-    const uint32_t pos = (bb.x & 0xFFFFu) + p_fp[f];
+    const uint32_t pos = (bp[b].x & 0xFFFFu) + p_fp[f];
     const uint2 q = sh[f];
-    const uint2 sn = tsn[(bb.y >> 8) & 0xFFu];
-    pos4[pos] = make_uint4(f | (b << 16), q.x, q.y, shuttle_count(q.x, sn.y, sn.x, 0xFFFFFFFFu / sn.x));
+    pfb[pos] = f | (b << 16); psq[pos] = q.x; phq[pos] = q.y;
     posf[f] = (uint16_t)pos;
   }
   __syncthreads();
-  // the two legs of every position of the incumbent (S0: one rounding per operation)
+  // the two legs of every position of the incumbent (S0: one rounding per operation) and its shuttle term
+  // N * D(f, b) under the tour's SU set (eq. (4); R4)
   const double2 *xy = MV_TAB(const double2, M.off_xy);
-  double2 *leg2 = MV_TAB(double2, M.off_leg2);
+  double *legx = MV_TAB(double, M.off_legx), *legy = MV_TAB(double, M.off_legy), *term = MV_TAB(double, M.off_term);
   for (uint32_t p = tid; p < n_f; p += T) {
-    const uint4 e = pos4[p];
-    const uint32_t f = e.x & 0xFFFFu, b = e.x >> 16;
+    const uint32_t e = pfb[p];
+    const uint32_t f = e & 0xFFFFu, b = e >> 16;
     uint32_t pred = 0u;                                                        // HQ: first field of its tour (L21)
-    if (p > 0u) { const uint4 ep = pos4[p - 1u]; if (((bp[ep.x >> 16].y ^ bp[b].y) & 0xFF00u) == 0u) pred = 1u + n_b + (ep.x & 0xFFFFu); }
-    leg2[p] = make_double2(edge_from_xy(xy, pred, 1u + n_b + f), edge_from_xy(xy, 1u + n_b + f, 1u + b));
+    if (p > 0u) { const uint32_t ep = pfb[p - 1u]; if (((bp[ep >> 16].y ^ bp[b].y) & 0xFF00u) == 0u) pred = 1u + n_b + (ep & 0xFFFFu); }
+    const double ly = edge_from_xy(xy, 1u + n_b + f, 1u + b);
+    const uint2 sn = tsn[(bp[b].y >> 8) & 0xFFu];
+    legx[p] = edge_from_xy(xy, pred, 1u + n_b + f); legy[p] = ly;
+    term[p] = __dmul_rn((double)shuttle_count(psq[p], sn.y, sn.x, 0xFFFFFFFFu / sn.x), ly);
   }
   __syncthreads();
   // per tour, one lane each: the walk of DESIGN.md S4 / S7 over the tour's positions, in order; it also leaves the
-  // running sums before every position (pre2) and the per-BP supplies, areas and mean legs
+  // running sums before every position (prex, prey) and the per-BP supplies, areas and mean legs
   uint2 *bsh = MV_TAB(uint2, M.off_bsh);
   double *bpq = MV_TAB(double, M.off_bpq);
   for (uint32_t b = tid; b < n_b; b += T) { bsh[b] = make_uint2(0u, 0u); bpq[b] = 0.0; }
@@ -229,7 +237,7 @@ __device__ void mv_encode(const MvParams &P, uint8_t *sm, const uint8_t *plan, u
   {
     const uint2 *thu = MV_TAB(const uint2, M.off_thu);
     double *tst = MV_TAB(double, M.off_tst);
-    double2 *pre2 = MV_TAB(double2, M.off_pre2);
+    double *prex = MV_TAB(double, M.off_prex), *prey = MV_TAB(double, M.off_prey);
     uint32_t *thq = MV_TAB(uint32_t, M.off_thq);
     const uint32_t n_warps = T >> 5;
     if ((tid & 31u) == 0u)
@@ -238,8 +246,9 @@ __device__ void mv_encode(const MvParams &P, uint8_t *sm, const uint8_t *plan, u
         double Lt = 0.0, sd = 0.0, sumE = 0.0, shut = 0.0;
         uint32_t Hq = 0, Sq = 0, Hb = 0, k = 0, m = 0, b_cur = kNone, f_last = 0;
         for (uint32_t p = r.x; p < r.y; ++p) {
-          const uint4 e = pos4[p]; const double2 lg = leg2[p];
-          const uint32_t b = e.x >> 16;
+          const uint32_t e = pfb[p], sq_p = psq[p], hq_p = phq[p];
+          const double lgx = legx[p], lgy = legy[p];
+          const uint32_t b = e >> 16;
           if (b != b_cur) {
             if (b_cur != kNone) {
               const double q = div_small(sd, k, rcp);
@@ -248,10 +257,10 @@ __device__ void mv_encode(const MvParams &P, uint8_t *sm, const uint8_t *plan, u
             }
             b_cur = b; sd = 0.0; Sq = 0u; Hb = 0u; k = 0u;
           }
-          pre2[p] = make_double2(Lt, shut);
-          Lt = __dadd_rn(Lt, lg.x); sd = __dadd_rn(sd, lg.y); Hq += e.z; Hb += e.z; Sq += e.y; ++k;
-          shut = __dadd_rn(shut, __dmul_rn((double)e.w, lg.y));
-          f_last = e.x & 0xFFFFu;
+          prex[p] = Lt; prey[p] = shut;
+          Lt = __dadd_rn(Lt, lgx); sd = __dadd_rn(sd, lgy); Hq += hq_p; Hb += hq_p; Sq += sq_p; ++k;
+          shut = __dadd_rn(shut, term[p]);
+          f_last = e & 0xFFFFu;
         }
         double E = 0.0;
         const double lt_open = Lt;
@@ -297,7 +306,7 @@ __device__ void mv_encode(const MvParams &P, uint8_t *sm, const uint8_t *plan, u
       const uint32_t magic = 0xFFFFFFFFu / C2;
       const uint2 r = trng[g];
       double shut = 0.0;
-      for (uint32_t p = r.x; p < r.y; ++p) shut = __dadd_rn(shut, __dmul_rn((double)shuttle_count(pos4[p].y, n2, C2, magic), leg2[p].y));
+      for (uint32_t p = r.x; p < r.y; ++p) shut = __dadd_rn(shut, __dmul_rn((double)shuttle_count(psq[p], n2, C2, magic), legy[p]));
       sv[task] = shut;
     }
   }
@@ -327,7 +336,7 @@ __device__ __forceinline__ Move mv_derive(const MvParams &P, const uint8_t *sm, 
   Move m;
   if (v < n_f) {
     const uint32_t a = MV_TAB(const uint16_t, M.off_posf)[v];
-    const uint32_t A = MV_TAB(const uint4, M.off_pos4)[a].x >> 16;
+    const uint32_t A = MV_TAB(const uint32_t, M.off_pfb)[a] >> 16;
     // §2.6 (L249): with the field->BP assignment fixed (flag bit 3) the field is reinserted into its own BP
     const uint32_t t = (H.flags & 8u) ? A : __umulhi(w1, n_b);
     const uint2 bt = bp[t], bA = bp[A];
@@ -370,16 +379,20 @@ struct EvalOut { bool feasible; double cost, path, makespan; };
 // same order, hence the same bits: integer sums (supplies, areas: eq. (2) is decided in O(1)), the mean leg of every
 // BP whose field list is unchanged, L_tour / E / T / T_wait / shuttle sum of the tours the move does not touch.  In a
 // touched tour the FP64 running sums restart from the incumbent's prefix value at the first position the move
-// changes (pre2) and only the rest of the tour is re-added in order; the mean legs of the two BPs a field move
+// changes (prex, prey) and only the rest of the tour is re-added in order; the mean legs of the two BPs a field move
 // changes are re-summed over those BPs alone; E(g) re-sums the tour's per-BP means.
 template <int MASKW, bool HB>
 __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm, const St &s, const Move &mv)
 {
   const ImgHdr &H = P.H; const MvHdr &M = P.M;
   const uint32_t n_b = H.n_b, n_t = H.n_t, n_su = H.n_su;
-  const uint4    *pos4 = MV_TAB(const uint4, M.off_pos4);
-  const double2  *leg2 = MV_TAB(const double2, M.off_leg2);
-  const double2  *pre2 = MV_TAB(const double2, M.off_pre2);
+  const uint32_t *pfb  = MV_TAB(const uint32_t, M.off_pfb);
+  const uint32_t *psq  = MV_TAB(const uint32_t, M.off_psq);
+  const double   *term = MV_TAB(const double, M.off_term);
+  const double   *legx = MV_TAB(const double, M.off_legx);
+  const double   *legy = MV_TAB(const double, M.off_legy);
+  const double   *prex = MV_TAB(const double, M.off_prex);
+  const double   *prey = MV_TAB(const double, M.off_prey);
   const uint2    *bp   = MV_TAB(const uint2, M.off_bp);
   const uint2    *bsh  = MV_TAB(const uint2, M.off_bsh);
   const double   *bpq  = MV_TAB(const double, M.off_bpq);
@@ -409,11 +422,11 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
   {
     uint32_t bad = MV_TAB(const uint32_t, M.off_misc)[0];
     if (fld) {
-      const uint4 ef = pos4[mv.a];
-      h_blk = ef.z;
+      const uint32_t sq_f = psq[mv.a];
+      h_blk = MV_TAB(const uint32_t, M.off_phq)[mv.a];
       if (A != t) {
         const uint32_t SA = bsh[A].x, ST = bsh[t].x, dA = dq[A], dT = dq[t];
-        bad = bad - (SA < dA ? 1u : 0u) - (ST < dT ? 1u : 0u) + (SA - ef.y < dA ? 1u : 0u) + (ST + ef.y < dT ? 1u : 0u);
+        bad = bad - (SA < dA ? 1u : 0u) - (ST < dT ? 1u : 0u) + (SA - sq_f < dA ? 1u : 0u) + (ST + sq_f < dT ? 1u : 0u);
       }
     } else if (nr > 0u) h_blk = bsh[A].y;
     if (bad != 0u) return out;                                                 // discarded (L186; R19)
@@ -450,13 +463,13 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
   if (nr > 0u) {
     auto into = [&](uint32_t q) -> double {
       if (q >= (uint32_t)H.n_f) return 0.0;                                    // past the last position: never reached
-      const uint32_t vf = 1u + n_b + (pos4[map_idx(q)].x & 0xFFFFu);
+      const uint32_t vf = 1u + n_b + (pfb[map_idx(q)] & 0xFFFFu);
       const bool first = (q == wb_a) || (nr > 1u && q == wb_b);                // first field of its tour: from HQ (L21)
-      const uint32_t vp = first ? 0u : 1u + n_b + (pos4[map_idx(q - 1u)].x & 0xFFFFu);
+      const uint32_t vp = first ? 0u : 1u + n_b + (pfb[map_idx(q - 1u)] & 0xFFFFu);
       return edge_from_xy(xy, vp, vf);
     };
     X1 = into(Q1); X2 = into(Q2); X3 = into(Q3);
-    if (fld) xlb = edge_from_xy(xy, 1u + n_b + (pos4[mv.a].x & 0xFFFFu), 1u + t);
+    if (fld) xlb = edge_from_xy(xy, 1u + n_b + (pfb[mv.a] & 0xFFFFu), 1u + t);
   }
 
   // ---- untouched tours: the incumbent's values
@@ -479,14 +492,25 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
     // the BP's k fields in the worker's order, straight from the incumbent's segment [start, ...): element `ra` of it is
     // skipped when the moved field left this BP, and the moved field sits at offset q when it joined it
     auto mean_leg = [&](uint32_t start, uint32_t k, bool has_rem, uint32_t ra, bool has_ins, uint32_t q) -> double {
+      // Offset i of the worker's list reads incumbent offset i - (i > q, once the field is in) + (>= ra, once it is out).
+      // ONE loop for the whole list (the lanes of a warp stay together): four table legs at a time where neither the
+      // inserted field nor the removal's shift falls among them, else one.
+      const uint32_t bq = has_ins ? q : kNone;
+      const uint32_t br = has_rem ? ra + ((has_ins && ra >= q) ? 1u : 0u) : kNone;   // first offset shifted by the removal
+      const double *lg = legy + start;
       double sd = 0.0;
-      for (uint32_t i = 0; i < k; ++i) {
-        double leg = xlb;
-        if (!(has_ins && i == q)) {
-          const uint32_t j = i - ((has_ins && i > q) ? 1u : 0u);
-          leg = leg2[start + j + ((has_rem && j >= ra) ? 1u : 0u)].y;
+      uint32_t i = 0;
+      while (i < k) {
+        const uint32_t off = (i >= br ? 1u : 0u) - ((has_ins && i > q) ? 1u : 0u);    // (mod 2^32)
+        if (i + 4u <= k && (bq - i) >= 4u && (br - i - 1u) >= 3u) {             // bq not in [i, i+4), br not in (i, i+4)
+          const double *lp = lg + (i + off);
+          const double a0 = lp[0], a1 = lp[1], a2 = lp[2], a3 = lp[3];
+          sd = __dadd_rn(sd, a0); sd = __dadd_rn(sd, a1); sd = __dadd_rn(sd, a2); sd = __dadd_rn(sd, a3);
+          i += 4u;
+        } else {
+          sd = __dadd_rn(sd, (i == bq) ? xlb : lg[i + off]);
+          ++i;
         }
-        sd = __dadd_rn(sd, leg);
       }
       return div_small(sd, k, rcp);
     };
@@ -530,29 +554,40 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
     // L_tour(g): the incumbent's running sum before the first changed position, the rest re-added in order
     const uint2 rg = trng[g];
     const uint32_t p0 = first_change(wb, we);
-    double Lt = (p0 - wb == rg.y - rg.x) ? tst[5u * n_t + g] : pre2[rg.x + (p0 - wb)].x;
+    double Lt = (p0 - wb == rg.y - rg.x) ? tst[5u * n_t + g] : prex[rg.x + (p0 - wb)];
     {
       uint32_t P1 = Q1, J1 = K1, P2 = Q2, J2 = K2, P3 = Q3, J3 = K3;
       double Y1 = X1, Y2 = X2, Y3 = X3;
       while (P1 < p0) { P1 = P2; J1 = J2; Y1 = Y2; P2 = P3; J2 = J3; Y2 = Y3; P3 = kNone; }
+      // ONE loop (the lanes of a warp stay together): eight or four table legs at a time while no breakpoint lies among
+      // them, else one step — a breakpoint's leg was computed up front
       uint32_t idx = 0, p = p0;
       while (p < we) {
-        if (p + 4u <= we && p + 4u <= P1) {                                    // four table legs, no breakpoint among them
-          const double2 *lp = leg2 + idx;
-          Lt = __dadd_rn(Lt, lp[1].x); Lt = __dadd_rn(Lt, lp[2].x); Lt = __dadd_rn(Lt, lp[3].x); Lt = __dadd_rn(Lt, lp[4].x);
+        const uint32_t room = min(we, P1) - p;                                 // positions before the next breakpoint / the end
+        if (room >= 8u) {
+          const double *lp = legx + idx + 1u;
+          const double l0 = lp[0], l1 = lp[1], l2 = lp[2], l3 = lp[3], l4 = lp[4], l5 = lp[5], l6 = lp[6], l7 = lp[7];
+          Lt = __dadd_rn(Lt, l0); Lt = __dadd_rn(Lt, l1); Lt = __dadd_rn(Lt, l2); Lt = __dadd_rn(Lt, l3);
+          Lt = __dadd_rn(Lt, l4); Lt = __dadd_rn(Lt, l5); Lt = __dadd_rn(Lt, l6); Lt = __dadd_rn(Lt, l7);
+          idx += 8u; p += 8u;
+        } else if (room >= 4u) {
+          const double *lp = legx + idx + 1u;
+          const double l0 = lp[0], l1 = lp[1], l2 = lp[2], l3 = lp[3];
+          Lt = __dadd_rn(Lt, l0); Lt = __dadd_rn(Lt, l1); Lt = __dadd_rn(Lt, l2); Lt = __dadd_rn(Lt, l3);
           idx += 4u; p += 4u;
-          continue;
-        }
-        ++idx;
-        if (p == P1) {
+        } else if (room == 0u) {
           double lh = 0.0;
           do { idx = J1; lh = Y1; P1 = P2; J1 = J2; Y1 = Y2; P2 = P3; J2 = J3; Y2 = Y3; P3 = kNone; } while (p == P1);
           Lt = __dadd_rn(Lt, lh);
-        } else Lt = __dadd_rn(Lt, leg2[idx].x);                                // field to field (L69)
-        ++p;
+          ++p;
+        } else {
+          ++idx;
+          Lt = __dadd_rn(Lt, legx[idx]);                                       // field to field (L69)
+          ++p;
+        }
       }
     }
-    if (we > wb) Lt = __dadd_rn(Lt, edge_from_xy(xy, 1u + n_b + (pos4[map_idx(we - 1u)].x & 0xFFFFu), 0u));   // back to HQ (L21; R2)
+    if (we > wb) Lt = __dadd_rn(Lt, edge_from_xy(xy, 1u + n_b + (pfb[map_idx(we - 1u)] & 0xFFFFu), 0u));   // back to HQ (L21; R2)
     const uint32_t Hq = thq[g] - ((g == mv.g1) ? h_blk : 0u) + ((g == mv.g2) ? h_blk : 0u);
     const uint2 hu = thu[g];
     const double road = __ddiv_rn(Lt, H.v_hu);
@@ -707,40 +742,47 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
     if (!recount) {                              // a touched tour under its old SU set: restart from the incumbent's prefix
       const uint2 rg = trng[g];
       const uint32_t p0 = (g == ga) ? p0_a : p0_b;
-      shut = (p0 - p == rg.y - rg.x) ? tst[4u * n_t + g] : pre2[rg.x + (p0 - p)].y;
+      shut = (p0 - p == rg.y - rg.x) ? tst[4u * n_t + g] : prey[rg.x + (p0 - p)];
       p = p0;
     }
     uint32_t P0 = p, J0 = map_idx(p), P1 = Q1, J1 = K1, P2 = Q2, J2 = K2, P3 = Q3, J3 = K3;
     while (P1 < p) { P1 = P2; J1 = J2; P2 = P3; J2 = J3; P3 = kNone; }
+    // ONE loop (the lanes of a warp stay together): table terms N * D(f,b) (tabulated under the incumbent's SU set) eight
+    // or four at a time while no breakpoint lies among them; counts re-derived where the tour's SU set changed or inside
+    // the moved block (its terms were tabulated under another tour's SU set)
     uint32_t idx = 0;
     bool inblk = false;
     while (p < pe) {
-      if (!inblk && p + 4u <= pe && p + 4u <= P0) {                            // four positions, no breakpoint among them
-        const uint4 *ep = pos4 + idx; const double2 *lp = leg2 + idx;
-        uint32_t N1 = ep[1].w, N2 = ep[2].w, N3 = ep[3].w, N4 = ep[4].w;       // tabulated under the incumbent's SU set
-        if (recount) {
-          N1 = shuttle_count(ep[1].y, n_g, C_g, magic); N2 = shuttle_count(ep[2].y, n_g, C_g, magic);
-          N3 = shuttle_count(ep[3].y, n_g, C_g, magic); N4 = shuttle_count(ep[4].y, n_g, C_g, magic);
-        }
-        shut = __dadd_rn(shut, __dmul_rn((double)N1, lp[1].y)); shut = __dadd_rn(shut, __dmul_rn((double)N2, lp[2].y));
-        shut = __dadd_rn(shut, __dmul_rn((double)N3, lp[3].y)); shut = __dadd_rn(shut, __dmul_rn((double)N4, lp[4].y));
-        idx += 4u; p += 4u;
+      const uint32_t room = min(pe, P0) - p;
+      if (room == 0u) {                          // a breakpoint: position p reads incumbent index J0
+        do { idx = J0; P0 = P1; J0 = J1; P1 = P2; J1 = J2; P2 = P3; J2 = J3; P3 = kNone; } while (p == P0);
+        inblk = (p - mv.c) < L;
         continue;
       }
-      ++idx;
-      if (p == P0) {
-        do { idx = J0; P0 = P1; J0 = J1; P1 = P2; J1 = J2; P2 = P3; J2 = J3; P3 = kNone; } while (p == P0);
-        inblk = (p - mv.c) < L;                  // the moved block's counts were tabulated under another tour's SU set
+      const bool rc = recount || inblk;
+      if (!rc && room >= 8u) {
+        const double *tp = term + idx;
+        const double t0 = tp[0], t1 = tp[1], t2 = tp[2], t3 = tp[3], t4 = tp[4], t5 = tp[5], t6 = tp[6], t7 = tp[7];
+        shut = __dadd_rn(shut, t0); shut = __dadd_rn(shut, t1); shut = __dadd_rn(shut, t2); shut = __dadd_rn(shut, t3);
+        shut = __dadd_rn(shut, t4); shut = __dadd_rn(shut, t5); shut = __dadd_rn(shut, t6); shut = __dadd_rn(shut, t7);
+        idx += 8u; p += 8u;
+      } else if (!rc && room >= 4u) {
+        const double *tp = term + idx;
+        const double t0 = tp[0], t1 = tp[1], t2 = tp[2], t3 = tp[3];
+        shut = __dadd_rn(shut, t0); shut = __dadd_rn(shut, t1); shut = __dadd_rn(shut, t2); shut = __dadd_rn(shut, t3);
+        idx += 4u; p += 4u;
+      } else if (rc && room >= 4u && !(inblk && fld)) {
+        const uint32_t *sp = psq + idx; const double *lp = legy + idx;
+        const double t0 = __dmul_rn((double)shuttle_count(sp[0], n_g, C_g, magic), lp[0]), t1 = __dmul_rn((double)shuttle_count(sp[1], n_g, C_g, magic), lp[1]);
+        const double t2 = __dmul_rn((double)shuttle_count(sp[2], n_g, C_g, magic), lp[2]), t3 = __dmul_rn((double)shuttle_count(sp[3], n_g, C_g, magic), lp[3]);
+        shut = __dadd_rn(shut, t0); shut = __dadd_rn(shut, t1); shut = __dadd_rn(shut, t2); shut = __dadd_rn(shut, t3);
+        idx += 4u; p += 4u;
+      } else {
+        double tm = term[idx];
+        if (rc) tm = __dmul_rn((double)shuttle_count(psq[idx], n_g, C_g, magic), (inblk && fld) ? xlb : legy[idx]);
+        shut = __dadd_rn(shut, tm);
+        ++idx; ++p;
       }
-      const uint4 en = pos4[idx];
-      double leg = leg2[idx].y;
-      uint32_t N = en.w;
-      if (recount || inblk) {
-        if (inblk && fld) leg = xlb;
-        N = shuttle_count(en.y, n_g, C_g, magic);
-      }
-      shut = __dadd_rn(shut, __dmul_rn((double)N, leg));
-      ++p;
     }
     s.d(M.m64_w + g) = shut;
   }
@@ -796,10 +838,13 @@ __device__ __forceinline__ void mv_for_workers(const MvParams &P, uint8_t *sm, u
   // key = (unordered pair of touched tours, bucket of the first changed position inside the lower tour): lanes of a
   // warp then share the tours AND roughly the point from which their running sums must be re-added
   const uint32_t n_pairs = n_t * (n_t + 1u) / 2u;
+  // A BP move re-derives the shuttle counts of the whole moved block (its terms were tabulated under another tour's SU
+  // set): such workers get keys of their own so that they share warps — the lowest keys: the warps draw the sorted
+  // chunks in order, so the longest jobs start first.
   uint32_t nbk = 1u;
-  while (nbk < 16u && n_pairs * nbk * 2u <= kSortKeys) nbk *= 2u;
-  const bool by_pair = n_pairs <= kSortKeys;
-  const uint32_t nk = by_pair ? n_pairs * nbk : n_t;
+  while (nbk < 16u && n_pairs * (nbk * 2u + 1u) <= kSortKeys) nbk *= 2u;
+  const bool by_pair = n_pairs * 2u <= kSortKeys;
+  const uint32_t nk = by_pair ? n_pairs * (nbk + 1u) : 2u * n_t;
   const uint2 *trng = MV_TAB(const uint2, P.M.off_trng);
   uint32_t *hist = MV_TAB(uint32_t, P.M.off_sort);       // [nk + 2]: offsets per key, total, the warps' draw counter
   uint16_t *order = MV_TAB(uint16_t, P.M.off_order);
@@ -824,8 +869,9 @@ __device__ __forceinline__ void mv_for_workers(const MvParams &P, uint8_t *sm, u
           const uint32_t pos = (mv.g1 == mv.g2) ? min(mv.a, mv.c) : ((mv.g1 == ga) ? mv.a : mv.c);
           const uint32_t rel = pos > rg.x ? pos - rg.x : 0u;
           const uint32_t bk = min(nbk - 1u, rel * nbk / (rg.y - rg.x + 1u));
-          key[r] = (ga * (2u * n_t - ga + 1u) / 2u + (gb - ga)) * nbk + bk;
-        } else key[r] = ga;
+          const uint32_t pair = ga * (2u * n_t - ga + 1u) / 2u + (gb - ga);
+          key[r] = (mv.fld_b == kNone) ? pair : n_pairs + pair * nbk + bk;
+        } else key[r] = ga + ((mv.fld_b == kNone) ? 0u : n_t);
         rank[r] = atomicAdd(&hist[key[r]], 1u);
       }
     }
