@@ -103,18 +103,6 @@ struct MvParams {
 #define MV_TAB(type, off) (reinterpret_cast<type *>(sm + (off)))
 #define MV_CTAB(type, offc) (reinterpret_cast<const type *>(sm + (P.M.off_c + ((offc) - P.H.offc_cs))))
 
-// eq. (4) (L89) with the tour's mean capacity (R4): N = ceil(s_q n_g / C_g) = floor(x'/C_g), x' = s_q n_g + C_g - 1 < 2^32;
-// q = mulhi(x', floor((2^32-1)/C_g)) is at most 2 below; two conditional increments fix it.
-__device__ __forceinline__ uint32_t shuttle_count(uint32_t s_q, uint32_t n_g, uint32_t C_g, uint32_t magic)
-{
-  const uint32_t xq = s_q * n_g + (C_g - 1u);
-  uint32_t N = __umulhi(xq, magic);
-  uint32_t rem = xq - N * C_g;
-  if (rem >= C_g) { ++N; rem -= C_g; }
-  if (rem >= C_g) { ++N; }
-  return N;
-}
-
 // ------------------------------------------------------------------ plan -> shared memory
 
 // Copy the plan arrays from global memory into a plan slot; SU sets become masks over capacity ranks.
