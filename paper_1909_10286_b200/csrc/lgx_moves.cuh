@@ -520,7 +520,8 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
 
   // ---- S4 for the touched tours (L69, L106, L213)
   double lt_a = 0.0, lt_b = 0.0, E_a = 0.0, E_b = 0.0, road_a = 0.0, road_b = 0.0;
-  uint32_t p0_a = 0, p0_b = 0, hq_a = 0, hq_b = 0;
+  uint32_t hq_a = 0, hq_b = 0;
+  double sh_a = 0.0, sh_b = 0.0;          // the touched tours' shuttle sums IF Algorithm 2 leaves their SU sets alone
   for (uint32_t r = 0; r < nr; ++r) {
     const uint32_t g = r ? gb : ga;
     const uint32_t wb = r ? wb_b : wb_a, we = r ? we_b : we_a;
@@ -542,36 +543,55 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
     // L_tour(g): the incumbent's running sum before the first changed position, the rest re-added in order
     const uint2 rg = trng[g];
     const uint32_t p0 = first_change(wb, we);
-    double Lt = (p0 - wb == rg.y - rg.x) ? tst[5u * n_t + g] : prex[rg.x + (p0 - wb)];
+    const bool at_end = (p0 - wb == rg.y - rg.x);
+    double Lt = at_end ? tst[5u * n_t + g] : prex[rg.x + (p0 - wb)];
+    // ... and, in the same walk, the tour's shuttle sum under the incumbent's SU set (a second, independent chain of
+    // additions): table terms N * D(f,b); inside the moved block — tabulated under another tour's SU set, and a moved
+    // field has a new BP — the count is re-derived.  Pass 2 below takes it if Algorithm 2 left this tour's set alone.
+    double sh = at_end ? tst[4u * n_t + g] : prey[rg.x + (p0 - wb)];
     {
+      const uint2 sn_g = tsn[g];
+      const uint32_t magic_g = 0xFFFFFFFFu / sn_g.x;
       uint32_t P1 = Q1, J1 = K1, P2 = Q2, J2 = K2, P3 = Q3, J3 = K3;
       double Y1 = X1, Y2 = X2, Y3 = X3;
       while (P1 < p0) { P1 = P2; J1 = J2; Y1 = Y2; P2 = P3; J2 = J3; Y2 = Y3; P3 = kNone; }
-      // ONE loop (the lanes of a warp stay together): eight or four table legs at a time while no breakpoint lies among
-      // them, else one step — a breakpoint's leg was computed up front
-      uint32_t idx = 0, p = p0;
+      // ONE loop (the lanes of a warp stay together): eight or four positions at a time while no breakpoint lies among
+      // them, else one — a breakpoint's route leg was computed up front.  cur = incumbent index of position p.
+      uint32_t cur = 0, p = p0;
+      bool inblk = false;
       while (p < we) {
         const uint32_t room = min(we, P1) - p;                                 // positions before the next breakpoint / the end
-        if (room >= 8u) {
-          const double *lp = legx + idx + 1u;
+        if (room >= 8u && !inblk) {
+          const double *lp = legx + cur, *tp = term + cur;
           const double l0 = lp[0], l1 = lp[1], l2 = lp[2], l3 = lp[3], l4 = lp[4], l5 = lp[5], l6 = lp[6], l7 = lp[7];
-          Lt = __dadd_rn(Lt, l0); Lt = __dadd_rn(Lt, l1); Lt = __dadd_rn(Lt, l2); Lt = __dadd_rn(Lt, l3);
-          Lt = __dadd_rn(Lt, l4); Lt = __dadd_rn(Lt, l5); Lt = __dadd_rn(Lt, l6); Lt = __dadd_rn(Lt, l7);
-          idx += 8u; p += 8u;
-        } else if (room >= 4u) {
-          const double *lp = legx + idx + 1u;
+          const double t0 = tp[0], t1 = tp[1], t2 = tp[2], t3 = tp[3], t4 = tp[4], t5 = tp[5], t6 = tp[6], t7 = tp[7];
+          Lt = __dadd_rn(Lt, l0); sh = __dadd_rn(sh, t0); Lt = __dadd_rn(Lt, l1); sh = __dadd_rn(sh, t1);
+          Lt = __dadd_rn(Lt, l2); sh = __dadd_rn(sh, t2); Lt = __dadd_rn(Lt, l3); sh = __dadd_rn(sh, t3);
+          Lt = __dadd_rn(Lt, l4); sh = __dadd_rn(sh, t4); Lt = __dadd_rn(Lt, l5); sh = __dadd_rn(sh, t5);
+          Lt = __dadd_rn(Lt, l6); sh = __dadd_rn(sh, t6); Lt = __dadd_rn(Lt, l7); sh = __dadd_rn(sh, t7);
+          cur += 8u; p += 8u;
+        } else if (room >= 4u && !(inblk && fld)) {
+          const double *lp = legx + cur;
           const double l0 = lp[0], l1 = lp[1], l2 = lp[2], l3 = lp[3];
-          Lt = __dadd_rn(Lt, l0); Lt = __dadd_rn(Lt, l1); Lt = __dadd_rn(Lt, l2); Lt = __dadd_rn(Lt, l3);
-          idx += 4u; p += 4u;
-        } else if (room == 0u) {
-          double lh = 0.0;
-          do { idx = J1; lh = Y1; P1 = P2; J1 = J2; Y1 = Y2; P2 = P3; J2 = J3; Y2 = Y3; P3 = kNone; } while (p == P1);
-          Lt = __dadd_rn(Lt, lh);
-          ++p;
+          double t0, t1, t2, t3;
+          if (inblk) {
+            const uint32_t *sp = psq + cur; const double *yp = legy + cur;
+            t0 = __dmul_rn((double)shuttle_count(sp[0], sn_g.y, sn_g.x, magic_g), yp[0]); t1 = __dmul_rn((double)shuttle_count(sp[1], sn_g.y, sn_g.x, magic_g), yp[1]);
+            t2 = __dmul_rn((double)shuttle_count(sp[2], sn_g.y, sn_g.x, magic_g), yp[2]); t3 = __dmul_rn((double)shuttle_count(sp[3], sn_g.y, sn_g.x, magic_g), yp[3]);
+          } else { const double *tp = term + cur; t0 = tp[0]; t1 = tp[1]; t2 = tp[2]; t3 = tp[3]; }
+          Lt = __dadd_rn(Lt, l0); sh = __dadd_rn(sh, t0); Lt = __dadd_rn(Lt, l1); sh = __dadd_rn(sh, t1);
+          Lt = __dadd_rn(Lt, l2); sh = __dadd_rn(sh, t2); Lt = __dadd_rn(Lt, l3); sh = __dadd_rn(sh, t3);
+          cur += 4u; p += 4u;
         } else {
-          ++idx;
-          Lt = __dadd_rn(Lt, legx[idx]);                                       // field to field (L69)
-          ++p;
+          double lh;
+          if (room == 0u) {
+            do { cur = J1; lh = Y1; P1 = P2; J1 = J2; Y1 = Y2; P2 = P3; J2 = J3; Y2 = Y3; P3 = kNone; } while (p == P1);
+            inblk = (p - mv.c) < L;
+          } else lh = legx[cur];                                               // field to field (L69)
+          double tm = term[cur];
+          if (inblk) tm = __dmul_rn((double)shuttle_count(psq[cur], sn_g.y, sn_g.x, magic_g), fld ? xlb : legy[cur]);
+          Lt = __dadd_rn(Lt, lh); sh = __dadd_rn(sh, tm);
+          ++cur; ++p;
         }
       }
     }
@@ -584,7 +604,7 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
     if (HB) s.d(M.m64_t + g) = t_g;
     const Mask<MASKW> mk = mask_load<MASKW>(s, M.m64_mask + MASKW * g);
     s.d(M.m64_w + g) = wait_time(E, tsn[g].x, cs[mask_top(mk)], hu.x, H.kappa, rcp);
-    if (r == 0u) { lt_a = Lt; E_a = E; p0_a = p0; road_a = road; hq_a = Hq; } else { lt_b = Lt; E_b = E; p0_b = p0; road_b = road; hq_b = Hq; }
+    if (r == 0u) { lt_a = Lt; E_a = E; sh_a = sh; road_a = road; hq_a = Hq; } else { lt_b = Lt; E_b = E; sh_b = sh; road_b = road; hq_b = Hq; }
   }
   auto E_of  = [&](uint32_t g) -> double { return g == ga ? E_a : (g == gb ? E_b : tst[n_t + g]); };
   auto lt_of = [&](uint32_t g) -> double { return g == ga ? lt_a : (g == gb ? lt_b : tst[g]); };
@@ -703,7 +723,10 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
   for (uint32_t g = 0; g < n_t; ++g) {
     const uint2 sn = tsn[g];
     const bool same = (s.w(M.m32_s + g) == sn.x) && ((uint32_t)mask_count(mask_load<MASKW>(s, M.m64_mask + MASKW * g)) == sn.y);
-    if (g == ga || g == gb) { need |= 1ull << g; continue; }
+    if (g == ga || g == gb) {                  // a touched tour: its sum under the old SU set came with the route walk
+      if (same) s.d(M.m64_w + g) = (g == ga) ? sh_a : sh_b; else need |= 1ull << g;
+      continue;
+    }
     if (same) { s.d(M.m64_w + g) = tst[4u * n_t + g]; continue; }
     // an untouched tour one SU away from the incumbent's set: tabulated (mv_encode)
     const uint32_t C2 = s.w(M.m32_s + g), n2 = (uint32_t)mask_count(mask_load<MASKW>(s, M.m64_mask + MASKW * g));
@@ -722,22 +745,13 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
     need &= need - 1ull;
     const uint32_t C_g = s.w(M.m32_s + g), n_g = (uint32_t)mask_count(mask_load<MASKW>(s, M.m64_mask + MASKW * g));
     const uint32_t magic = 0xFFFFFFFFu / C_g;
-    const uint2 sn = tsn[g];
-    const bool recount = !(C_g == sn.x && n_g == sn.y);
+    // every tour that gets here has a changed SU set: all its counts are re-derived, from the tour's first position
     uint32_t p, pe;
     wrange(g, p, pe);
     double shut = 0.0;
-    if (!recount) {                              // a touched tour under its old SU set: restart from the incumbent's prefix
-      const uint2 rg = trng[g];
-      const uint32_t p0 = (g == ga) ? p0_a : p0_b;
-      shut = (p0 - p == rg.y - rg.x) ? tst[4u * n_t + g] : prey[rg.x + (p0 - p)];
-      p = p0;
-    }
     uint32_t P0 = p, J0 = map_idx(p), P1 = Q1, J1 = K1, P2 = Q2, J2 = K2, P3 = Q3, J3 = K3;
     while (P1 < p) { P1 = P2; J1 = J2; P2 = P3; J2 = J3; P3 = kNone; }
-    // ONE loop (the lanes of a warp stay together): table terms N * D(f,b) (tabulated under the incumbent's SU set) eight
-    // or four at a time while no breakpoint lies among them; counts re-derived where the tour's SU set changed or inside
-    // the moved block (its terms were tabulated under another tour's SU set)
+    // ONE loop (the lanes of a warp stay together), four positions at a time while no breakpoint lies among them
     uint32_t idx = 0;
     bool inblk = false;
     while (p < pe) {
@@ -747,28 +761,14 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
         inblk = (p - mv.c) < L;
         continue;
       }
-      const bool rc = recount || inblk;
-      if (!rc && room >= 8u) {
-        const double *tp = term + idx;
-        const double t0 = tp[0], t1 = tp[1], t2 = tp[2], t3 = tp[3], t4 = tp[4], t5 = tp[5], t6 = tp[6], t7 = tp[7];
-        shut = __dadd_rn(shut, t0); shut = __dadd_rn(shut, t1); shut = __dadd_rn(shut, t2); shut = __dadd_rn(shut, t3);
-        shut = __dadd_rn(shut, t4); shut = __dadd_rn(shut, t5); shut = __dadd_rn(shut, t6); shut = __dadd_rn(shut, t7);
-        idx += 8u; p += 8u;
-      } else if (!rc && room >= 4u) {
-        const double *tp = term + idx;
-        const double t0 = tp[0], t1 = tp[1], t2 = tp[2], t3 = tp[3];
-        shut = __dadd_rn(shut, t0); shut = __dadd_rn(shut, t1); shut = __dadd_rn(shut, t2); shut = __dadd_rn(shut, t3);
-        idx += 4u; p += 4u;
-      } else if (rc && room >= 4u && !(inblk && fld)) {
+      if (room >= 4u && !(inblk && fld)) {
         const uint32_t *sp = psq + idx; const double *lp = legy + idx;
         const double t0 = __dmul_rn((double)shuttle_count(sp[0], n_g, C_g, magic), lp[0]), t1 = __dmul_rn((double)shuttle_count(sp[1], n_g, C_g, magic), lp[1]);
         const double t2 = __dmul_rn((double)shuttle_count(sp[2], n_g, C_g, magic), lp[2]), t3 = __dmul_rn((double)shuttle_count(sp[3], n_g, C_g, magic), lp[3]);
         shut = __dadd_rn(shut, t0); shut = __dadd_rn(shut, t1); shut = __dadd_rn(shut, t2); shut = __dadd_rn(shut, t3);
         idx += 4u; p += 4u;
       } else {
-        double tm = term[idx];
-        if (rc) tm = __dmul_rn((double)shuttle_count(psq[idx], n_g, C_g, magic), (inblk && fld) ? xlb : legy[idx]);
-        shut = __dadd_rn(shut, tm);
+        shut = __dadd_rn(shut, __dmul_rn((double)shuttle_count(psq[idx], n_g, C_g, magic), (inblk && fld) ? xlb : legy[idx]));
         ++idx; ++p;
       }
     }
