@@ -9,10 +9,12 @@
  * argmin (L167).  DESIGN.md states every reading (R1..R30) the paper leaves open.
  *
  * Conventions
- *  - extern "C", no exceptions.  Return 0 (LGX_OK) or a negative code.  No process-wide state: the library
- *    reads no environment variables; every tuning knob is a flag of the descriptor or an lgx_instance_set_option
- *    key; the only per-function CUDA state (the opt-in shared-memory size of a kernel) is set once, to the device
- *    maximum, when an instance that uses the kernel is created.
+ *  - extern "C", no exceptions.  Return 0 (LGX_OK) or a negative code.  The library reads no environment
+ *    variables; every tuning knob is a flag of the descriptor or an lgx_instance_set_option key.  Process-wide
+ *    state, all of it result-neutral: the opt-in shared-memory size of a kernel (set once, to the device maximum,
+ *    when an instance that uses the kernel is created) and ONE cached workspace pool per device (the queue of
+ *    feasible candidates is allocated stream-ordered from it and stays mapped between calls and instances;
+ *    lgx_workspace_trim releases it).
  *  - Every compute call must run with the CUDA device the instance was created on as the current device
  *    (its images live there): otherwise LGX_EINVAL.
  *  - "d_" pointers are DEVICE pointers (caller-allocated, e.g. torch tensors' data_ptr());
@@ -101,6 +103,10 @@ typedef struct {
  * 227 KB of shared memory), LGX_ECUDA, LGX_ENOMEM.                                          */
 int lgx_instance_create (const lgx_instance_desc *desc, lgx_instance **out);
 int lgx_instance_destroy(lgx_instance *inst);
+
+/* Hands the workspace memory the library caches per device (see Conventions) back to the driver.  Safe at any
+ * time no compute call is in flight; the next compute call maps what it needs again.  LGX_OK or LGX_ECUDA.    */
+int lgx_workspace_trim(void);
 
 /* Candidate decoder + tour simulator + demand check + Algorithm 2 + cost (a2..a6), one
  * candidate per thread.  ids: d_ids[i] if d_ids != NULL, else first_id + i.  Row i of every

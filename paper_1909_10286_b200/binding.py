@@ -40,7 +40,7 @@ class lgx_instance_desc(C.Structure):
 
 EXPORTS = ("lgx_instance_create", "lgx_instance_destroy", "lgx_eval_batch", "lgx_eval_batch_host",
            "lgx_search_range", "lgx_search", "lgx_decode_batch", "lgx_instance_query", "lgx_instance_set_timing",
-           "lgx_instance_set_option", "lgx_selftest",
+           "lgx_instance_set_option", "lgx_selftest", "lgx_workspace_trim",
            "lgx_init_plan", "lgx_move_eval_batch", "lgx_local_search", "lgx_strerror")
 
 _lib = None
@@ -142,6 +142,11 @@ def selftest(what: int, n: int, seed: int = 0):
     out = (C.c_uint64 * 2)()
     _check(load().lgx_selftest(what, n, seed, out))
     return int(out[0]), int(out[1])
+
+
+def workspace_trim():
+    """lgx_workspace_trim: release the workspace memory the library caches per device."""
+    _check(load().lgx_workspace_trim())
 
 
 class Instance:

@@ -15,6 +15,7 @@
 #include <new>
 #include <numeric>
 #include <string>
+#include <mutex>
 #include <vector>
 
 using namespace lgx;
@@ -31,7 +32,7 @@ struct lgx_instance {
   int threads_a = 0, threads_a_dec = 0, threads_b = 0, grid = 0;
   uint64_t a_state = 0, a_state_dec = 0, b_state = 0;   // per-candidate shared-memory bytes
   uint64_t chunk = 0;                          // candidates per decode/finish kernel pair
-  cudaMemPool_t pool = nullptr;                // stream-ordered workspace allocations of this instance
+  cudaMemPool_t pool = nullptr;                // the device's workspace pool (owned by the library, not by the instance)
   mutable std::atomic<long long> launches{0};
   // optional per-kernel timing (lgx_instance_set_timing): CUDA events around every launch of a search
   mutable std::atomic<int> timing{0};
@@ -118,12 +119,39 @@ int64_t fit_threads(int64_t budget, int64_t image, int64_t state, int64_t cap)
   return std::min<int64_t>(t, cap) / 32 * 32;
 }
 
+// Stream-ordered workspace memory (the queue of feasible candidates, a few hundred bytes of counters) comes from ONE
+// memory pool per device, created on first use and kept for the life of the process with its release threshold at the
+// maximum: a freed workspace stays mapped, so creating an instance and searching with it does not pay for mapping
+// the queue again (measured: ~150 ms per 2 GiB).  lgx_workspace_trim() hands the cached memory back.
+constexpr int kMaxDevices = 64;
+std::mutex g_pool_mutex;
+cudaMemPool_t g_pools[kMaxDevices] = {};
+
+int device_pool(int device, cudaMemPool_t *out)
+{
+  if (device < 0 || device >= kMaxDevices) return LGX_EINVAL;
+  std::lock_guard<std::mutex> lock(g_pool_mutex);
+  if (!g_pools[device]) {
+    cudaMemPoolProps props{};
+    props.allocType = cudaMemAllocationTypePinned;
+    props.handleTypes = cudaMemHandleTypeNone;
+    props.location.type = cudaMemLocationTypeDevice;
+    props.location.id = device;
+    cudaMemPool_t pool = nullptr;
+    CU(cudaMemPoolCreate(&pool, &props));
+    uint64_t keep = ~0ull;
+    cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    g_pools[device] = pool;
+  }
+  *out = g_pools[device];
+  return LGX_OK;
+}
+
 void free_instance(lgx_instance *I)
 {
   if (I->d_xy) cudaFree(I->d_xy);
   if (I->d_image) cudaFree(I->d_image);
   if (I->d_image_c) cudaFree(I->d_image_c);
-  if (I->pool) cudaMemPoolDestroy(I->pool);
   delete I;
 }
 
@@ -394,17 +422,8 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   }
   if ((e = cudaMalloc((void **)&I->d_image_c, H.imagec_bytes)) != cudaSuccess) { free_instance(I); return cuda_fail(e, "cudaMalloc(image C)"); }
   if ((e = cudaMemcpy(I->d_image_c, imc, H.imagec_bytes, cudaMemcpyHostToDevice)) != cudaSuccess) { free_instance(I); return cuda_fail(e, "cudaMemcpy(image C)"); }
-  {
-    // workspaces come from a pool of this instance that keeps its memory between calls
-    cudaMemPoolProps props{};
-    props.allocType = cudaMemAllocationTypePinned;
-    props.handleTypes = cudaMemHandleTypeNone;
-    props.location.type = cudaMemLocationTypeDevice;
-    props.location.id = I->device;
-    if ((e = cudaMemPoolCreate(&I->pool, &props)) != cudaSuccess) { I->pool = nullptr; free_instance(I); return cuda_fail(e, "cudaMemPoolCreate"); }
-    uint64_t keep = ~0ull;
-    cudaMemPoolSetAttribute(I->pool, cudaMemPoolAttrReleaseThreshold, &keep);
-  }
+  // workspaces come from the library's per-device pool, which keeps its memory between calls and between instances
+  if ((rc = device_pool(I->device, &I->pool)) != LGX_OK) { I->pool = nullptr; free_instance(I); return rc; }
   {
     KernelFn ka, kb;
     pick_kernels<MODE_EVAL>(H, ka, kb);
@@ -494,6 +513,14 @@ int lgx_instance_destroy(lgx_instance *I)
 {
   if (!I) return LGX_EINVAL;
   free_instance(I);
+  return LGX_OK;
+}
+
+int lgx_workspace_trim(void)
+{
+  std::lock_guard<std::mutex> lock(g_pool_mutex);
+  for (int dev = 0; dev < kMaxDevices; ++dev)
+    if (g_pools[dev]) CU(cudaMemPoolTrimTo(g_pools[dev], 0));
   return LGX_OK;
 }
 
