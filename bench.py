@@ -60,6 +60,11 @@ SM_MAX_MHZ_FALLBACK = 1965.0
 # with the candidates that launch covered.  The path's algorithmic HBM bytes are 0 per candidate in lgx_search
 # (everything lives in shared memory and the L2-resident queue); these numbers show the real traffic is negligible.
 TRAFFIC = {
+    # name: (capture, candidates the captured kernel pair covered, bytes of lgx_decode_cut, bytes of lgx_walk_finish)
+    "medium":      ("profiles/r02_medium_ncu_full.md", 16777216, 4.409e8, 4.995e8),
+    "large":       ("profiles/r02_large_ncu_full.md", 932068, 1.784e8, 2.390e8),
+    "sweep":       ("profiles/r02_sweep_ncu_full.md", 1973790, 2.088e9, 2.252e9),
+    "paper_scale": ("profiles/r02_paper_scale_ncu_full.md", 860370, 2.086e9, 4.059e9),
 }
 
 
@@ -421,11 +426,15 @@ def main():
         ach_r1 = (w_dw + feas * w_fin) * rate_per_gpu / 1e9
         ach_strict = (w_a + feas * w_b) * rate_per_gpu / 1e9
         tr = TRAFFIC.get(name)
+        if tr:      # the dominant kernel's bytes, scaled from the captured launch to this run's candidates per launch
+            tr = {"file": tr[0], "candidates_per_launch": tr[1], "bytes_per_launch": (tr[2] if a_dominant else tr[3]) * per_launch / tr[1]}
         return {"bound": "alu",
                 "kernel": "%s (dominant: %.0f %% of the kernel time of a step)" % ("lgx_decode_cut" if a_dominant else "lgx_walk_finish", 100.0 * max(ns_a_, ns_b_) / max(ns_a_ + ns_b_, 1)),
                 "achieved": ach_d, "peak": peak_ginst, "unit": "G thread-inst/s", "frac": ach_d / peak_ginst if ach_d else None,
                 "traffic": tr["bytes_per_launch"] if tr else None,
-                "traffic_source": ("profile constant: %s, %d candidates per launch" % (tr["file"], tr["candidates_per_launch"])) if tr else None,
+                "traffic_source": ("profile constant, not measured in this run: dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel in %s "
+                                   "(%d candidates in the captured launch), scaled to this run's candidates per launch; it is the queue of "
+                                   "feasible candidates, the path's algorithmic HBM bytes are 0" % (tr["file"], tr["candidates_per_launch"])) if tr else None,
                 "launch_ms": ms_d, "launches_timed": pairs, "candidates_per_launch": per_launch,
                 "work_model": "w_alg (bench.py; DESIGN.md s8): a hand model of the thread-instructions the method needs, not a measured count; "
                               "A2 = mean accepted Algorithm-2 moves, oracle-measured in this run",

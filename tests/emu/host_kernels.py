@@ -168,6 +168,11 @@ def main():
         z = replace(z, field_xy=z.field_xy[:nf].copy(), field_supply_t=z.field_supply_t[:nf].copy(), field_area_ha=z.field_area_ha[:nf].copy(),
                     bp_demand_t=z.bp_demand_t * (z.field_supply_t[:nf].sum() / z.field_supply_t.sum()))
         ok &= check(z, 128, f"sweep/nf={nf}", seed=5)
+    for nf in (510, 511, 512, 513, 514, 515, 1022, 1023, 1024, 1025):     # 16-bit field ids around 512 and 1024, every padding and tail length of the blocked Fisher-Yates steps
+        z = wl.make("paper_scale")
+        z = replace(z, field_xy=z.field_xy[:nf].copy(), field_supply_t=z.field_supply_t[:nf].copy(), field_area_ha=z.field_area_ha[:nf].copy(),
+                    bp_demand_t=z.bp_demand_t * (0.9 * z.field_supply_t[:nf].sum() / z.bp_demand_t.sum()))
+        ok &= check(z, 96, f"paper_scale/nf={nf}", seed=6)
     inst = wl.make("small")
     ids = np.array([(1 << 40) + 3, (1 << 63) + 11, 2**64 - 1], dtype=np.uint64)
     ok &= check(inst, 3, "small/bigids", seed=0xDEADBEEFCAFEF00D, ids=ids)

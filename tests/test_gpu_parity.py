@@ -302,3 +302,52 @@ def test_distance_modes_agree(ctxs, mode):
         got = [t.cpu().numpy() for t in g2.eval_batch(inst.seed, first_id=0, n=4096)]
         assert np.array_equal(got[3], want[3]) and np.array_equal(got[0], want[0])
         assert g2.search(inst.seed, 4096) == o.search(inst.seed, 4096)
+
+
+def test_workspace_pool_is_shared_and_trimmable(ctxs):
+    """The queue of feasible candidates comes from ONE cached pool per device (include/lgx.h, Conventions): a second
+    instance, an instance created after the first was destroyed, and calls after lgx_workspace_trim all give the same
+    results; trimming is legal whenever no call is in flight."""
+    inst, o, g = ctxs("small")
+    n = 1 << 16
+    ref = g.search(inst.seed, n)
+    assert ref == o.search(inst.seed, n)
+    g2 = binding.Instance(inst)
+    assert g2.search(inst.seed, n) == ref
+    g2.close()
+    torch.cuda.synchronize()
+    binding.workspace_trim()
+    g3 = binding.Instance(inst)
+    assert g3.search(inst.seed, n) == ref and g.search(inst.seed, n) == ref
+    g3.close()
+    binding.workspace_trim(); binding.workspace_trim()
+    got = g.eval_batch(inst.seed, first_id=5, n=1000)
+    want = o.eval_batch(inst.seed, first_id=5, n=1000)
+    assert np.array_equal(got[3].cpu().numpy(), want[3]) and np.array_equal(got[0].cpu().numpy(), want[0])
+
+
+@pytest.mark.parametrize("nf", [253, 255, 256, 257, 258, 259, 510, 511, 512, 513, 1022, 1023, 1024, 1025, 1026, 1027])
+def test_field_count_boundaries(nf):
+    """Field counts around the 8-bit / 16-bit switch of the Fisher-Yates array (255 | 256) and around 512 and 1024, for
+    every padding of the right-aligned words (and every length of the last, partial block of four steps): plans,
+    flags, costs and the argmin against the oracle."""
+    from dataclasses import replace
+    z = wl.make("paper_scale")
+    z = replace(z, field_xy=z.field_xy[:nf].copy(), field_supply_t=z.field_supply_t[:nf].copy(), field_area_ha=z.field_area_ha[:nf].copy(),
+                bp_demand_t=z.bp_demand_t * (0.9 * z.field_supply_t[:nf].sum() / z.bp_demand_t.sum()))
+    o, g = lgo.Oracle(z), binding.Instance(z)
+    n = 512
+    want = o.eval_batch(6, first_id=0, n=n)
+    got = [t.cpu().numpy() for t in g.eval_batch(6, first_id=0, n=n)]
+    assert np.array_equal(got[3], want[3])
+    for k in range(3):
+        assert_costs(got[k], want[k], f"nf={nf} output {k}")
+    wd = o.decode_batch(6, first_id=0, n=128); gd = g.decode_batch(6, first_id=0, n=128)
+    for key in wd:
+        a_ = gd[key].cpu().numpy()
+        if a_.dtype == np.int16: a_ = a_.view(np.uint16)
+        assert np.array_equal(a_, wd[key]), key
+    fin = np.isfinite(want[0])
+    best = (float(want[0][fin].min()), int(np.flatnonzero(want[0] == want[0][fin].min())[0])) if fin.any() else (float("inf"), 0)
+    assert g.search(6, n) == best == o.search(6, n)
+    g.close()
