@@ -64,6 +64,9 @@ extern "C" {
 #define LGX_OPT_THREADS_B   2    /* threads per block of the walk/finish kernel: multiple of 32, 32 .. what fits */
 #define LGX_OPT_THREADS_MV  3    /* threads per block of the move kernels: multiple of 32, 64 .. what fits      */
 #define LGX_OPT_CHUNK_LOG2  4    /* log2 of the candidates per kernel pair, 10 .. 26 (queue memory = chunk * record bytes) */
+#define LGX_OPT_CUT_WARP    6    /* 1: the decode/cut kernel works one candidate per WARP (lgx_decode_cut_w; needs N_F > 255, no
+                                    zero-demand BP and room for its per-warp state: else LGX_EINVAL), 0 (default): one per thread.
+                                    An alternative mapping kept for measurement: slower on every config so far */
 #define LGX_OPT_SQ_SHIFT    5    /* log2 of the replication of the s_q table in the decode/cut kernel's shared memory, 0 .. 5;
                                     synchronises the device and re-uploads the image                            */
 
@@ -155,7 +158,9 @@ int lgx_decode_batch(const lgx_instance *inst, uint64_t seed,
  * kernel, 10 candidates per kernel pair (chunk), 11 bytes per queue record, 15 / 16 threads per
  * block / shared memory bytes of the move kernels (Algorithm 1 entry points below; 0 threads: they do not fit),
  * 17 log2 of the s_q replication, 18 threads per block of the decode/cut kernel in lgx_decode_batch,
- * 19 per-candidate state bytes of the walk/finish kernel, 20 the instance's CUDA device.    */
+ * 19 per-candidate state bytes of the walk/finish kernel, 20 the instance's CUDA device, 21 decode/cut mapping in
+ * use (0 one candidate per thread, 1 per warp), 22 warps per block of the per-warp kernel (0 when not in use),
+ * 23 whether the per-warp mapping is possible for this instance (LGX_OPT_CUT_WARP).        */
 int lgx_instance_query(const lgx_instance *inst, int what, int64_t *out);
 
 /* Launch-configuration knobs (LGX_OPT_* above).  Results never depend on them.              */

@@ -24,7 +24,7 @@ UNITS = [("api", "lgx_api.cu", []),
          ("moves1", "lgx_inst_moves.cu", ["-DLGX_MASKW=1"]),
          ("moves2", "lgx_inst_moves.cu", ["-DLGX_MASKW=2"])]
 DEPS = [os.path.join(CSRC, f) for f in ("lgx_api.cu", "lgx_inst_decode.cu", "lgx_inst_walk.cu", "lgx_inst_moves.cu",
-                                        "lgx_dispatch.h", "lgx_kernels.cuh", "lgx_moves.cuh", "lgx_image.h")] + \
+                                        "lgx_dispatch.h", "lgx_kernels.cuh", "lgx_cutw.cuh", "lgx_moves.cuh", "lgx_image.h")] + \
        [os.path.join(ROOT, "include", "lgx.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

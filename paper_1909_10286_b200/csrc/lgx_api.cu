@@ -5,6 +5,7 @@
 #include "lgx_image.h"
 #include "lgx_dispatch.h"
 #include "lgx_moves.cuh"
+#include "lgx_cutw.cuh"
 
 #include <algorithm>
 #include <atomic>
@@ -30,6 +31,8 @@ struct lgx_instance {
   int64_t smem_budget = 0;                   // dynamic shared memory one block may take
   // launch configuration of the persistent kernels (lgx_decode_cut: a, its diagnostic decode mode: a_dec; lgx_walk_finish: b)
   int threads_a = 0, threads_a_dec = 0, threads_b = 0, grid = 0;
+  int cut_warp = 0, cut_warp_ok = 0, warps_w = 0;   // lgx_decode_cut_w (one candidate per warp): in use, possible, warps per block
+  uint32_t w_bytes = 0;                             // its shared memory per warp
   uint64_t a_state = 0, a_state_dec = 0, b_state = 0;   // per-candidate shared-memory bytes
   uint64_t chunk = 0;                          // candidates per decode/finish kernel pair
   cudaMemPool_t pool = nullptr;                // the device's workspace pool (owned by the library, not by the instance)
@@ -412,6 +415,20 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   I->threads_a_dec = (int)fit_threads(budget, H.image_bytes, (int64_t)I->a_state_dec, H.perm16 ? kMaxThreadsA16 : kMaxThreadsA);
   I->threads_b     = (int)fit_threads(budget, H.imagec_bytes, (int64_t)I->b_state, H.coords == 0 ? kMaxThreadsB : kMaxThreadsBC);
   if (I->threads_a < 32 || I->threads_a_dec < 32 || I->threads_b < 32) { free_instance(I); return LGX_ETOOBIG; }
+#ifndef LGX_EMU
+  {
+    // one candidate per warp (lgx_cutw.cuh): possible with 16-bit field ids, no zero-demand BP, the BP partition's draws
+    // inside the permutation's words, and room for at least four warps.  Opt-in (LGX_OPT_CUT_WARP): it measured slower
+    // than the per-thread mapping on every config, so it is never chosen by default
+    const CutWLayout WL = cutw_layout(H);
+    const int64_t wfit = std::min<int64_t>((budget - (int64_t)H.image_bytes) / (int64_t)WL.bytes, kMaxThreadsW / 32);
+    const uint32_t draw_words = 4u * cdiv(2u * (uint32_t)nb - 1u - (uint32_t)nt, 4u);
+    I->w_bytes = WL.bytes;
+    I->warps_w = (int)std::max<int64_t>(wfit, 0);
+    I->cut_warp_ok = (H.perm16 && !H.zero_demand && wfit >= 4 && draw_words <= H.n_perm_words) ? 1 : 0;
+    I->cut_warp = 0;
+  }
+#endif
   I->grid = I->sm_count;                       // one persistent block per SM
   // candidates per kernel pair: the queue holds a whole chunk (every candidate may pass eq. (2)); <= 2 GiB, <= 2^24
   // (measured: Medium gains 1.4 % from 2^22 -> 2^24, Toy 7 %; the big-record configs are flat between 2^18 and 2^21)
@@ -433,6 +450,10 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
     if (rc == LGX_OK) rc = allow_max_smem((const void *)ka, smem_optin); if (rc == LGX_OK) rc = allow_max_smem((const void *)kb, smem_optin);
     pick_kernels<MODE_DECODE>(H, ka, kb);
     if (rc == LGX_OK) rc = allow_max_smem((const void *)ka, smem_optin); if (rc == LGX_OK) rc = allow_max_smem((const void *)kb, smem_optin);
+    if (I->cut_warp_ok) {
+      if (rc == LGX_OK) rc = allow_max_smem((const void *)pick_decode_cut_w(H, MODE_EVAL), smem_optin);
+      if (rc == LGX_OK) rc = allow_max_smem((const void *)pick_decode_cut_w(H, MODE_SEARCH), smem_optin);
+    }
     if (rc != LGX_OK) { free_instance(I); return rc; }
   }
   // ---- move kernels: shared-memory layout (lgx_moves.cuh) and vertex coordinates for lgx_init_plan
@@ -554,6 +575,12 @@ int lgx_instance_set_option(lgx_instance *I, int key, int64_t value)
       I->chunk = 1ull << value;
       return LGX_OK;
     }
+    case LGX_OPT_CUT_WARP: {
+      if (value != 0 && value != 1) return LGX_EINVAL;
+      if (value == 1 && !I->cut_warp_ok) return LGX_EINVAL;
+      I->cut_warp = (int)value;
+      return LGX_OK;
+    }
     case LGX_OPT_SQ_SHIFT: {
       if (value < 0 || value > 5) return LGX_EINVAL;
       const int64_t img = 16 + 4ll * ((int64_t)H.n_f << value) + 16 + 4ll * H.n_b;
@@ -563,6 +590,10 @@ int lgx_instance_set_option(lgx_instance *I, int key, int64_t value)
       if (rc != LGX_OK) return rc;
       I->threads_a     = (int)std::min<int64_t>(I->threads_a, fit_threads(budget, H.image_bytes, (int64_t)I->a_state, H.perm16 ? kMaxThreadsA16 : kMaxThreadsA));
       I->threads_a_dec = (int)std::min<int64_t>(I->threads_a_dec, fit_threads(budget, H.image_bytes, (int64_t)I->a_state_dec, H.perm16 ? kMaxThreadsA16 : kMaxThreadsA));
+      if (I->w_bytes) {
+        I->warps_w = (int)std::min<int64_t>((budget - (int64_t)H.image_bytes) / (int64_t)I->w_bytes, 32);
+        if (I->warps_w < 4) { I->cut_warp_ok = 0; I->cut_warp = 0; }
+      }
       return LGX_OK;
     }
     default: return LGX_EINVAL;
@@ -606,8 +637,12 @@ int run_chunks(const lgx_instance *I, KernelFn ka, KernelFn kb, KParams &P, uint
                bool decode_mode, std::vector<cudaEvent_t> *evs = nullptr)
 {
   if (!ka || !kb) return LGX_EINVAL;
-  const uint64_t ta = LGX_BLOCK_THREADS((uint64_t)(decode_mode ? I->threads_a_dec : I->threads_a)), tb = LGX_BLOCK_THREADS((uint64_t)I->threads_b);
-  const size_t smem_a = (size_t)I->hdr.image_bytes + (size_t)(decode_mode ? I->a_state_dec : I->a_state) * ta;
+  const bool per_warp = I->cut_warp && !decode_mode;      // lgx_decode_cut_w: a block of warps_w warps works warps_w candidates at a time
+  const uint64_t ta = per_warp ? 32ull * (uint64_t)I->warps_w : LGX_BLOCK_THREADS((uint64_t)(decode_mode ? I->threads_a_dec : I->threads_a));
+  const uint64_t tb = LGX_BLOCK_THREADS((uint64_t)I->threads_b);
+  const uint64_t cand_a = per_warp ? (uint64_t)I->warps_w : ta;          // candidates a block of kernel 1 holds
+  const size_t smem_a = per_warp ? (size_t)I->hdr.image_bytes + (size_t)I->w_bytes * (size_t)I->warps_w
+                                 : (size_t)I->hdr.image_bytes + (size_t)(decode_mode ? I->a_state_dec : I->a_state) * ta;
   const size_t smem_b = (size_t)I->hdr.imagec_bytes + (size_t)I->b_state * tb;
   P.H = I->hdr; P.image = I->d_image; P.image_c = I->d_image_c;
   P.queue = W.queue; P.cap = (uint32_t)W.cap; P.q_count = W.q_count; P.ctr_a = W.ctr_a; P.ctr_b = W.ctr_b;
@@ -615,7 +650,7 @@ int run_chunks(const lgx_instance *I, KernelFn ka, KernelFn kb, KParams &P, uint
   void *args[] = { (void *)&P };
   for (uint64_t base = 0; base < n; base += W.cap) {
     P.base_i = base; P.n = std::min<uint64_t>(W.cap, n - base);
-    const unsigned grid_a = (unsigned)std::min<uint64_t>((uint64_t)I->grid, (P.n + ta - 1) / ta);
+    const unsigned grid_a = (unsigned)std::min<uint64_t>((uint64_t)I->grid, (P.n + cand_a - 1) / cand_a);
     const unsigned grid_b = (unsigned)std::min<uint64_t>((uint64_t)I->grid, (P.n + tb - 1) / tb);
     cudaEvent_t e3[3] = {nullptr, nullptr, nullptr};
     if (evs) { for (auto &e : e3) { CU(cudaEventCreate(&e)); evs->push_back(e); } CU(cudaEventRecord(e3[0], st)); }
@@ -639,7 +674,7 @@ int lgx_instance_query(const lgx_instance *I, int what, int64_t *out)
     case 0: *out = (int64_t)I->hdr.image_bytes + I->hdr.imagec_bytes; break;
     case 1: *out = I->threads_a; break;
     case 2: *out = I->grid; break;
-    case 3: *out = (int64_t)I->hdr.image_bytes + (int64_t)I->a_state * I->threads_a; break;
+    case 3: *out = I->cut_warp ? (int64_t)I->hdr.image_bytes + (int64_t)I->w_bytes * I->warps_w : (int64_t)I->hdr.image_bytes + (int64_t)I->a_state * I->threads_a; break;
     case 4: *out = I->hdr.coords; break;
     case 5: *out = (int64_t)I->a_state; break;
     case 6: *out = I->sm_count; break;
@@ -657,6 +692,9 @@ int lgx_instance_query(const lgx_instance *I, int what, int64_t *out)
     case 18: *out = I->threads_a_dec; break;
     case 19: *out = (int64_t)I->b_state; break;
     case 20: *out = I->device; break;
+    case 21: *out = I->cut_warp; break;
+    case 22: *out = I->cut_warp ? I->warps_w : 0; break;
+    case 23: *out = I->cut_warp_ok; break;
     default: return LGX_EINVAL;
   }
   return LGX_OK;
@@ -701,6 +739,7 @@ int lgx_eval_batch(const lgx_instance *I, uint64_t seed, const uint64_t *d_ids, 
   P.ids = d_ids; P.first_id = first_id;
   P.cost = d_cost; P.path_km = d_path_km; P.makespan_h = d_makespan_h; P.feasible = d_feasible;
   KernelFn ka, kb; pick_kernels<MODE_EVAL>(I->hdr, ka, kb);
+  if (I->cut_warp) ka = pick_decode_cut_w(I->hdr, MODE_EVAL);
   Workspace W;
   rc = ws_alloc(I, n, false, st, W);
   if (rc != LGX_OK) return rc;
@@ -743,6 +782,7 @@ int lgx_search_range(const lgx_instance *I, uint64_t seed, uint64_t first_id, ui
   fill_round_keys(P, seed);
   P.ids = nullptr; P.first_id = first_id;
   KernelFn ka, kb; pick_kernels<MODE_SEARCH>(I->hdr, ka, kb);
+  if (I->cut_warp) ka = pick_decode_cut_w(I->hdr, MODE_SEARCH);
   Workspace W;
   rc = ws_alloc(I, n, true, st, W);
   if (rc != LGX_OK) return rc;

@@ -64,7 +64,6 @@ static inline void __syncthreads() {}
 static inline void __syncwarp() {}
 static inline void __threadfence() {}
 template <class T, class U> static inline T atomicAdd(T *p, U v) { T o = *p; *p = (T)(o + (T)v); return o; }
-template <class T, class U> static inline T atomicXor(T *p, U v) { T o = *p; *p = (T)(o ^ (T)v); return o; }
 template <class T> static inline T __ldcg(const T *p) { return *p; }
 
 // ---- runtime
