@@ -889,14 +889,15 @@ struct PlanDev {
   size_t bytes = 0;
 };
 
-int plan_dev_alloc(const ImgHdr &H, cudaStream_t st, PlanDev &D)
+int plan_dev_alloc(const lgx_instance *I, cudaStream_t st, PlanDev &D)
 {
+  const ImgHdr &H = I->hdr;
   const size_t nb = H.n_b, nf = H.n_f, nhu = H.n_hu, nsu = H.n_su;
   size_t o = 0;
   const size_t o_fb = o; o += 2 * nf; const size_t o_fq = o; o += 2 * nf;
   const size_t o_bt = o; o += nb; const size_t o_bq = o; o += nb; const size_t o_hu = o; o += nhu; const size_t o_su = o; o += nsu;
   D.bytes = o;
-  CU(cudaMallocAsync((void **)&D.base, o, st));
+  CU(cudaMallocFromPoolAsync((void **)&D.base, o, I->pool, st));        // the library's cached per-device pool
   D.fb = reinterpret_cast<uint16_t *>(D.base + o_fb); D.fq = reinterpret_cast<uint16_t *>(D.base + o_fq);
   D.bt = D.base + o_bt; D.bq = D.base + o_bq; D.hu = D.base + o_hu; D.su = D.base + o_su;
   return LGX_OK;
@@ -947,12 +948,12 @@ int lgx_init_plan(const lgx_instance *I, uint8_t *h_bp_tour, uint8_t *h_bp_pos, 
   cudaStream_t st = (cudaStream_t)stream;
   const ImgHdr &H = I->hdr;
   PlanDev D;
-  rc = plan_dev_alloc(H, st, D);
+  rc = plan_dev_alloc(I, st, D);
   if (rc != LGX_OK) return rc;
   const size_t nb = H.n_b, nf = H.n_f;
   const size_t scratch_bytes = 4 * (3 * nb + 1) + 2 * (nf + (nf & 1)) + 2 * nb + 16;
   uint32_t *scratch = nullptr;
-  cudaError_t e = cudaMallocAsync((void **)&scratch, scratch_bytes, st);
+  cudaError_t e = cudaMallocFromPoolAsync((void **)&scratch, scratch_bytes, I->pool, st);
   if (e != cudaSuccess) { cudaFreeAsync(D.base, st); return cuda_fail(e, "cudaMallocAsync(init scratch)"); }
   InitParams P{};
   P.n_f = H.n_f; P.n_b = H.n_b; P.n_t = H.n_t; P.n_hu = H.n_hu; P.n_su = H.n_su;
@@ -991,7 +992,7 @@ int lgx_move_eval_batch(const lgx_instance *I,
   MvKernelFn kb, ks; pick_move_kernels(H, kb, ks);
   if (!kb) return LGX_EINVAL;
   PlanDev D;
-  rc = plan_dev_alloc(H, st, D);
+  rc = plan_dev_alloc(I, st, D);
   if (rc != LGX_OK) return rc;
   rc = plan_upload(H, D, h_bp_tour, h_bp_pos, h_field_bp, h_field_pos, h_hu_tour, h_su_tour, st);
   if (rc == LGX_OK) {
@@ -1039,13 +1040,13 @@ int lgx_local_search(const lgx_instance *I,
   const uint64_t blocks = ((uint64_t)n_workers + (uint64_t)I->threads_mv - 1) / (uint64_t)I->threads_mv;
   const unsigned grid = (unsigned)std::min<uint64_t>((uint64_t)I->sm_count, blocks);
   PlanDev D;
-  rc = plan_dev_alloc(H, st, D);
+  rc = plan_dev_alloc(I, st, D);
   if (rc != LGX_OK) return rc;
   uint8_t *ws = nullptr;
   const size_t slots_bytes = 2ull * grid * I->mv.slot_words * 8ull;
   const size_t hist_bytes = (size_t)n_iters * 8ull;
   const size_t ws_bytes = slots_bytes + 2 * hist_bytes + 16;
-  cudaError_t e = cudaMallocAsync((void **)&ws, ws_bytes, st);
+  cudaError_t e = cudaMallocFromPoolAsync((void **)&ws, ws_bytes, I->pool, st);
   if (e != cudaSuccess) { cudaFreeAsync(D.base, st); return cuda_fail(e, "cudaMallocAsync(search workspace)"); }
   rc = plan_upload(H, D, h_bp_tour, h_bp_pos, h_field_bp, h_field_pos, h_hu_tour, h_su_tour, st);
   double best = 0.0;
