@@ -273,6 +273,7 @@ def main():
     ap.add_argument("--threads-a", type=int, default=None, help="LGX_OPT_THREADS_A (tuning)")
     ap.add_argument("--threads-b", type=int, default=None, help="LGX_OPT_THREADS_B (tuning)")
     ap.add_argument("--cut-warp", type=int, default=None, help="LGX_OPT_CUT_WARP: 1 = the per-warp decode/cut kernel (alternative mapping; profiling)")
+    ap.add_argument("--walk-lockstep", type=int, default=None, help="LGX_OPT_WALK_LOCKSTEP (tuning)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--alg1-workload", default="paper_scale", help="instance of the Algorithm 1 leg (SURVEY §8(f) N1/N3)")
     ap.add_argument("--alg1-iters", type=int, default=500)
@@ -300,7 +301,7 @@ def main():
     inst = wl.make(args.workload)
     per_gpu = 1 << (args.batch_log2 if args.batch_log2 is not None else min(28, inst.budget.bit_length() - 1))
     total = per_gpu * world                      # weak scaling: fixed ids per GPU
-    opts = ((4, args.chunk_log2), (1, args.threads_a), (2, args.threads_b), (6, args.cut_warp))
+    opts = ((4, args.chunk_log2), (1, args.threads_a), (2, args.threads_b), (6, args.cut_warp), (7, args.walk_lockstep))
 
     def new_instance(ins):
         gi = binding.Instance(ins)

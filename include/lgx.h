@@ -67,6 +67,9 @@ extern "C" {
 #define LGX_OPT_CUT_WARP    6    /* 1: the decode/cut kernel works one candidate per WARP (lgx_decode_cut_w; needs N_F > 255, no
                                     zero-demand BP and room for its per-warp state: else LGX_EINVAL), 0 (default): one per thread.
                                     An alternative mapping kept for measurement: slower on every config so far */
+#define LGX_OPT_WALK_LOCKSTEP 7  /* 1: the warps of a walk/finish block draw their queue records together (one barrier per batch; they
+                                    then share instruction-cache lines), 0: every warp on its own.  Only with coordinates (distance modes 1, 2;
+                                    ignored with the tables, where it measured slower).  Default: 1 with coordinates and N_F < 1024 */
 #define LGX_OPT_SQ_SHIFT    5    /* log2 of the replication of the s_q table in the decode/cut kernel's shared memory, 0 .. 5;
                                     synchronises the device and re-uploads the image                            */
 
@@ -160,7 +163,7 @@ int lgx_decode_batch(const lgx_instance *inst, uint64_t seed,
  * 17 log2 of the s_q replication, 18 threads per block of the decode/cut kernel in lgx_decode_batch,
  * 19 per-candidate state bytes of the walk/finish kernel, 20 the instance's CUDA device, 21 decode/cut mapping in
  * use (0 one candidate per thread, 1 per warp), 22 warps per block of the per-warp kernel (0 when not in use),
- * 23 whether the per-warp mapping is possible for this instance (LGX_OPT_CUT_WARP).        */
+ * 23 whether the per-warp mapping is possible for this instance (LGX_OPT_CUT_WARP), 24 LGX_OPT_WALK_LOCKSTEP.  */
 int lgx_instance_query(const lgx_instance *inst, int what, int64_t *out);
 
 /* Launch-configuration knobs (LGX_OPT_* above).  Results never depend on them.              */

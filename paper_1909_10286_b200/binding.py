@@ -18,7 +18,7 @@ LGX_OK, LGX_EINVAL, LGX_ETOOBIG, LGX_ECUDA, LGX_ENOMEM = 0, -1, -2, -3, -4
 # include/lgx.h: descriptor flags and lgx_instance_set_option keys
 LGX_FLAG_HU_BALANCE, LGX_FLAG_MAKESPAN_FILTER, LGX_FLAG_FIX_FIELD_BP = 2, 4, 8
 LGX_FLAG_DIST_COORDS, LGX_FLAG_DIST_MIXED = 16, 32
-LGX_OPT_THREADS_A, LGX_OPT_THREADS_B, LGX_OPT_THREADS_MV, LGX_OPT_CHUNK_LOG2, LGX_OPT_SQ_SHIFT, LGX_OPT_CUT_WARP = 1, 2, 3, 4, 5, 6
+LGX_OPT_THREADS_A, LGX_OPT_THREADS_B, LGX_OPT_THREADS_MV, LGX_OPT_CHUNK_LOG2, LGX_OPT_SQ_SHIFT, LGX_OPT_CUT_WARP, LGX_OPT_WALK_LOCKSTEP = 1, 2, 3, 4, 5, 6, 7
 LGX_MAX_BPS, LGX_MAX_SUS, LGX_MAX_MOVE_TOURS, LGX_MAX_MOVE_HUS = 127, 128, 64, 64
 
 _dp = C.POINTER(C.c_double)

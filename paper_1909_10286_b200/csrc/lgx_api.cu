@@ -31,6 +31,7 @@ struct lgx_instance {
   int64_t smem_budget = 0;                   // dynamic shared memory one block may take
   // launch configuration of the persistent kernels (lgx_decode_cut: a, its diagnostic decode mode: a_dec; lgx_walk_finish: b)
   int threads_a = 0, threads_a_dec = 0, threads_b = 0, grid = 0;
+  int walk_lockstep = 0;                            // lgx_walk_finish: block-synchronous work fetch (default with coordinates)
   int cut_warp = 0, cut_warp_ok = 0, warps_w = 0;   // lgx_decode_cut_w (one candidate per warp): in use, possible, warps per block
   uint32_t w_bytes = 0;                             // its shared memory per warp
   uint64_t a_state = 0, a_state_dec = 0, b_state = 0;   // per-candidate shared-memory bytes
@@ -430,6 +431,10 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   }
 #endif
   I->grid = I->sm_count;                       // one persistent block per SM
+  // block-synchronous work fetch of lgx_walk_finish: measured -6 % (Large) and -10 % (Sweep) kernel time with coordinates, where warps
+  // in different phases evict each other's code; +3.6 % with the tables (Medium) and +1.7 % on paper_scale, whose warps spend
+  // all their time in the same two loops anyway
+  I->walk_lockstep = (H.coords != 0 && nf < 1024) ? 1 : 0;
   // candidates per kernel pair: the queue holds a whole chunk (every candidate may pass eq. (2)); <= 2 GiB, <= 2^24
   // (measured: Medium gains 1.4 % from 2^22 -> 2^24, Toy 7 %; the big-record configs are flat between 2^18 and 2^21)
   {
@@ -575,6 +580,11 @@ int lgx_instance_set_option(lgx_instance *I, int key, int64_t value)
       I->chunk = 1ull << value;
       return LGX_OK;
     }
+    case LGX_OPT_WALK_LOCKSTEP: {
+      if (value != 0 && value != 1) return LGX_EINVAL;
+      I->walk_lockstep = (int)value;
+      return LGX_OK;
+    }
     case LGX_OPT_CUT_WARP: {
       if (value != 0 && value != 1) return LGX_EINVAL;
       if (value == 1 && !I->cut_warp_ok) return LGX_EINVAL;
@@ -647,6 +657,7 @@ int run_chunks(const lgx_instance *I, KernelFn ka, KernelFn kb, KParams &P, uint
   P.H = I->hdr; P.image = I->d_image; P.image_c = I->d_image_c;
   P.queue = W.queue; P.cap = (uint32_t)W.cap; P.q_count = W.q_count; P.ctr_a = W.ctr_a; P.ctr_b = W.ctr_b;
   P.done_counter = W.done; P.block_best = W.block_best; P.result = W.result;
+  P.lockstep = I->walk_lockstep ? 1u : 0u;
   void *args[] = { (void *)&P };
   for (uint64_t base = 0; base < n; base += W.cap) {
     P.base_i = base; P.n = std::min<uint64_t>(W.cap, n - base);
@@ -695,6 +706,7 @@ int lgx_instance_query(const lgx_instance *I, int what, int64_t *out)
     case 21: *out = I->cut_warp; break;
     case 22: *out = I->cut_warp ? I->warps_w : 0; break;
     case 23: *out = I->cut_warp_ok; break;
+    case 24: *out = I->walk_lockstep; break;
     default: return LGX_EINVAL;
   }
   return LGX_OK;

@@ -410,3 +410,22 @@ def test_cut_per_warp_is_refused_where_it_cannot_work():
     g = binding.Instance(z)
     assert g.query(23) == 0 and g.query(21) == 0
     g.close()
+
+
+@pytest.mark.parametrize("name", ["small", "large", "sweep", "paper_scale"])
+def test_walk_lockstep_does_not_change_results(ctxs, name):
+    """LGX_OPT_WALK_LOCKSTEP only changes how the warps of a walk/finish block draw their records: same bits either way,
+    also when the last batch of a launch is ragged and when a block's batch is larger than the queue."""
+    inst, o, g = ctxs(name)
+    default = g.query(24)
+    assert default == (1 if g.query(4) != 0 and inst.n_fields < 1024 else 0)      # coordinates and N_F < 1024: on by default
+    outs = []
+    for mode in (0, 1):
+        g.set_option(binding.LGX_OPT_WALK_LOCKSTEP, mode)
+        assert g.query(24) == mode
+        r = [t.clone() for t in g.eval_batch(inst.seed, first_id=9, n=100003)] + [g.search(inst.seed, 70001, first_id=3), g.search(inst.seed, 17)]
+        outs.append(r)
+    g.set_option(binding.LGX_OPT_WALK_LOCKSTEP, default)
+    assert all(torch.equal(a, b) for a, b in zip(outs[0][:4], outs[1][:4])) and outs[0][4:] == outs[1][4:]
+    want = o.eval_batch(inst.seed, first_id=9, n=512)
+    assert np.array_equal(outs[1][0][:512].cpu().numpy(), want[0]) and np.array_equal(outs[1][3][:512].cpu().numpy(), want[3])
