@@ -22,8 +22,8 @@
 // test_gpu_parity.py), never chosen by default.  Measured on B200 (profiles/r02_alt_cut_per_warp_paper_scale.md): 32
 // resident warps instead of 2 and 47 % instead of 14 % of the SM's issue slots busy, but 8.5 k instead of 2.3 k
 // warp-instructions per candidate (the conflict resolution, the scans and the lane-0 BP partition), most of them
-// shuffles, votes and shared-memory accesses that queue in the MIO pipe: paper_scale 13.2 ms vs 10.0 ms per 860 k
-// candidates, Sweep 14.2 ms vs 4.3 ms per 1.97 M.  It cannot be used when a BP has zero demand or in the decode mode.
+// shuffles, votes and shared-memory accesses that queue in the MIO pipe: paper_scale 13.2 ms vs 9.8 ms per 860 k
+// candidates, Sweep 14.2 ms vs 4.4 ms per 1.97 M.  It cannot be used when a BP has zero demand or in the decode mode.
 #pragma once
 #include "lgx_kernels.cuh"
 
