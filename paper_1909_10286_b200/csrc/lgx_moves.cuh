@@ -661,7 +661,7 @@ __device__ __forceinline__ EvalOut mv_eval(const MvParams &P, const uint8_t *sm,
     for (uint32_t g = 0; g < n_t; ++g) { const double t_g = s.d(M.m64_t + g); if (t_g > makespan) makespan = t_g; }
   }
 
-  // ---- S6: Algorithm 2 (L209-227), readings R11-R16 (same procedure as in lgx_finish)
+  // ---- S6: Algorithm 2 (L209-227), readings R11-R16 (same procedure as in lgx_walk_finish)
   if (n_t >= 2u) {
     for (uint32_t iter = 0; iter < n_su; ++iter) {
       uint32_t g_max = 0, g_2nd = kNone; double w_max = s.d(M.m64_w), w_2nd = 0.0;
