@@ -124,8 +124,11 @@ int lgx_eval_batch(const lgx_instance *inst, uint64_t seed,
                    double *d_cost, double *d_path_km, double *d_makespan_h, uint8_t *d_feasible,
                    void *cuda_stream);
 
-/* Same, with HOST buffers: copies ids in (if given) and results out inside the call
- * (chunked, synchronous).  Used for the end-to-end number in bench.py.                     */
+/* Same, with HOST buffers: copies ids in (if given) and results out inside the call, which returns when every
+ * output is in place.  Chunks of 2^21 candidates alternate between two internal streams: with page-locked host
+ * buffers (cudaHostAlloc / cudaHostRegister, torch pin_memory) the copies of one chunk overlap the kernels of the
+ * next; pageable buffers work too, chunk after chunk.  Any output pointer may be NULL.  Used for the
+ * end-to-end number of lgx_eval_batch in bench.py.                                          */
 int lgx_eval_batch_host(const lgx_instance *inst, uint64_t seed,
                         const uint64_t *h_ids, uint64_t first_id, uint64_t n,
                         double *h_cost, double *h_path_km, double *h_makespan_h, uint8_t *h_feasible);

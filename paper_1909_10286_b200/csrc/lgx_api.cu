@@ -839,26 +839,42 @@ int lgx_eval_batch_host(const lgx_instance *I, uint64_t seed, const uint64_t *h_
   if (n == 0) return LGX_OK;
   int rc = check_device(I);
   if (rc != LGX_OK) return rc;
-  const uint64_t chunk = std::min<uint64_t>(n, 1ull << 22);
-  uint64_t *d_ids = nullptr; double *d_c = nullptr, *d_p = nullptr, *d_m = nullptr; uint8_t *d_f = nullptr;
+  // Chunks of 2^21 candidates alternate between two streams, each with its own device buffers (from the cached pool):
+  // with page-locked host buffers the copies of one chunk overlap the kernels of the next; with pageable buffers the
+  // driver stages every copy and the chunks simply run one after the other.
+  const uint64_t chunk = std::min<uint64_t>(n, 1ull << 21);
+  cudaStream_t st[2] = {nullptr, nullptr};
+  uint8_t *buf[2] = {nullptr, nullptr};
+  const size_t o_c = 0, o_p = 8 * chunk, o_m = 16 * chunk, o_i = 24 * chunk, o_f = 32 * chunk, bytes = 33 * chunk + 256;
   cudaError_t e = cudaSuccess;
-  auto cleanup = [&]() { cudaFree(d_ids); cudaFree(d_c); cudaFree(d_p); cudaFree(d_m); cudaFree(d_f); };
-  if (h_ids && (e = cudaMalloc((void **)&d_ids, chunk * 8)) != cudaSuccess) { cleanup(); return cuda_fail(e, "cudaMalloc"); }
-  if (h_cost && (e = cudaMalloc((void **)&d_c, chunk * 8)) != cudaSuccess) { cleanup(); return cuda_fail(e, "cudaMalloc"); }
-  if (h_path_km && (e = cudaMalloc((void **)&d_p, chunk * 8)) != cudaSuccess) { cleanup(); return cuda_fail(e, "cudaMalloc"); }
-  if (h_makespan_h && (e = cudaMalloc((void **)&d_m, chunk * 8)) != cudaSuccess) { cleanup(); return cuda_fail(e, "cudaMalloc"); }
-  if (h_feasible && (e = cudaMalloc((void **)&d_f, chunk)) != cudaSuccess) { cleanup(); return cuda_fail(e, "cudaMalloc"); }
-  for (uint64_t o = 0; o < n && rc == LGX_OK; o += chunk) {
-    const uint64_t m = std::min<uint64_t>(chunk, n - o);
-    if (h_ids && (e = cudaMemcpyAsync(d_ids, h_ids + o, m * 8, cudaMemcpyHostToDevice, 0)) != cudaSuccess) { rc = cuda_fail(e, "H2D ids"); break; }
-    rc = lgx_eval_batch(I, seed, h_ids ? d_ids : nullptr, first_id + o, m, d_c, d_p, d_m, d_f, nullptr);
-    if (rc != LGX_OK) break;
-    if (h_cost && (e = cudaMemcpyAsync(h_cost + o, d_c, m * 8, cudaMemcpyDeviceToHost, 0)) != cudaSuccess) { rc = cuda_fail(e, "D2H"); break; }
-    if (h_path_km && (e = cudaMemcpyAsync(h_path_km + o, d_p, m * 8, cudaMemcpyDeviceToHost, 0)) != cudaSuccess) { rc = cuda_fail(e, "D2H"); break; }
-    if (h_makespan_h && (e = cudaMemcpyAsync(h_makespan_h + o, d_m, m * 8, cudaMemcpyDeviceToHost, 0)) != cudaSuccess) { rc = cuda_fail(e, "D2H"); break; }
-    if (h_feasible && (e = cudaMemcpyAsync(h_feasible + o, d_f, m, cudaMemcpyDeviceToHost, 0)) != cudaSuccess) { rc = cuda_fail(e, "D2H"); break; }
-    if ((e = cudaStreamSynchronize(0)) != cudaSuccess) { rc = cuda_fail(e, "cudaStreamSynchronize"); break; }
+  auto cleanup = [&]() {
+    for (int k = 0; k < 2; ++k) {
+      if (buf[k]) cudaFreeAsync(buf[k], st[k]);
+      if (st[k]) { cudaStreamSynchronize(st[k]); cudaStreamDestroy(st[k]); }
+    }
+  };
+  for (int k = 0; k < 2 && e == cudaSuccess; ++k) {
+    e = cudaStreamCreateWithFlags(&st[k], cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaMallocFromPoolAsync((void **)&buf[k], bytes, I->pool, st[k]);
   }
+  if (e != cudaSuccess) { cleanup(); return cuda_fail(e, "lgx_eval_batch_host: streams / buffers"); }
+  uint64_t k = 0;
+  for (uint64_t o = 0; o < n && rc == LGX_OK; o += chunk, ++k) {
+    const uint64_t m = std::min<uint64_t>(chunk, n - o);
+    cudaStream_t s = st[k & 1]; uint8_t *b = buf[k & 1];
+    uint64_t *d_ids = reinterpret_cast<uint64_t *>(b + o_i);
+    double *d_c = h_cost ? reinterpret_cast<double *>(b + o_c) : nullptr, *d_p = h_path_km ? reinterpret_cast<double *>(b + o_p) : nullptr;
+    double *d_m = h_makespan_h ? reinterpret_cast<double *>(b + o_m) : nullptr; uint8_t *d_f = h_feasible ? b + o_f : nullptr;
+    if (h_ids && (e = cudaMemcpyAsync(d_ids, h_ids + o, m * 8, cudaMemcpyHostToDevice, s)) != cudaSuccess) { rc = cuda_fail(e, "H2D ids"); break; }
+    rc = lgx_eval_batch(I, seed, h_ids ? d_ids : nullptr, first_id + o, m, d_c, d_p, d_m, d_f, (void *)s);
+    if (rc != LGX_OK) break;
+    if (h_cost && (e = cudaMemcpyAsync(h_cost + o, d_c, m * 8, cudaMemcpyDeviceToHost, s)) != cudaSuccess) { rc = cuda_fail(e, "D2H"); break; }
+    if (h_path_km && (e = cudaMemcpyAsync(h_path_km + o, d_p, m * 8, cudaMemcpyDeviceToHost, s)) != cudaSuccess) { rc = cuda_fail(e, "D2H"); break; }
+    if (h_makespan_h && (e = cudaMemcpyAsync(h_makespan_h + o, d_m, m * 8, cudaMemcpyDeviceToHost, s)) != cudaSuccess) { rc = cuda_fail(e, "D2H"); break; }
+    if (h_feasible && (e = cudaMemcpyAsync(h_feasible + o, d_f, m, cudaMemcpyDeviceToHost, s)) != cudaSuccess) { rc = cuda_fail(e, "D2H"); break; }
+  }
+  for (int j = 0; j < 2; ++j)
+    if ((e = cudaStreamSynchronize(st[j])) != cudaSuccess && rc == LGX_OK) rc = cuda_fail(e, "cudaStreamSynchronize");
   cleanup();
   return rc;
 }

@@ -197,6 +197,20 @@ def test_eval_batch_host_buffers(ctxs):
     got = g.eval_batch_host(inst.seed, first_id=10, n=(1 << 22) + 17)       # crosses a chunk boundary
     want = o.eval_batch(inst.seed, first_id=10 + (1 << 22) - 8, n=25)
     assert np.array_equal(got[0][(1 << 22) - 8:], want[0])
+    # page-locked buffers (copies overlap the next chunk's kernels), five chunks on two streams, explicit ids: every
+    # element equal to the device-buffer call
+    n = (1 << 23) + 4099
+    ids = torch.arange(n, dtype=torch.int64) * 3 + 7
+    pinned = tuple(torch.empty(n, dtype=dt, pin_memory=True) for dt in (torch.float64, torch.float64, torch.float64, torch.uint8))
+    g.eval_batch_host(inst.seed, ids=ids.numpy().astype(np.uint64), out=tuple(t.numpy() for t in pinned))
+    dev = g.eval_batch(inst.seed, ids=ids.cuda())
+    torch.cuda.synchronize()
+    for a, b in zip(pinned, dev):
+        assert torch.equal(a, b.cpu())
+    for k in (1 << 21) - 1, 1 << 21, (1 << 22) + 5, n - 1:               # chunk seams against the oracle
+        w = o.eval_batch(inst.seed, ids=np.array([3 * k + 7], dtype=np.uint64))
+        assert pinned[0][k].item() == w[0][0] or (np.isinf(w[0][0]) and np.isinf(pinned[0][k].item()))
+        assert pinned[3][k].item() == w[3][0]
 
 
 def test_paper_scale_workload(ctxs):
