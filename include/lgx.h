@@ -36,6 +36,7 @@ extern "C" {
                                or a kernel limit below is exceeded                           */
 #define LGX_ECUDA    (-3)   /* CUDA runtime error; text via lgx_strerror(LGX_ECUDA)          */
 #define LGX_ENOMEM   (-4)
+#define LGX_ESTATIC  (-5)   /* lgx_eval_batch_static: n above lgx_eval_batch_static_max()     */
 
 /* Kernel limits of this build (beyond them lgx_instance_create returns LGX_ETOOBIG; the move kernels'
  * limits make lgx_move_eval_batch / lgx_local_search return LGX_ETOOBIG, the instance itself is still created). */
@@ -132,6 +133,46 @@ int lgx_eval_batch(const lgx_instance *inst, uint64_t seed,
 int lgx_eval_batch_host(const lgx_instance *inst, uint64_t seed,
                         const uint64_t *h_ids, uint64_t first_id, uint64_t n,
                         double *h_cost, double *h_path_km, double *h_makespan_h, uint8_t *h_feasible);
+
+/* lgx_eval_batch for callers that must not allocate device memory at call time.
+ *
+ * Who needs it: lgx_eval_batch takes the queue between its two kernels from the library's memory pool, and a pool
+ * that has to grow goes to the driver for memory.  Some hosts cannot afford or are not allowed that: a service whose
+ * start-up phase hands every free byte of HBM to another owner (a tensor framework's caching allocator, a
+ * pre-sized cache), so that a later request to the driver simply fails; a control or serving loop with a latency
+ * bound, because driver allocation and release may stall the whole device for an unbounded time; a plug-in running
+ * under a host application that forbids allocator calls after initialisation.  For them the queue and the
+ * kernels' counters live in ONE fixed array of LGX_STATIC_SCRATCH_BYTES (16 MiB) that is part of the library's
+ * device image: a GPU carries those 16 MiB from the moment the CUDA runtime loads that image on it (with eager
+ * module loading when the library is first used there, otherwise at the latest at the first call below) until
+ * the process exits, whether the call is used again or not; nothing releases them earlier.  The call itself
+ * issues one 64-byte memset and the two kernels on cuda_stream: no cudaMalloc / cudaFree, no pool, no stream or
+ * event creation, no library routine that allocates.  Inputs and outputs are the caller's, exactly as in
+ * lgx_eval_batch (same arguments, same results bit for bit, asynchronous on cuda_stream).
+ *
+ * Limit: the whole call is one kernel pair, so n queue records must fit in the array:
+ * n <= lgx_eval_batch_static_max(inst) = (16 MiB - a header of 64 B + 16 B per SM) / record bytes, rounded down
+ * to a multiple of 32 (record bytes = lgx_instance_query what 11: about 135 000 candidates on the 100-field
+ * config, about 6 700 with 1200 fields).  A larger n returns LGX_ESTATIC before anything is launched; split the
+ * ids over several calls on the same stream instead.
+ *
+ * First call on a device: the library looks up the array's device address (cudaGetSymbolAddress, with the
+ * instance's device current) and remembers it per device; that call loads the module if it is not loaded yet.
+ * Make this first call during set-up, outside any stream capture; a small n is enough.  Later calls only read
+ * the remembered address.
+ *
+ * Sharing: there is one array per device, not per instance, stream or call, and it keeps the previous call's
+ * contents; each call zeroes the counters it needs before its kernels start.  Two calls may therefore follow each
+ * other on ONE stream (stream order keeps them apart), but calls that can overlap on the GPU (different streams
+ * without an event between them, different host threads on different streams, two instances at once) race on the
+ * queue and give wrong results.  Callers that need concurrency use lgx_eval_batch.                             */
+#define LGX_STATIC_SCRATCH_BYTES (16u << 20)
+int lgx_eval_batch_static(const lgx_instance *inst, uint64_t seed,
+                          const uint64_t *d_ids, uint64_t first_id, uint64_t n,
+                          double *d_cost, double *d_path_km, double *d_makespan_h, uint8_t *d_feasible,
+                          void *cuda_stream);
+/* Largest n lgx_eval_batch_static accepts for this instance (host-only arithmetic, no CUDA call). */
+int lgx_eval_batch_static_max(const lgx_instance *inst, uint64_t *max_n);
 
 /* a2..a7: evaluate ids [first_id, first_id + n) and return the ordered minimum of
  * (cost bit pattern, id): lowest cost, lowest id on ties (R29).  No feasible

@@ -14,7 +14,8 @@ from . import build as _build
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "liblgx.so")
 
-LGX_OK, LGX_EINVAL, LGX_ETOOBIG, LGX_ECUDA, LGX_ENOMEM = 0, -1, -2, -3, -4
+LGX_OK, LGX_EINVAL, LGX_ETOOBIG, LGX_ECUDA, LGX_ENOMEM, LGX_ESTATIC = 0, -1, -2, -3, -4, -5
+LGX_STATIC_SCRATCH_BYTES = 16 << 20
 # include/lgx.h: descriptor flags and lgx_instance_set_option keys
 LGX_FLAG_HU_BALANCE, LGX_FLAG_MAKESPAN_FILTER, LGX_FLAG_FIX_FIELD_BP = 2, 4, 8
 LGX_FLAG_DIST_COORDS, LGX_FLAG_DIST_MIXED = 16, 32
@@ -39,6 +40,7 @@ class lgx_instance_desc(C.Structure):
 
 
 EXPORTS = ("lgx_instance_create", "lgx_instance_destroy", "lgx_eval_batch", "lgx_eval_batch_host",
+           "lgx_eval_batch_static", "lgx_eval_batch_static_max",
            "lgx_search_range", "lgx_search", "lgx_decode_batch", "lgx_instance_query", "lgx_instance_set_timing",
            "lgx_instance_set_option", "lgx_selftest", "lgx_workspace_trim",
            "lgx_init_plan", "lgx_move_eval_batch", "lgx_local_search", "lgx_strerror")
@@ -61,6 +63,8 @@ def load(rebuild_if_stale: bool = True):
     lib.lgx_instance_destroy.argtypes = [vp]
     lib.lgx_eval_batch.argtypes = [vp, u64, vp, u64, u64, vp, vp, vp, vp, vp]
     lib.lgx_eval_batch_host.argtypes = [vp, u64, vp, u64, u64, vp, vp, vp, vp]
+    lib.lgx_eval_batch_static.argtypes = [vp, u64, vp, u64, u64, vp, vp, vp, vp, vp]
+    lib.lgx_eval_batch_static_max.argtypes = [vp, C.POINTER(u64)]
     lib.lgx_search_range.argtypes = [vp, u64, u64, u64, C.POINTER(C.c_double), C.POINTER(u64), vp]
     lib.lgx_search.argtypes = [vp, u64, u64, C.POINTER(C.c_double), C.POINTER(u64), vp]
     lib.lgx_decode_batch.argtypes = [vp, u64, vp, u64, u64] + [vp] * 7 + [vp]
@@ -205,6 +209,24 @@ class Instance:
         cost, path, mk, feas = out
         _check(self._lib.lgx_eval_batch(self._h, seed, _ptr(ids), first_id, n, _ptr(cost), _ptr(path),
                                         _ptr(mk), _ptr(feas), _stream_ptr(stream)))
+        return out
+
+    # -- lgx_eval_batch_static: lgx_eval_batch without any allocation inside the library (fixed 16 MiB device array)
+    def eval_batch_static_max(self) -> int:
+        """Largest n eval_batch_static takes for this instance (lgx_eval_batch_static_max)."""
+        v = C.c_uint64()
+        _check(self._lib.lgx_eval_batch_static_max(self._h, C.byref(v)))
+        return v.value
+
+    def eval_batch_static(self, seed, out, ids=None, first_id=0, n=None, stream=None):
+        """lgx_eval_batch_static.  `out` = the caller's (cost, path_km, makespan_h, feasible) device tensors: unlike
+        eval_batch this wrapper creates none, because the callers it is for cannot allocate.  One call at a time per
+        device: every call shares the library's one scratch array (include/lgx.h)."""
+        if ids is not None:
+            n = ids.numel()
+        cost, path, mk, feas = out
+        _check(self._lib.lgx_eval_batch_static(self._h, seed, _ptr(ids), first_id, n, _ptr(cost), _ptr(path),
+                                               _ptr(mk), _ptr(feas), _stream_ptr(stream)))
         return out
 
     # -- lgx_eval_batch_host: numpy host buffers in/out

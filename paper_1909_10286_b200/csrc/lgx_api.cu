@@ -184,6 +184,7 @@ const char *lgx_strerror(int code)
     case LGX_ETOOBIG: return "instance image or per-candidate state does not fit (shared memory / 32-bit quanta / kernel limits)";
     case LGX_ECUDA:   return g_cuda_msg.c_str();
     case LGX_ENOMEM:  return "out of memory";
+    case LGX_ESTATIC: return "lgx_eval_batch_static: n is larger than the library's fixed device scratch holds for this instance (lgx_eval_batch_static_max)";
     default:          return "unknown lgx error code";
   }
 }
@@ -880,6 +881,93 @@ int lgx_eval_batch_host(const lgx_instance *I, uint64_t seed, const uint64_t *h_
 }
 
 }  // extern "C"
+
+// ================================================================== lgx_eval_batch_static: no allocation at call time
+#ifndef LGX_EMU
+
+namespace {
+
+// The queue of feasible candidates and the kernels' counters for lgx_eval_batch_static.  It is part of the library's
+// device image: the driver places it when the module is loaded on a GPU and it stays there until the process exits, so
+// the entry point below never has to ask an allocator for memory.  One array per device, shared by every call: it keeps
+// whatever the last call left in it.
+static __device__ __align__(256) unsigned char g_static_scratch[LGX_STATIC_SCRATCH_BYTES];
+
+// In host code `g_static_scratch` is only a handle for the runtime, not memory a kernel can use; the address the kernels
+// get is looked up once per device, with that device current, and cached here.
+std::mutex g_static_mutex;
+unsigned char *g_static_ptr[kMaxDevices] = {};
+
+int static_scratch(int device, unsigned char **out)
+{
+  if (device < 0 || device >= kMaxDevices) return LGX_EINVAL;
+  std::lock_guard<std::mutex> lock(g_static_mutex);
+  if (!g_static_ptr[device]) {
+    unsigned char *p = nullptr;
+    CU(cudaGetSymbolAddress((void **)&p, g_static_scratch));      // check_device() made `device` the current one
+    if (!p) { g_cuda_msg = "cudaGetSymbolAddress returned a null address for the static scratch"; return LGX_ECUDA; }
+    g_static_ptr[device] = p;
+  }
+  *out = g_static_ptr[device];
+  return LGX_OK;
+}
+
+// Candidates one call can take: the array holds the counters, one 16-byte slot per block and one queue record each.
+uint64_t static_capacity(const lgx_instance *I, size_t *qoff_out)
+{
+  const size_t head = 64 + 16ull * (size_t)I->grid;
+  const size_t qoff = (head + 255) & ~(size_t)255;
+  if (qoff_out) *qoff_out = qoff;
+  if (qoff >= (size_t)LGX_STATIC_SCRATCH_BYTES) return 0;
+  return ((size_t)LGX_STATIC_SCRATCH_BYTES - qoff) / (4ull * I->hdr.rec_words) / 32 * 32;
+}
+
+}  // namespace
+
+extern "C" {
+
+int lgx_eval_batch_static_max(const lgx_instance *I, uint64_t *max_n)
+{
+  if (!I || !max_n) return LGX_EINVAL;
+  *max_n = static_capacity(I, nullptr);
+  return LGX_OK;
+}
+
+int lgx_eval_batch_static(const lgx_instance *I, uint64_t seed, const uint64_t *d_ids, uint64_t first_id, uint64_t n,
+                          double *d_cost, double *d_path_km, double *d_makespan_h, uint8_t *d_feasible, void *stream)
+{
+  if (!I) return LGX_EINVAL;
+  size_t qoff = 0;
+  if (n > static_capacity(I, &qoff)) return LGX_ESTATIC;             // before anything is touched or launched
+  if (n == 0) return LGX_OK;
+  int rc = check_device(I);
+  if (rc != LGX_OK) return rc;
+  unsigned char *base = nullptr;
+  rc = static_scratch(I->device, &base);                             // first call on this device: looks the address up
+  if (rc != LGX_OK) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  KParams P{};
+  fill_round_keys(P, seed);
+  P.ids = d_ids; P.first_id = first_id;
+  P.cost = d_cost; P.path_km = d_path_km; P.makespan_h = d_makespan_h; P.feasible = d_feasible;
+  KernelFn ka, kb; pick_kernels<MODE_EVAL>(I->hdr, ka, kb);
+  if (I->cut_warp) ka = pick_decode_cut_w(I->hdr, MODE_EVAL);
+  Workspace W;                                                        // same layout as ws_alloc, inside the static array
+  W.base = base;
+  W.cap = (n + 31) / 32 * 32;                                         // one kernel pair takes the whole call
+  W.q_count = reinterpret_cast<unsigned int *>(base);
+  W.done = W.q_count + 1; W.ctr_a = W.q_count + 2; W.ctr_b = W.q_count + 3;
+  W.result = reinterpret_cast<unsigned long long *>(base + 16);
+  W.block_best = reinterpret_cast<unsigned long long *>(base + 64);
+  W.queue = reinterpret_cast<uint32_t *>(base + qoff);
+  // the array still holds the previous call's counters: the queue length and the work counters must start at zero
+  CU(cudaMemsetAsync(base, 0, 64, st));
+  return run_chunks(I, ka, kb, P, n, W, st, false);
+}
+
+}  // extern "C"
+
+#endif  // LGX_EMU
 
 // ================================================================== Algorithm 1
 
