@@ -181,3 +181,84 @@ def test_create_rejects_bad_input():
         lgo.Oracle(inst)
     assert e.value.code == -2
     lgo.Oracle(ok)
+
+
+# ---- P9: the decoder's draw ORDER, derived by hand from published random words (S1-S3; PAPER.md:L233,
+#      "identical random process control"; L116-118 the decision variables the draws fix).  The invariants and the
+#      chi-square tests of test_oracle_invariants.py would still pass with a wrong draw index that keeps the
+#      distribution; these values would not.
+
+def _kat_row0():
+    for l in open(os.path.join(HERE, "golden", "philox4x32_10_kat.txt")):
+        p = l.split()
+        if p and not l.startswith("#"):
+            return [int(x, 16) for x in p]
+    raise AssertionError("no known-answer vector")
+
+
+def test_bp_partition_of_seed0_id0_from_the_published_vector():
+    """Stream 0 / block 0 of (seed 0, id 0) has counter (0, 0, 0, 0) and key (0, 0): exactly the first published
+    known-answer vector of Philox4x32-10, output words w = (6627e8d5, e169c58d, bc57ac4c, 9b00dbd8).
+    S2 with n = N_B = 3 items, k = N_T = 2 bins, below(x, m) = floor(x m / 2^32):
+      a = [0 1 2]
+      i = 2: j = below(w0, 3) = floor(0x6627e8d5 * 3 / 2^32) = floor(1.197) = 1 -> swap a[2], a[1] -> a = [0 2 1]
+      i = 1: j = below(w1, 2) = top bit of 0xe169c58d            = 1 -> swap a[1], a[1] -> a = [0 2 1]
+      consumption p = 0 reads a[2] = BP 1 -> bin 0 = tour 0, position 0
+                  p = 1 reads a[1] = BP 2 -> bin 1 = tour 1, position 0
+                  p = 2 reads a[0] = BP 0 -> bin below(draw 2 + (2 - 2) = w2, 2) = top bit of 0xbc57ac4c = 1 -> tour 1, position 1
+    so bp_tour = [1 0 1] and bp_pos = [1 0 0] (indexed by BP)."""
+    kat = _kat_row0()
+    assert kat[:6] == [0, 0, 0, 0, 0, 0] and kat[6:] == [0x6627e8d5, 0xe169c58d, 0xbc57ac4c, 0x9b00dbd8]
+    w = kat[6:]
+    assert [(w[0] * 3) >> 32, (w[1] * 2) >> 32, (w[2] * 2) >> 32] == [1, 1, 1]
+    from paper_1909_10286_b200 import workloads as wl
+    inst = wl.make("toy")
+    assert (inst.n_bps, inst.n_tours, inst.n_fields) == (3, 2, 11)
+    plan = lgo.Oracle(inst).decode_batch(0, first_id=0, n=1)
+    assert plan["bp_tour"][0].tolist() == [1, 0, 1]
+    assert plan["bp_pos"][0].tolist() == [1, 0, 0]
+
+
+def test_first_field_swaps_of_seed0_id0_from_the_curand_header(tmp_path):
+    """Stream 3 (field permutation) and stream 4 (extras), block 0 of (seed 0, id 0): counters (0, 0, 3, 0) and
+    (0, 0, 4, 0), key (0, 0).  The words come from NVIDIA's cuRAND header compiled for the host (an implementation that
+    is neither the oracle's nor the kernels').
+    S3 over N_F = 11 fields: i = 10: j = below(w0, 11), swap a[10], a[j]; i = 9: j = below(w1, 10), swap a[9], a[j].
+    a[10] and a[9] are final after their steps and are the first two fields consumed.  The first BP in plan order is
+    BP 1 (tour 0's only BP, see the pin above), the second BP 2 (first on tour 1).  Field a[10] goes to BP 1 at
+    position 0.  In the toy instance any one field covers BP 1's demand many times over, so the minimal prefix ends
+    there and the first extras draw x = word 0 of stream 4 decides where a[9] goes: x < extra_field_thresh -> BP 1,
+    position 1; otherwise BP 1 is closed and a[9] opens BP 2 at position 0."""
+    import shutil, subprocess, textwrap
+    if shutil.which("nvcc") is None:
+        pytest.skip("nvcc not found")
+    src = tmp_path / "w.cu"
+    src.write_text(textwrap.dedent(r"""
+        #include <cstdio>
+        #include <cuda_runtime.h>
+        #define QUALIFIERS static inline __host__ __device__
+        #include <curand_philox4x32_x.h>
+        int main() {
+          for (unsigned s = 3; s <= 4; ++s) {
+            uint4 r = curand_Philox4x32_10(make_uint4(0u, 0u, s, 0u), make_uint2(0u, 0u));
+            printf("%08x %08x %08x %08x\n", r.x, r.y, r.z, r.w);
+          }
+          return 0;
+        }"""))
+    exe = tmp_path / "w"
+    r = subprocess.run(["nvcc", "-O1", "-o", str(exe), str(src)], capture_output=True, text=True)
+    if r.returncode != 0:
+        pytest.skip("cuRAND header does not compile for the host here: " + r.stderr[-300:])
+    words = [int(x, 16) for x in subprocess.run([str(exe)], capture_output=True, text=True, check=True).stdout.split()]
+    w3, w4 = words[:4], words[4:]
+    a = list(range(11))
+    j = (w3[0] * 11) >> 32; a[10], a[j] = a[j], a[10]
+    j = (w3[1] * 10) >> 32; a[9], a[j] = a[j], a[9]
+    from paper_1909_10286_b200 import workloads as wl
+    inst = wl.make("toy")
+    assert inst.field_supply_t.min() > 2.0 * inst.bp_demand_t[1]          # one field is a complete minimal prefix of BP 1
+    second = (1, 1) if w4[0] < inst.extra_field_thresh else (2, 0)
+    plan = lgo.Oracle(inst).decode_batch(0, first_id=0, n=1)
+    fb, fp = plan["field_bp"][0], plan["field_pos"][0]
+    assert (int(fb[a[10]]), int(fp[a[10]])) == (1, 0)
+    assert (int(fb[a[9]]), int(fp[a[9]])) == second
