@@ -2,7 +2,10 @@
 // that their index arithmetic and memory layout can be checked on a CPU under AddressSanitizer / UBSan and compared
 // with the oracle without a GPU.  Single-lane emulation: every block runs ONE thread, blocks run one after the other,
 // warp collectives degenerate to the identity; every "device" allocation and every launch's dynamic shared memory is
-// a heap block of exactly the requested size, so an out-of-bounds index trips the sanitizer.  Only valid for kernels
+// a heap block of exactly the requested size (shared memory: rounded up to 16 for alignment, the tail poisoned under
+// ASan), so an out-of-bounds index trips the sanitizer.  Kernels are entered through a function-pointer cast to a
+// by-value dummy struct (see cudaLaunchKernel below): that call is itself outside the C++ standard, so UBSan vouches
+// for the kernels' arithmetic and indexing, not for the launch shim.  Only valid for kernels
 // without block-wide cooperation beyond "copy the image, barrier" (lgx_decode_cut, lgx_walk_finish); the Algorithm-1
 // kernels are not emulated (cooperative launches fail here).  This is NOT a CPU fallback of the product: nothing in
 // the package builds, loads or links it; it checks what compute-sanitizer's memcheck would, not races.
@@ -14,6 +17,14 @@
 #include <algorithm>
 #include <cstdio>
 #define LGX_EMU 1
+#if defined(__SANITIZE_ADDRESS__)
+#include <sanitizer/asan_interface.h>
+#define LGX_EMU_POISON(p, n)   do { if ((n) != 0) __asan_poison_memory_region((p), (n)); } while (0)
+#define LGX_EMU_UNPOISON(p, n) do { if ((n) != 0) __asan_unpoison_memory_region((p), (n)); } while (0)
+#else
+#define LGX_EMU_POISON(p, n)   do { } while (0)
+#define LGX_EMU_UNPOISON(p, n) do { } while (0)
+#endif
 #define LGX_LANES 1u
 #define LGX_BLOCK_THREADS(t) 1u       /* one thread per block: shared memory sized for one candidate */
 #define LGX_DYN_SMEM(name) uint8_t *name = lgx_emu::g_smem
@@ -117,8 +128,15 @@ static inline cudaError_t cudaLaunchKernel(const void *fn, dim3 grid, dim3 block
   EmuBig big; memset(&big, 0, sizeof big); memcpy(&big, args[0], lgx_emu_param_bytes());
   lgx_emu::gridDim = grid; lgx_emu::blockDim = dim3(1); lgx_emu::threadIdx = dim3(0);
   for (unsigned b = 0; b < grid.x; ++b) {
-    lgx_emu::g_smem = (uint8_t *)aligned_alloc(16, (smem + 15) / 16 * 16 + 16);
+    // exactly `smem` addressable bytes: aligned_alloc wants a multiple of the alignment, so the block is rounded up to 16
+    // and, under AddressSanitizer, the 0..15 bytes behind the launch's size are poisoned (byte-exact: ASan's shadow encodes
+    // "first k bytes of a granule addressable"); an index one past the last state row or sentinel cell is reported.
+    // Without ASan the tail is ordinary heap slack.
+    const size_t rounded = (std::max<size_t>(smem, 1) + 15) / 16 * 16;
+    lgx_emu::g_smem = (uint8_t *)aligned_alloc(16, rounded);
+    LGX_EMU_POISON(lgx_emu::g_smem + smem, rounded - smem);
     lgx_emu::blockIdx = dim3(b); ((void (*)(EmuBig))fn)(big);
+    LGX_EMU_UNPOISON(lgx_emu::g_smem + smem, rounded - smem);
     free(lgx_emu::g_smem); lgx_emu::g_smem = nullptr;
   }
   return cudaSuccess; }
