@@ -66,13 +66,18 @@ extern "C" {
 #define LGX_OPT_THREADS_MV  3    /* threads per block of the move kernels: multiple of 32, 64 .. what fits      */
 #define LGX_OPT_CHUNK_LOG2  4    /* log2 of the candidates per kernel pair, 10 .. 26 (queue memory = chunk * record bytes) */
 #define LGX_OPT_CUT_WARP    6    /* 1: the decode/cut kernel works one candidate per WARP (lgx_decode_cut_w; needs N_F > 255, no
-                                    zero-demand BP and room for its per-warp state: else LGX_EINVAL), 0 (default): one per thread.
+                                    zero-demand BP, room for the per-warp state of >= 4 warps, and the 2 N_B - 1 - N_T draws of the BP
+                                    partition, rounded up to whole Philox blocks, within the permutation's 32-bit words
+                                    (4 ceil((2 N_B - 1 - N_T) / 4) <= ceil(N_F / 2)): else LGX_EINVAL; lgx_instance_query what 23
+                                    tells), 0 (default): one per thread.
                                     An alternative mapping kept for measurement: slower on every config so far */
 #define LGX_OPT_WALK_LOCKSTEP 7  /* 1: the warps of a walk/finish block draw their queue records together (one barrier per batch; they
                                     then share instruction-cache lines), 0: every warp on its own.  Only with coordinates (distance modes 1, 2;
                                     ignored with the tables, where it measured slower).  Default: 1 with coordinates and N_F < 1024 */
 #define LGX_OPT_SQ_SHIFT    5    /* log2 of the replication of the s_q table in the decode/cut kernel's shared memory, 0 .. 5;
-                                    synchronises the device and re-uploads the image                            */
+                                    synchronises the device, uploads a new image and then resets LGX_OPT_THREADS_A and
+                                    LGX_OPT_CUT_WARP to their defaults for the new image size (set this key first).  On
+                                    failure (LGX_ETOOBIG, LGX_ECUDA) the instance keeps its previous image and settings */
 
 typedef struct lgx_instance lgx_instance;   /* opaque; owns host + device copies */
 
@@ -249,7 +254,8 @@ int lgx_init_plan(const lgx_instance *inst,
  * v = floor(w0 (N_F+N_B) / 2^32) is a field (v < N_F) or BP v-N_F; a field goes to BP floor(w1 N_B / 2^32),
  * a BP (with all its fields) to tour floor(w1 N_T / 2^32); position floor(w2 (len+1) / 2^32), len = the
  * target list's length after the removal.  Outputs are DEVICE pointers (any may be NULL), row i-first_id.
- * The plan is copied before the call returns; the kernel is asynchronous on cuda_stream.            */
+ * The plan arrays are copied into a buffer of the library's before the call returns (the caller may change them
+ * at once, page-locked or not); the upload from that buffer and the kernel are asynchronous on cuda_stream.  */
 int lgx_move_eval_batch(const lgx_instance *inst,
                         const uint8_t *h_bp_tour, const uint8_t *h_bp_pos,
                         const uint16_t *h_field_bp, const uint16_t *h_field_pos,

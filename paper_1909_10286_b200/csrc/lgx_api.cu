@@ -95,25 +95,31 @@ int check_device(const lgx_instance *I)
 }
 
 // Image A: s_q replicated 2^sq_shift times (replica r of field f at (f << sq_shift) + r: lanes of a warp read
-// different banks whatever field they hold) and the demand quanta.  Uploads it.
+// different banks whatever field they hold) and the demand quanta.  Built and uploaded into a NEW device buffer; the
+// instance (header offsets, host copy, device pointer) changes only once the upload has succeeded, so a failure
+// leaves it exactly as it was, still usable with its previous image.
 int build_image_a(lgx_instance *I, uint32_t sq_shift)
 {
   ImgHdr &H = I->hdr;
   const uint32_t nf = (uint32_t)H.n_f, nb = (uint32_t)H.n_b;
-  H.sq_shift = sq_shift;
   uint32_t off = 0;
-  H.off_sq = off; off = align16(off + 4u * (nf << sq_shift));
-  H.off_dq = off; off = align16(off + 4u * nb);
-  H.image_bytes = off;
-  I->image.assign(H.image_bytes, 0);
-  uint32_t *sq = reinterpret_cast<uint32_t *>(I->image.data() + H.off_sq);
+  const uint32_t off_sq = off; off = align16(off + 4u * (nf << sq_shift));
+  const uint32_t off_dq = off; off = align16(off + 4u * nb);
+  const uint32_t bytes = off;
+  std::vector<uint8_t> img(bytes, 0);
+  uint32_t *sq = reinterpret_cast<uint32_t *>(img.data() + off_sq);
   for (uint32_t f = 0; f < nf; ++f)
     for (uint32_t r = 0; r < (1u << sq_shift); ++r) sq[(f << sq_shift) + r] = I->s_q[f];
-  uint32_t *dq = reinterpret_cast<uint32_t *>(I->image.data() + H.off_dq);
+  uint32_t *dq = reinterpret_cast<uint32_t *>(img.data() + off_dq);
   for (uint32_t b = 0; b < nb; ++b) dq[b] = I->d_q[b];
-  if (I->d_image && I->d_image_cap < H.image_bytes) { cudaFree(I->d_image); I->d_image = nullptr; }
-  if (!I->d_image) { CU(cudaMalloc((void **)&I->d_image, H.image_bytes)); I->d_image_cap = H.image_bytes; }
-  CU(cudaMemcpy(I->d_image, I->image.data(), H.image_bytes, cudaMemcpyHostToDevice));
+  uint8_t *d_new = nullptr;
+  CU(cudaMalloc((void **)&d_new, bytes));
+  cudaError_t e = cudaMemcpy(d_new, img.data(), bytes, cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) { cudaFree(d_new); return cuda_fail(e, "cudaMemcpy(image A)"); }
+  if (I->d_image) cudaFree(I->d_image);
+  I->d_image = d_new; I->d_image_cap = bytes;
+  I->image.swap(img);
+  H.sq_shift = sq_shift; H.off_sq = off_sq; H.off_dq = off_dq; H.image_bytes = bytes;
   return LGX_OK;
 }
 
@@ -121,6 +127,31 @@ int64_t fit_threads(int64_t budget, int64_t image, int64_t state, int64_t cap)
 {
   const int64_t t = (budget - image) / std::max<int64_t>(state, 1);
   return std::min<int64_t>(t, cap) / 32 * 32;
+}
+
+// Launch configuration of the decode/cut kernel as a function of image A's size: the create-time defaults.  Used by
+// lgx_instance_create and again whenever LGX_OPT_SQ_SHIFT has rebuilt the image (it resets LGX_OPT_THREADS_A and
+// LGX_OPT_CUT_WARP to these defaults; nothing is derived from the values in place before).
+void config_decode_cut(lgx_instance *I)
+{
+  const ImgHdr &H = I->hdr;
+  const int64_t budget = I->smem_budget;
+  I->threads_a     = (int)fit_threads(budget, H.image_bytes, (int64_t)I->a_state, H.perm16 ? kMaxThreadsA16 : kMaxThreadsA);
+  I->threads_a_dec = (int)fit_threads(budget, H.image_bytes, (int64_t)I->a_state_dec, H.perm16 ? kMaxThreadsA16 : kMaxThreadsA);
+#ifndef LGX_EMU
+  {
+    // one candidate per warp (lgx_cutw.cuh): possible with 16-bit field ids, no zero-demand BP, the BP partition's draws
+    // inside the permutation's words, and room for at least four warps.  Opt-in (LGX_OPT_CUT_WARP): it measured slower
+    // than the per-thread mapping on every config (DESIGN.md s5), so it is never chosen by default
+    const CutWLayout WL = cutw_layout(H);
+    const int64_t wfit = std::min<int64_t>((budget - (int64_t)H.image_bytes) / (int64_t)WL.bytes, kMaxThreadsW / 32);
+    const uint32_t draw_words = 4u * cdiv(2u * (uint32_t)H.n_b - 1u - (uint32_t)H.n_t, 4u);
+    I->w_bytes = WL.bytes;
+    I->warps_w = (int)std::max<int64_t>(wfit, 0);
+    I->cut_warp_ok = (H.perm16 && !H.zero_demand && wfit >= 4 && draw_words <= H.n_perm_words) ? 1 : 0;
+    I->cut_warp = 0;
+  }
+#endif
 }
 
 // Stream-ordered workspace memory (the queue of feasible candidates, a few hundred bytes of counters) comes from ONE
@@ -143,8 +174,11 @@ int device_pool(int device, cudaMemPool_t *out)
     props.location.id = device;
     cudaMemPool_t pool = nullptr;
     CU(cudaMemPoolCreate(&pool, &props));
+    // without the threshold every freed workspace goes back to the driver at the next synchronisation and each call
+    // maps its queue again (correct, but several times slower end to end): treat a refusal as an error, not as a detail
     uint64_t keep = ~0ull;
-    cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    cudaError_t e = cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    if (e != cudaSuccess) { cudaMemPoolDestroy(pool); return cuda_fail(e, "cudaMemPoolSetAttribute(release threshold)"); }
     g_pools[device] = pool;
   }
   *out = g_pools[device];
@@ -413,24 +447,9 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   while (sq_shift < 5u && 4ull * ((uint64_t)nf << (sq_shift + 1u)) <= 16ull * 1024) ++sq_shift;
   int rc = build_image_a(I, sq_shift);
   if (rc != LGX_OK) { free_instance(I); return rc; }
-  I->threads_a     = (int)fit_threads(budget, H.image_bytes, (int64_t)I->a_state, H.perm16 ? kMaxThreadsA16 : kMaxThreadsA);
-  I->threads_a_dec = (int)fit_threads(budget, H.image_bytes, (int64_t)I->a_state_dec, H.perm16 ? kMaxThreadsA16 : kMaxThreadsA);
+  config_decode_cut(I);
   I->threads_b     = (int)fit_threads(budget, H.imagec_bytes, (int64_t)I->b_state, H.coords == 0 ? kMaxThreadsB : kMaxThreadsBC);
   if (I->threads_a < 32 || I->threads_a_dec < 32 || I->threads_b < 32) { free_instance(I); return LGX_ETOOBIG; }
-#ifndef LGX_EMU
-  {
-    // one candidate per warp (lgx_cutw.cuh): possible with 16-bit field ids, no zero-demand BP, the BP partition's draws
-    // inside the permutation's words, and room for at least four warps.  Opt-in (LGX_OPT_CUT_WARP): it measured slower
-    // than the per-thread mapping on every config (DESIGN.md s5), so it is never chosen by default
-    const CutWLayout WL = cutw_layout(H);
-    const int64_t wfit = std::min<int64_t>((budget - (int64_t)H.image_bytes) / (int64_t)WL.bytes, kMaxThreadsW / 32);
-    const uint32_t draw_words = 4u * cdiv(2u * (uint32_t)nb - 1u - (uint32_t)nt, 4u);
-    I->w_bytes = WL.bytes;
-    I->warps_w = (int)std::max<int64_t>(wfit, 0);
-    I->cut_warp_ok = (H.perm16 && !H.zero_demand && wfit >= 4 && draw_words <= H.n_perm_words) ? 1 : 0;
-    I->cut_warp = 0;
-  }
-#endif
   I->grid = I->sm_count;                       // one persistent block per SM
   // block-synchronous work fetch of lgx_walk_finish: measured -6 % (Large) and -10 % (Sweep) kernel time with coordinates, where warps
   // in different phases evict each other's code; +3.6 % with the tables (Medium) and +1.7 % on paper_scale, whose warps spend
@@ -597,14 +616,11 @@ int lgx_instance_set_option(lgx_instance *I, int key, int64_t value)
       const int64_t img = 16 + 4ll * ((int64_t)H.n_f << value) + 16 + 4ll * H.n_b;
       if (fit_threads(budget, img, (int64_t)I->a_state_dec, H.perm16 ? kMaxThreadsA16 : kMaxThreadsA) < 32) return LGX_ETOOBIG;
       int rc = check_device(I);
-      if (rc == LGX_OK) { cudaDeviceSynchronize(); rc = build_image_a(I, (uint32_t)value); }
       if (rc != LGX_OK) return rc;
-      I->threads_a     = (int)std::min<int64_t>(I->threads_a, fit_threads(budget, H.image_bytes, (int64_t)I->a_state, H.perm16 ? kMaxThreadsA16 : kMaxThreadsA));
-      I->threads_a_dec = (int)std::min<int64_t>(I->threads_a_dec, fit_threads(budget, H.image_bytes, (int64_t)I->a_state_dec, H.perm16 ? kMaxThreadsA16 : kMaxThreadsA));
-      if (I->w_bytes) {
-        I->warps_w = (int)std::min<int64_t>((budget - (int64_t)H.image_bytes) / (int64_t)I->w_bytes, 32);
-        if (I->warps_w < 4) { I->cut_warp_ok = 0; I->cut_warp = 0; }
-      }
+      CU(cudaDeviceSynchronize());                       // no kernel may still be reading the image that is replaced
+      rc = build_image_a(I, (uint32_t)value);            // on failure the instance keeps its previous image and configuration
+      if (rc != LGX_OK) return rc;
+      config_decode_cut(I);                              // create-time defaults for the new image size
       return LGX_OK;
     }
     default: return LGX_EINVAL;
@@ -1019,15 +1035,22 @@ int plan_dev_alloc(const lgx_instance *I, cudaStream_t st, PlanDev &D)
   return LGX_OK;
 }
 
+// The six host arrays are packed into ONE pageable buffer of the library's, in the device layout of plan_dev_alloc, and
+// uploaded with one copy.  A copy from pageable memory has left its source when cudaMemcpyAsync returns (the driver stages
+// it), so neither the caller's arrays (which may be page-locked: a direct copy from those would still be in flight after the
+// return) nor the local buffer are read after this function.
 int plan_upload(const ImgHdr &H, const PlanDev &D, const uint8_t *bt, const uint8_t *bq, const uint16_t *fb, const uint16_t *fq,
                 const uint8_t *hu, const uint8_t *su, cudaStream_t st)
 {
-  CU(cudaMemcpyAsync(D.bt, bt, (size_t)H.n_b, cudaMemcpyHostToDevice, st));
-  CU(cudaMemcpyAsync(D.bq, bq, (size_t)H.n_b, cudaMemcpyHostToDevice, st));
-  CU(cudaMemcpyAsync(D.fb, fb, 2 * (size_t)H.n_f, cudaMemcpyHostToDevice, st));
-  CU(cudaMemcpyAsync(D.fq, fq, 2 * (size_t)H.n_f, cudaMemcpyHostToDevice, st));
-  CU(cudaMemcpyAsync(D.hu, hu, (size_t)H.n_hu, cudaMemcpyHostToDevice, st));
-  CU(cudaMemcpyAsync(D.su, su, (size_t)H.n_su, cudaMemcpyHostToDevice, st));
+  std::vector<uint8_t> stage(D.bytes);
+  uint8_t *s0 = stage.data();
+  std::memcpy(s0 + ((uint8_t *)D.fb - D.base), fb, 2 * (size_t)H.n_f);
+  std::memcpy(s0 + ((uint8_t *)D.fq - D.base), fq, 2 * (size_t)H.n_f);
+  std::memcpy(s0 + (D.bt - D.base), bt, (size_t)H.n_b);
+  std::memcpy(s0 + (D.bq - D.base), bq, (size_t)H.n_b);
+  std::memcpy(s0 + (D.hu - D.base), hu, (size_t)H.n_hu);
+  std::memcpy(s0 + (D.su - D.base), su, (size_t)H.n_su);
+  CU(cudaMemcpyAsync(D.base, s0, D.bytes, cudaMemcpyHostToDevice, st));
   return LGX_OK;
 }
 
