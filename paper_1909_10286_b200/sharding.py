@@ -43,8 +43,8 @@ def search_sharded(search_fn, seed: int, budget: int, rank: int, world: int, fir
     import torch.distributed as dist
     first, n = split_range(budget, world, rank, first_id)
     local = search_fn(seed, n, first) if n > 0 else None
-    if world == 1:
-        return combine([local])
+    if world == 1 and not (dist.is_available() and dist.is_initialized()):
+        return combine([local])          # no launcher, no process group: nothing to exchange
     dev = torch.device("cuda", torch.cuda.current_device()) if dist.get_backend() == "nccl" else torch.device("cpu")
     # (valid, cost bits, id) as int64 words; bit patterns are moved, never re-rounded
     def s64(v):
