@@ -54,6 +54,44 @@ def w_alg(inst, a2_iters):
     return (decode + pass1, finish), (decode + cut, geo1 + finish)
 
 
+def w_alg_coords(inst, a2_iters, mode):
+    """The same MODEL with the distances computed from coordinates (a leg = 2 sub, 2 mul, 1 add and an
+    FP64 square root ~ 20 thread-instructions instead of one table look-up ~ 3).  Distance mode 1 (coordinates only):
+    the field->BP leg of pass 1, the route leg and the field->BP leg of pass 2 = 3 legs per field; mode 2 (field x BP
+    table + coordinates): the route leg only.  Returns the walk/finish kernel's work per feasible candidate."""
+    (_, _), (_, w_b) = w_alg(inst, a2_iters)
+    legs = {0: 0, 1: 3, 2: 1}[mode]
+    return w_b + 17 * legs * inst.n_fields
+
+
+# PROFILE CONSTANTS (not measured in this run): each pipe's utilisation (sm__inst_executed_pipe_*.avg.pct_of_peak_sustained_active)
+# in ONE captured launch of each kernel, with that launch's duration and candidates, from the `ncu --set full` capture named
+# per entry.  pipes_of() scales them to this run's time per candidate; the binding pipe is the busiest one.  The pipe peaks
+# measured IN this run (lgx_selftest 1..5, `pipe_peaks`) say what those pipes sustain on this GPU: ALU 2, FP64 2, IMAD.WIDE 1,
+# shared-memory byte accesses 1, MUFU.RSQ64H 0.5 warp-instructions/clk/SM against the schedulers' 4.
+PIPE_MIX = {
+    "medium": {"file": "profiles/r03_medium_ncu_full.md",
+               "lgx_decode_cut":  {"ms": 3.862624, "candidates": 16777216, "pct": {"alu": 57.93, "fma": 26.90, "lsu": 43.59, "fp64": 0.0, "xu": 0.66}},
+               "lgx_walk_finish": {"ms": 3.505408, "candidates": 16777216 * 0.23804, "pct": {"alu": 44.18, "fma": 19.13, "lsu": 29.90, "fp64": 12.75, "xu": 11.33}}},
+}
+
+
+PIPE_OF = {"alu": "alu_lop3", "fma": "imad_wide_u32", "lsu": "lds_sts_u8", "fp64": "fp64_dfma", "xu": "mufu_rsq64h"}
+
+
+def pipe_peaks(binding, n_sm):
+    """Sustained warp-instructions per clock per SM of five pipes, measured by lgx_selftest what = 1..5."""
+    names = {1: "imad_wide_u32", 2: "alu_lop3", 3: "lds_sts_u8", 4: "fp64_dfma", 5: "mufu_rsq64h"}
+    out = {}
+    for what, nm in names.items():
+        binding.selftest(what, 1 << 10)
+        n_inst, cyc = binding.selftest(what, 1 << 14)
+        out[nm] = n_inst / max(cyc, 1) / n_sm
+    out["unit"] = "warp-instructions / clk / SM (scheduler limit: 4)"
+    out["how"] = "lgx_selftest what=1..5: 8 independent chains per thread, 2 x 1024 threads per SM, cycles by clock64 in the kernel"
+    return out
+
+
 SM_MAX_MHZ_FALLBACK = 1965.0
 # PROFILE CONSTANTS (not measured in this run): dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the
 # config's dominant kernel from the `ncu --set full` captures summarised under profiles/ (file named per entry),
@@ -272,7 +310,6 @@ def main():
     ap.add_argument("--chunk-log2", type=int, default=None, help="candidates per kernel pair (LGX_OPT_CHUNK_LOG2; profiling)")
     ap.add_argument("--threads-a", type=int, default=None, help="LGX_OPT_THREADS_A (tuning)")
     ap.add_argument("--threads-b", type=int, default=None, help="LGX_OPT_THREADS_B (tuning)")
-    ap.add_argument("--cut-warp", type=int, default=None, help="LGX_OPT_CUT_WARP: 1 = the per-warp decode/cut kernel (alternative mapping; profiling)")
     ap.add_argument("--walk-lockstep", type=int, default=None, help="LGX_OPT_WALK_LOCKSTEP (tuning)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--alg1-workload", default="paper_scale", help="instance of the Algorithm 1 leg (SURVEY §8(f) N1/N3)")
@@ -319,7 +356,7 @@ def main():
     inst = wl.make(args.workload)
     per_gpu = 1 << (args.batch_log2 if args.batch_log2 is not None else min(28, inst.budget.bit_length() - 1))
     total = per_gpu * world                      # weak scaling: fixed ids per GPU
-    opts = ((4, args.chunk_log2), (1, args.threads_a), (2, args.threads_b), (6, args.cut_warp), (7, args.walk_lockstep))
+    opts = ((4, args.chunk_log2), (1, args.threads_a), (2, args.threads_b), (7, args.walk_lockstep))
 
     def new_instance(ins):
         gi = binding.Instance(ins)
@@ -330,6 +367,7 @@ def main():
 
     g = new_instance(inst)
     info = g.info()
+    binding_mode = {args.workload: info["coords"]}           # distance mode per config (lgx_instance_query 4)
     stream = torch.cuda.current_stream()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
 
@@ -448,6 +486,21 @@ def main():
     n_sm = info["sm_count"]
     peak_ginst = n_sm * 4 * 32 * sm_max * 1e6 / 1e9          # thread-instructions/s at max clock
     cores = os.cpu_count() or 1
+    ppeaks = pipe_peaks(binding, n_sm)                       # measured in this run (five short kernels)
+
+    def pipes_of(name, kernel, ms_per_cand):
+        """Utilisation of each pipe by `kernel` in this run: the captured launch's utilisation (profile constant, PIPE_MIX)
+        scaled by captured / current time per candidate.  The binding pipe is the busiest."""
+        mix = PIPE_MIX.get(name, {}).get(kernel)
+        if not mix or ms_per_cand <= 0:
+            return None
+        scale = (mix["ms"] / mix["candidates"]) / ms_per_cand
+        util = {pipe: pct / 100.0 * scale for pipe, pct in mix["pct"].items()}
+        bind = max(util, key=util.get)
+        return {"binding_pipe": bind, "frac_of_binding_pipe": util[bind], "pipe_utilisation": util,
+                "binding_pipe_peak_warp_inst_per_clk_per_sm": ppeaks.get(PIPE_OF[bind]),
+                "source": "pipe utilisation of the captured launch in %s (profile constant) scaled to this run's time per candidate; "
+                          "pipe peaks measured in this run" % PIPE_MIX[name]["file"]}
 
     def roofline_of(ins, name, feas, a2, rate_per_gpu, ns_a_, ns_b_, pairs, cand_timed, rec_bytes):
         """Issue roofline of one config from the work MODEL w_alg (a model) and the measured kernel times."""
@@ -460,6 +513,20 @@ def main():
         ach_d, ms_d = (ach_a, ms_a_) if a_dominant else (ach_b, ms_b_)
         ach_r1 = (w_dw + feas * w_fin) * rate_per_gpu / 1e9
         ach_strict = (w_a + feas * w_b) * rate_per_gpu / 1e9
+        mode = {"toy": 0, "small": 0, "medium": 0}.get(name)
+        w_b_coords = None
+        if ms_b_ > 0:
+            try:
+                mode = binding_mode[name]
+            except KeyError:
+                pass
+            if mode:
+                w_b_coords = w_alg_coords(ins, a2, mode)
+        ach_b_coords = per_launch * feas * w_b_coords / (ms_b_ * 1e-3) / 1e9 if w_b_coords and ms_b_ > 0 else None
+        # each kernel's share of the step's candidates/s: the kernel alone would run at per_launch / its launch time
+        pa = pipes_of(name, "lgx_decode_cut", ms_a_ / per_launch) if ms_a_ > 0 else None
+        pb = pipes_of(name, "lgx_walk_finish", ms_b_ / max(per_launch * feas, 1e-9)) if ms_b_ > 0 else None
+        pd = pa if a_dominant else pb
         tr = TRAFFIC.get(name)
         if tr:      # the dominant kernel's bytes, scaled from the captured launch to this run's candidates per launch
             tr = {"file": tr[0], "candidates_per_launch": tr[1], "bytes_per_launch": (tr[2] if a_dominant else tr[3]) * per_launch / tr[1]}
@@ -470,15 +537,21 @@ def main():
                 "traffic_source": ("profile constant, not measured in this run: dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel in %s "
                                    "(%d candidates in the captured launch), scaled to this run's candidates per launch; it is the queue of "
                                    "feasible candidates, the path's algorithmic HBM bytes are 0" % (tr["file"], tr["candidates_per_launch"])) if tr else None,
+                "pipe_peaks": ppeaks,
+                "binding_pipe": pd["binding_pipe"] if pd else None, "frac_of_binding_pipe": pd["frac_of_binding_pipe"] if pd else None,
                 "launch_ms": ms_d, "launches_timed": pairs, "candidates_per_launch": per_launch,
                 "work_model": "w_alg (bench.py; DESIGN.md s8): a hand model of the thread-instructions the method needs, not a measured count; "
                               "A2 = mean accepted Algorithm-2 moves, oracle-measured in this run",
                 "alg2_moves_mean": a2,
                 "peak_source": f"{n_sm} SMs x 4 schedulers x 32 lanes x {sm_max:.0f} MHz ({pk_src} sm_max_mhz; DESIGN.md s8)",
                 "kernels": [{"kernel": "lgx_decode_cut", "launch_ms": ms_a_, "achieved": ach_a, "frac": ach_a / peak_ginst if ach_a else None,
-                             "w_alg_thread_inst_per_candidate": w_a},
+                             "w_alg_thread_inst_per_candidate": w_a, "pipes": pa},
                             {"kernel": "lgx_walk_finish", "launch_ms": ms_b_, "achieved": ach_b, "frac": ach_b / peak_ginst if ach_b else None,
-                             "w_alg_thread_inst_per_feasible_candidate": w_b, "feasible_fraction": feas}],
+                             "w_alg_thread_inst_per_feasible_candidate": w_b, "feasible_fraction": feas, "pipes": pb,
+                             "coordinate_model": ({"distance_mode": mode, "w_alg_thread_inst_per_feasible_candidate": w_b_coords,
+                                                   "achieved": ach_b_coords, "frac": ach_b_coords / peak_ginst,
+                                                   "model": "w_alg + 17 thread-inst per leg computed from coordinates (SURVEY.md s8(d)): "
+                                                            "3 legs per field in mode 1, 1 in mode 2"} if ach_b_coords else None)}],
                 "whole_step": {"w_alg_thread_inst_per_candidate": w_dw + feas * w_fin, "achieved": ach_r1, "frac": ach_r1 / peak_ginst,
                                "model": "round-1 model (unchanged): decode + pass 1 charged to every candidate"},
                 "whole_step_strict": {"w_alg_thread_inst_per_candidate": w_a + feas * w_b, "achieved": ach_strict, "frac": ach_strict / peak_ginst,
@@ -516,6 +589,7 @@ def main():
         for name in ALL_CONFIGS:
             ins = wl.make(name)
             gi = g if name == args.workload and not any(v is not None for _, v in opts) else binding.Instance(ins)
+            binding_mode[name] = gi.query(4)
             n_s = 1 << CONFIG_SEARCH_LOG2[name]
             gi.search(ins.seed, n_s // 4); gi.search(ins.seed, n_s // 4); gi.search(ins.seed, n_s // 4)      # W = 3 warm-up calls
             # the reported rate comes from a call WITHOUT the per-kernel timing hook (which creates and records three events
@@ -544,7 +618,7 @@ def main():
             else:
                 a2 = {"toy": 2.3, "small": 5.5, "medium": 9.8, "large": 12.9, "sweep": 18.5, "paper_scale": 8.4}[name]
             r = roofline_of(ins, name, evb["feasible_fraction"], a2, n_s / ms * 1e3, ka, kb, kp, n_s, gi.query(11))
-            c["roofline"] = {k: r[k] for k in ("kernel", "frac", "launch_ms", "candidates_per_launch", "alg2_moves_mean", "kernels",
+            c["roofline"] = {k: r[k] for k in ("kernel", "frac", "binding_pipe", "frac_of_binding_pipe", "launch_ms", "candidates_per_launch", "alg2_moves_mean", "kernels",
                                                "whole_step", "whole_step_strict", "kernel_time_share_of_step", "traffic", "traffic_source")}
             configs[name] = c
             if gi is not g:

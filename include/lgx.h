@@ -65,18 +65,14 @@ extern "C" {
 #define LGX_OPT_THREADS_B   2    /* threads per block of the walk/finish kernel: multiple of 32, 32 .. what fits */
 #define LGX_OPT_THREADS_MV  3    /* threads per block of the move kernels: multiple of 32, 64 .. what fits      */
 #define LGX_OPT_CHUNK_LOG2  4    /* log2 of the candidates per kernel pair, 10 .. 26 (queue memory = chunk * record bytes) */
-#define LGX_OPT_CUT_WARP    6    /* 1: the decode/cut kernel works one candidate per WARP (lgx_decode_cut_w; needs N_F > 255, no
-                                    zero-demand BP, room for the per-warp state of >= 4 warps, and the 2 N_B - 1 - N_T draws of the BP
-                                    partition, rounded up to whole Philox blocks, within the permutation's 32-bit words
-                                    (4 ceil((2 N_B - 1 - N_T) / 4) <= ceil(N_F / 2)): else LGX_EINVAL; lgx_instance_query what 23
-                                    tells), 0 (default): one per thread.
-                                    An alternative mapping kept for measurement: slower on every config so far */
+/* (key 6 was LGX_OPT_CUT_WARP, a one-candidate-per-warp decode/cut kernel that measured slower on every config and was
+ * removed in round 3; profiles/r02_alt_cut_per_warp_paper_scale.md keeps the measurement.  The key is LGX_EINVAL now.) */
 #define LGX_OPT_WALK_LOCKSTEP 7  /* 1: the warps of a walk/finish block draw their queue records together (one barrier per batch; they
                                     then share instruction-cache lines), 0: every warp on its own.  Only with coordinates (distance modes 1, 2;
                                     ignored with the tables, where it measured slower).  Default: 1 with coordinates and N_F < 1024 */
 #define LGX_OPT_SQ_SHIFT    5    /* log2 of the replication of the s_q table in the decode/cut kernel's shared memory, 0 .. 5;
-                                    synchronises the device, uploads a new image and then resets LGX_OPT_THREADS_A and
-                                    LGX_OPT_CUT_WARP to their defaults for the new image size (set this key first).  On
+                                    synchronises the device, uploads a new image and then resets LGX_OPT_THREADS_A to its
+                                    default for the new image size (set this key first).  On
                                     failure (LGX_ETOOBIG, LGX_ECUDA) the instance keeps its previous image and settings */
 
 typedef struct lgx_instance lgx_instance;   /* opaque; owns host + device copies */
@@ -210,9 +206,8 @@ int lgx_decode_batch(const lgx_instance *inst, uint64_t seed,
  * kernel, 10 candidates per kernel pair (chunk), 11 bytes per queue record, 15 / 16 threads per
  * block / shared memory bytes of the move kernels (Algorithm 1 entry points below; 0 threads: they do not fit),
  * 17 log2 of the s_q replication, 18 threads per block of the decode/cut kernel in lgx_decode_batch,
- * 19 per-candidate state bytes of the walk/finish kernel, 20 the instance's CUDA device, 21 decode/cut mapping in
- * use (0 one candidate per thread, 1 per warp), 22 warps per block of the per-warp kernel (0 when not in use),
- * 23 whether the per-warp mapping is possible for this instance (LGX_OPT_CUT_WARP), 24 LGX_OPT_WALK_LOCKSTEP.  */
+ * 19 per-candidate state bytes of the walk/finish kernel, 20 the instance's CUDA device, 24 LGX_OPT_WALK_LOCKSTEP
+ * (21-23 belonged to the removed per-warp decode/cut kernel: LGX_EINVAL).                                      */
 int lgx_instance_query(const lgx_instance *inst, int what, int64_t *out);
 
 /* Launch-configuration knobs (LGX_OPT_* above).  Results never depend on them.              */
@@ -283,6 +278,12 @@ int lgx_local_search(const lgx_instance *inst,
  * (synchronous).  what = 0: the in-line correctly rounded square root of the walk/finish kernel against __dsqrt_rn
  * on n pseudo-random arguments drawn from `seed` (squared coordinate differences, random mantissas over 120 binades,
  * exact squares and their neighbours); h_out[0] = arguments checked, h_out[1] = mismatches (must be 0).
+ * what = 1..5: issue-rate microbenchmark of one execution pipe, n = loop iterations (2^14 takes about a millisecond):
+ * 1 IMAD.WIDE.U32 (Philox's 32x32->64 products), 2 LOP3 (the ALU pipe), 3 LDS.U8 + STS.U8 on per-thread shared-memory
+ * columns, 4 DFMA (the FP64 pipe), 5 MUFU.RSQ64H (the square root's seed); eight independent chains per thread, two
+ * blocks of 1024 threads per SM.  h_out[0] = warp-instructions of that kind issued by the whole grid, h_out[1] = clock
+ * cycles of the slowest block: h_out[0] / h_out[1] / SMs = the pipe's sustained warp-instructions per clock per SM
+ * (bench.py: roofline.pipe_peaks).  `seed` is unused there.
  * Other `what`, n == 0 or a null pointer => LGX_EINVAL.                                                         */
 int lgx_selftest(int what, uint64_t n, uint64_t seed, uint64_t *h_out);
 

@@ -19,7 +19,7 @@ LGX_STATIC_SCRATCH_BYTES = 16 << 20
 # include/lgx.h: descriptor flags and lgx_instance_set_option keys
 LGX_FLAG_HU_BALANCE, LGX_FLAG_MAKESPAN_FILTER, LGX_FLAG_FIX_FIELD_BP = 2, 4, 8
 LGX_FLAG_DIST_COORDS, LGX_FLAG_DIST_MIXED = 16, 32
-LGX_OPT_THREADS_A, LGX_OPT_THREADS_B, LGX_OPT_THREADS_MV, LGX_OPT_CHUNK_LOG2, LGX_OPT_SQ_SHIFT, LGX_OPT_CUT_WARP, LGX_OPT_WALK_LOCKSTEP = 1, 2, 3, 4, 5, 6, 7
+LGX_OPT_THREADS_A, LGX_OPT_THREADS_B, LGX_OPT_THREADS_MV, LGX_OPT_CHUNK_LOG2, LGX_OPT_SQ_SHIFT, LGX_OPT_WALK_LOCKSTEP = 1, 2, 3, 4, 5, 7
 LGX_MAX_BPS, LGX_MAX_SUS, LGX_MAX_MOVE_TOURS, LGX_MAX_MOVE_HUS = 127, 128, 64, 64
 
 _dp = C.POINTER(C.c_double)
@@ -192,7 +192,7 @@ class Instance:
         keys = ["image_bytes", "threads", "grid", "smem_bytes", "coords", "state_bytes", "sm_count", "launches",
                 "threads_finish", "smem_bytes_finish", "chunk", "record_bytes"]
         d = {k: self.query(i) for i, k in enumerate(keys)}
-        d.update(threads_mv=self.query(15), sq_shift=self.query(17), threads_decode=self.query(18), cut_warp=self.query(21), cut_warps=self.query(22),
+        d.update(threads_mv=self.query(15), sq_shift=self.query(17), threads_decode=self.query(18),
                  state_bytes_finish=self.query(19), device=self.query(20))
         return d
 

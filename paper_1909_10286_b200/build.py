@@ -17,14 +17,15 @@ LIB = os.path.join(HERE, "liblgx.so")
 OBJDIR = os.path.join(HERE, "build")
 # (object name, source, extra defines)
 UNITS = [("api", "lgx_api.cu", []),
+         ("pipes", "lgx_pipes.cu", []),
          ("decode", "lgx_inst_decode.cu", []),
          ("walk0", "lgx_inst_walk.cu", ["-DLGX_DM=0"]),
          ("walk1", "lgx_inst_walk.cu", ["-DLGX_DM=1"]),
          ("walk2", "lgx_inst_walk.cu", ["-DLGX_DM=2"]),
          ("moves1", "lgx_inst_moves.cu", ["-DLGX_MASKW=1"]),
          ("moves2", "lgx_inst_moves.cu", ["-DLGX_MASKW=2"])]
-DEPS = [os.path.join(CSRC, f) for f in ("lgx_api.cu", "lgx_inst_decode.cu", "lgx_inst_walk.cu", "lgx_inst_moves.cu",
-                                        "lgx_dispatch.h", "lgx_kernels.cuh", "lgx_cutw.cuh", "lgx_moves.cuh", "lgx_image.h")] + \
+DEPS = [os.path.join(CSRC, f) for f in ("lgx_api.cu", "lgx_pipes.cu", "lgx_inst_decode.cu", "lgx_inst_walk.cu", "lgx_inst_moves.cu",
+                                        "lgx_dispatch.h", "lgx_kernels.cuh", "lgx_moves.cuh", "lgx_image.h")] + \
        [os.path.join(ROOT, "include", "lgx.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

@@ -5,7 +5,6 @@
 #include "lgx_image.h"
 #include "lgx_dispatch.h"
 #include "lgx_moves.cuh"
-#include "lgx_cutw.cuh"
 
 #include <algorithm>
 #include <atomic>
@@ -32,8 +31,6 @@ struct lgx_instance {
   // launch configuration of the persistent kernels (lgx_decode_cut: a, its diagnostic decode mode: a_dec; lgx_walk_finish: b)
   int threads_a = 0, threads_a_dec = 0, threads_b = 0, grid = 0;
   int walk_lockstep = 0;                            // lgx_walk_finish: block-synchronous work fetch (default with coordinates)
-  int cut_warp = 0, cut_warp_ok = 0, warps_w = 0;   // lgx_decode_cut_w (one candidate per warp): in use, possible, warps per block
-  uint32_t w_bytes = 0;                             // its shared memory per warp
   uint64_t a_state = 0, a_state_dec = 0, b_state = 0;   // per-candidate shared-memory bytes
   uint64_t chunk = 0;                          // candidates per decode/finish kernel pair
   cudaMemPool_t pool = nullptr;                // the device's workspace pool (owned by the library, not by the instance)
@@ -130,28 +127,14 @@ int64_t fit_threads(int64_t budget, int64_t image, int64_t state, int64_t cap)
 }
 
 // Launch configuration of the decode/cut kernel as a function of image A's size: the create-time defaults.  Used by
-// lgx_instance_create and again whenever LGX_OPT_SQ_SHIFT has rebuilt the image (it resets LGX_OPT_THREADS_A and
-// LGX_OPT_CUT_WARP to these defaults; nothing is derived from the values in place before).
+// lgx_instance_create and again whenever LGX_OPT_SQ_SHIFT has rebuilt the image (it resets LGX_OPT_THREADS_A to
+// this default; nothing is derived from the values in place before).
 void config_decode_cut(lgx_instance *I)
 {
   const ImgHdr &H = I->hdr;
   const int64_t budget = I->smem_budget;
   I->threads_a     = (int)fit_threads(budget, H.image_bytes, (int64_t)I->a_state, H.perm16 ? kMaxThreadsA16 : kMaxThreadsA);
   I->threads_a_dec = (int)fit_threads(budget, H.image_bytes, (int64_t)I->a_state_dec, H.perm16 ? kMaxThreadsA16 : kMaxThreadsA);
-#ifndef LGX_EMU
-  {
-    // one candidate per warp (lgx_cutw.cuh): possible with 16-bit field ids, no zero-demand BP, the BP partition's draws
-    // inside the permutation's words, and room for at least four warps.  Opt-in (LGX_OPT_CUT_WARP): it measured slower
-    // than the per-thread mapping on every config, so it is never chosen by default
-    const CutWLayout WL = cutw_layout(H);
-    const int64_t wfit = std::min<int64_t>((budget - (int64_t)H.image_bytes) / (int64_t)WL.bytes, kMaxThreadsW / 32);
-    const uint32_t draw_words = 4u * cdiv(2u * (uint32_t)H.n_b - 1u - (uint32_t)H.n_t, 4u);
-    I->w_bytes = WL.bytes;
-    I->warps_w = (int)std::max<int64_t>(wfit, 0);
-    I->cut_warp_ok = (H.perm16 && !H.zero_demand && wfit >= 4 && draw_words <= H.n_perm_words) ? 1 : 0;
-    I->cut_warp = 0;
-  }
-#endif
 }
 
 // Stream-ordered workspace memory (the queue of feasible candidates, a few hundred bytes of counters) comes from ONE
@@ -207,6 +190,8 @@ int allow_max_smem(const void *fn, int smem_optin)
 void pick_move_kernels(const ImgHdr &h, MvKernelFn &kb, MvKernelFn &ks);
 
 }  // namespace
+
+namespace lgx { int pipe_bench(int what, uint64_t iters, uint64_t *h_out); }   // lgx_pipes.cu
 
 extern "C" {
 
@@ -350,7 +335,7 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   // ---- image C: packed distance tables when they leave room for >= 256 candidates per SM, else the
   //      field x BP table + coordinates while the table is small, else coordinates only
   const uint64_t tri_bytes = (uint64_t)(nf + 1) * (uint64_t)nf / 2 * 8, dfb_bytes = (uint64_t)nf * nb * 8;
-  const uint64_t xy_bytes = 16ull * (1 + nb + nf), room = (uint64_t)kMaxSmem - 1024;
+  const uint64_t xy_bytes = 16ull * (1 + nb + nf) + 128ull * nb, room = (uint64_t)kMaxSmem - 1024;   // (+ the BP replicas of mode 1)
   const int n_rcp = std::max(nf, std::max(nb, nhu)) + 1;
   const uint64_t tail_bytes = 8ull * nf + 8ull * nf + 6ull * nsu + 8ull * n_rcp + 2ull * nsu + 8ull * nhu + 2ull * nhu + 320;
   if (tail_bytes + tri_bytes + dfb_bytes + 256ull * I->b_state <= room) H.coords = 0;
@@ -362,7 +347,9 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   H.offc_dtri = H.offc_dfb = H.offc_xy = 0;
   if (H.coords == 0) { H.offc_dtri = off; off = align16(off + (uint32_t)tri_bytes); }
   if (H.coords != 1) { H.offc_dfb = off; off = align16(off + (uint32_t)dfb_bytes); }
-  if (H.coords != 0) { H.offc_xy = off; off = align16(off + (uint32_t)xy_bytes); }
+  if (H.coords != 0) { H.offc_xy = off; off = align16(off + 16u * (uint32_t)(1 + nb + nf)); }
+  H.offc_bxy = 0;
+  if (H.coords == 1) { H.offc_bxy = off; off = align16(off + 16u * 8u * (uint32_t)nb); }   // BP coordinates, 8 interleaved replicas
   H.offc_dhq = 0;
   if (H.coords != 0) { H.offc_dhq = off; off = align16(off + 8u * (uint32_t)nf); }
   H.offc_sh   = off; off = align16(off + 8u * (uint32_t)nf);
@@ -401,6 +388,13 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
   for (int f = 0; f < nf; ++f) { xyv[2 * (1 + nb + f)] = d->field_x[f]; xyv[2 * (1 + nb + f) + 1] = d->field_y[f]; }
   if (H.coords != 0) {
     std::memcpy(imc + H.offc_xy, xyv.data(), xyv.size() * 8);
+    if (H.coords == 1) {
+      // replica r of BP b at entry 8 b + r: lane l of a warp reads replica l & 7, so the eight lanes of a quarter-warp
+      // (one wavefront of a 16-byte load) always hit eight different groups of four banks, whatever BPs they hold
+      double *bx = reinterpret_cast<double *>(imc + H.offc_bxy);
+      for (int b = 0; b < nb; ++b)
+        for (int r = 0; r < 8; ++r) { bx[2 * (8 * b + r)] = d->bp_x[b]; bx[2 * (8 * b + r) + 1] = d->bp_y[b]; }
+    }
     double *dh = reinterpret_cast<double *>(imc + H.offc_dhq);
     for (int f = 0; f < nf; ++f) dh[f] = edge(d->field_x[f], d->field_y[f], d->hq_x, d->hq_y);
   }
@@ -475,10 +469,6 @@ int lgx_instance_create(const lgx_instance_desc *d, lgx_instance **out)
     if (rc == LGX_OK) rc = allow_max_smem((const void *)ka, smem_optin); if (rc == LGX_OK) rc = allow_max_smem((const void *)kb, smem_optin);
     pick_kernels<MODE_DECODE>(H, ka, kb);
     if (rc == LGX_OK) rc = allow_max_smem((const void *)ka, smem_optin); if (rc == LGX_OK) rc = allow_max_smem((const void *)kb, smem_optin);
-    if (I->cut_warp_ok) {
-      if (rc == LGX_OK) rc = allow_max_smem((const void *)pick_decode_cut_w(H, MODE_EVAL), smem_optin);
-      if (rc == LGX_OK) rc = allow_max_smem((const void *)pick_decode_cut_w(H, MODE_SEARCH), smem_optin);
-    }
     if (rc != LGX_OK) { free_instance(I); return rc; }
   }
   // ---- move kernels: shared-memory layout (lgx_moves.cuh) and vertex coordinates for lgx_init_plan
@@ -605,12 +595,6 @@ int lgx_instance_set_option(lgx_instance *I, int key, int64_t value)
       I->walk_lockstep = (int)value;
       return LGX_OK;
     }
-    case LGX_OPT_CUT_WARP: {
-      if (value != 0 && value != 1) return LGX_EINVAL;
-      if (value == 1 && !I->cut_warp_ok) return LGX_EINVAL;
-      I->cut_warp = (int)value;
-      return LGX_OK;
-    }
     case LGX_OPT_SQ_SHIFT: {
       if (value < 0 || value > 5) return LGX_EINVAL;
       const int64_t img = 16 + 4ll * ((int64_t)H.n_f << value) + 16 + 4ll * H.n_b;
@@ -664,12 +648,10 @@ int run_chunks(const lgx_instance *I, KernelFn ka, KernelFn kb, KParams &P, uint
                bool decode_mode, std::vector<cudaEvent_t> *evs = nullptr)
 {
   if (!ka || !kb) return LGX_EINVAL;
-  const bool per_warp = I->cut_warp && !decode_mode;      // lgx_decode_cut_w: a block of warps_w warps works warps_w candidates at a time
-  const uint64_t ta = per_warp ? 32ull * (uint64_t)I->warps_w : LGX_BLOCK_THREADS((uint64_t)(decode_mode ? I->threads_a_dec : I->threads_a));
+  const uint64_t ta = LGX_BLOCK_THREADS((uint64_t)(decode_mode ? I->threads_a_dec : I->threads_a));
   const uint64_t tb = LGX_BLOCK_THREADS((uint64_t)I->threads_b);
-  const uint64_t cand_a = per_warp ? (uint64_t)I->warps_w : ta;          // candidates a block of kernel 1 holds
-  const size_t smem_a = per_warp ? (size_t)I->hdr.image_bytes + (size_t)I->w_bytes * (size_t)I->warps_w
-                                 : (size_t)I->hdr.image_bytes + (size_t)(decode_mode ? I->a_state_dec : I->a_state) * ta;
+  const uint64_t cand_a = ta;                                            // candidates a block of kernel 1 holds
+  const size_t smem_a = (size_t)I->hdr.image_bytes + (size_t)(decode_mode ? I->a_state_dec : I->a_state) * ta;
   const size_t smem_b = (size_t)I->hdr.imagec_bytes + (size_t)I->b_state * tb;
   P.H = I->hdr; P.image = I->d_image; P.image_c = I->d_image_c;
   P.queue = W.queue; P.cap = (uint32_t)W.cap; P.q_count = W.q_count; P.ctr_a = W.ctr_a; P.ctr_b = W.ctr_b;
@@ -702,7 +684,7 @@ int lgx_instance_query(const lgx_instance *I, int what, int64_t *out)
     case 0: *out = (int64_t)I->hdr.image_bytes + I->hdr.imagec_bytes; break;
     case 1: *out = I->threads_a; break;
     case 2: *out = I->grid; break;
-    case 3: *out = I->cut_warp ? (int64_t)I->hdr.image_bytes + (int64_t)I->w_bytes * I->warps_w : (int64_t)I->hdr.image_bytes + (int64_t)I->a_state * I->threads_a; break;
+    case 3: *out = (int64_t)I->hdr.image_bytes + (int64_t)I->a_state * I->threads_a; break;
     case 4: *out = I->hdr.coords; break;
     case 5: *out = (int64_t)I->a_state; break;
     case 6: *out = I->sm_count; break;
@@ -720,9 +702,6 @@ int lgx_instance_query(const lgx_instance *I, int what, int64_t *out)
     case 18: *out = I->threads_a_dec; break;
     case 19: *out = (int64_t)I->b_state; break;
     case 20: *out = I->device; break;
-    case 21: *out = I->cut_warp; break;
-    case 22: *out = I->cut_warp ? I->warps_w : 0; break;
-    case 23: *out = I->cut_warp_ok; break;
     case 24: *out = I->walk_lockstep; break;
     default: return LGX_EINVAL;
   }
@@ -731,7 +710,14 @@ int lgx_instance_query(const lgx_instance *I, int what, int64_t *out)
 
 int lgx_selftest(int what, uint64_t n, uint64_t seed, uint64_t *h_out)
 {
-  if (what != 0 || !h_out || n == 0) return LGX_EINVAL;
+  if (!h_out || n == 0) return LGX_EINVAL;
+#ifndef LGX_EMU
+  if (what >= 1 && what <= 5) {                          // pipe microbenchmarks (lgx_pipes.cu); n = loop iterations
+    const int e = pipe_bench(what, n, h_out);
+    return e == 0 ? LGX_OK : cuda_fail((cudaError_t)e, "lgx_selftest: pipe microbenchmark");
+  }
+#endif
+  if (what != 0) return LGX_EINVAL;
   unsigned long long *d = nullptr;
   CU(cudaMalloc((void **)&d, 16));
   cudaError_t e = cudaMemset(d, 0, 16);
@@ -768,7 +754,6 @@ int lgx_eval_batch(const lgx_instance *I, uint64_t seed, const uint64_t *d_ids, 
   P.ids = d_ids; P.first_id = first_id;
   P.cost = d_cost; P.path_km = d_path_km; P.makespan_h = d_makespan_h; P.feasible = d_feasible;
   KernelFn ka, kb; pick_kernels<MODE_EVAL>(I->hdr, ka, kb);
-  if (I->cut_warp) ka = pick_decode_cut_w(I->hdr, MODE_EVAL);
   Workspace W;
   rc = ws_alloc(I, n, false, st, W);
   if (rc != LGX_OK) return rc;
@@ -811,7 +796,6 @@ int lgx_search_range(const lgx_instance *I, uint64_t seed, uint64_t first_id, ui
   fill_round_keys(P, seed);
   P.ids = nullptr; P.first_id = first_id;
   KernelFn ka, kb; pick_kernels<MODE_SEARCH>(I->hdr, ka, kb);
-  if (I->cut_warp) ka = pick_decode_cut_w(I->hdr, MODE_SEARCH);
   Workspace W;
   rc = ws_alloc(I, n, true, st, W);
   if (rc != LGX_OK) return rc;
@@ -967,7 +951,6 @@ int lgx_eval_batch_static(const lgx_instance *I, uint64_t seed, const uint64_t *
   P.ids = d_ids; P.first_id = first_id;
   P.cost = d_cost; P.path_km = d_path_km; P.makespan_h = d_makespan_h; P.feasible = d_feasible;
   KernelFn ka, kb; pick_kernels<MODE_EVAL>(I->hdr, ka, kb);
-  if (I->cut_warp) ka = pick_decode_cut_w(I->hdr, MODE_EVAL);
   Workspace W;                                                        // same layout as ws_alloc, inside the static array
   W.base = base;
   W.cap = (n + 31) / 32 * 32;                                         // one kernel pair takes the whole call

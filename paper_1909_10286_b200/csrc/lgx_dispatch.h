@@ -13,8 +13,6 @@ using MvKernelFn = void (*)(const MvParams);
 
 // lgx_decode_cut<P16, ZD, XB64, mode> for the instance (lgx_inst_decode.cu); mode = MODE_EVAL / _SEARCH / _DECODE
 KernelFn pick_decode_cut(const ImgHdr &h, int mode);
-// lgx_decode_cut_w<XB64, mode>: one candidate per warp (lgx_cutw.cuh, lgx_inst_decode.cu); MODE_EVAL / _SEARCH only
-KernelFn pick_decode_cut_w(const ImgHdr &h, int mode);
 // lgx_walk_finish<P16, DM, MASKW, mode>, one translation unit per distance mode DM (lgx_inst_walk.cu, -DLGX_DM=0|1|2)
 KernelFn pick_walk_finish_dm0(const ImgHdr &h, int mode);
 KernelFn pick_walk_finish_dm1(const ImgHdr &h, int mode);

@@ -68,6 +68,8 @@ struct ImgHdr {
   uint32_t offc_dtri;       // f64 [(n_f+1) n_f / 2]  strict lower triangle over {HQ, fields}      (mode 0)
   uint32_t offc_dfb;        // f64 [n_f][n_b]         field -> BP legs                              (modes 0, 2)
   uint32_t offc_xy;         // f64x2 [1 + n_b + n_f]  vertex coordinates                            (modes 1, 2)
+  uint32_t offc_bxy;        // f64x2 [n_b][8]         BP coordinates, replica r of BP b at 8 b + r (lane l reads replica l & 7:
+                            //                        the 16-byte loads of a quarter-warp never share a bank group)  (mode 1)
   uint32_t offc_dhq;        // f64 [n_f]              field -> HQ legs (the closing leg of a tour)  (modes 1, 2)
   uint32_t offc_sh;         // u32x2 [n_f]            {s_q, h_q}
   uint32_t offc_suinit;     // u32 [..]    initial array of the SU partition: capacity ranks of units 0.., right-aligned bytes
@@ -94,7 +96,6 @@ struct ImgHdr {
   //   0,1 index i | bpseq words | segend words | perm words
   uint32_t rec_bpseq, rec_segend, rec_perm, rec_words;
   uint32_t n_bpseq_words, n_segend_words, n_perm_words;
-  uint32_t pad_[1];
 };
 static_assert(sizeof(ImgHdr) % 16 == 0, "image header must keep 16-byte alignment");
 

@@ -2,7 +2,6 @@
 // Product code (CUDA path).  Shares nothing with oracle/.
 #define LGX_INSTANTIATE_SELFTEST
 #include "lgx_dispatch.h"
-#include "lgx_cutw.cuh"
 
 namespace lgx {
 
@@ -25,17 +24,6 @@ KernelFn pick_decode_cut(const ImgHdr &h, int mode)
     case MODE_DECODE: return pick_a<MODE_DECODE>(h);
     default:          return nullptr;
   }
-}
-
-KernelFn pick_decode_cut_w(const ImgHdr &h, int mode)
-{
-#ifndef LGX_EMU
-  const bool x64 = h.n_extra_blocks > 7u;
-  if (mode == MODE_EVAL)   return x64 ? lgx_decode_cut_w<true, MODE_EVAL>   : lgx_decode_cut_w<false, MODE_EVAL>;
-  if (mode == MODE_SEARCH) return x64 ? lgx_decode_cut_w<true, MODE_SEARCH> : lgx_decode_cut_w<false, MODE_SEARCH>;
-#endif
-  (void)h; (void)mode;
-  return nullptr;
 }
 
 const void *selftest_sqrt_kernel() { return (const void *)lgx_selftest_sqrt_k; }

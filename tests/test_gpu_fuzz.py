@@ -69,8 +69,6 @@ def test_random_instance(k):
         modes = [(None, None)]
         if g.query(4) != 0:
             modes.append((binding.LGX_OPT_WALK_LOCKSTEP, 1 - g.query(24)))
-        if g.query(23):
-            modes.append((binding.LGX_OPT_CUT_WARP, 1))
         for key, val in modes:
             if key is not None:
                 g.set_option(key, val)

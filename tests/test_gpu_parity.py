@@ -367,63 +367,6 @@ def test_field_count_boundaries(nf):
     g.close()
 
 
-def _truncated(base, nf):
-    from dataclasses import replace
-    z = wl.make(base)
-    return replace(z, field_xy=z.field_xy[:nf].copy(), field_supply_t=z.field_supply_t[:nf].copy(), field_area_ha=z.field_area_ha[:nf].copy(),
-                   bp_demand_t=z.bp_demand_t * (0.9 * z.field_supply_t[:nf].sum() / z.bp_demand_t.sum()))
-
-
-@pytest.mark.parametrize("case", ["sweep", "paper_scale", 257, 290, 511, 641, 1023, 1025, 1187])
-def test_cut_per_warp_matches_oracle(case):
-    """lgx_decode_cut_w (one candidate per warp, LGX_OPT_CUT_WARP = 1): the same flags, costs, argmin and — through the
-    queue records the walk kernel reads — the same plans as the oracle, on the configs with N_F > 255 and on field
-    counts that exercise every tail length of the 32-position blocks and of the 128-draw Philox rounds; ids >= 2^32;
-    more candidates than one grid round; tight demand (many infeasible candidates)."""
-    z = wl.make(case) if isinstance(case, str) else _truncated("paper_scale", case)
-    o, g = lgo.Oracle(z), binding.Instance(z)
-    assert g.query(23) == 1
-    g.set_option(binding.LGX_OPT_CUT_WARP, 1)
-    assert g.query(21) == 1 and g.query(22) >= 4
-    n = 768 if z.n_fields > 600 else 1536
-    for seed, first in ((z.seed, 0), (11, (1 << 40) + 5)):
-        want = o.eval_batch(seed, first_id=first, n=n)
-        got = [t.cpu().numpy() for t in g.eval_batch(seed, first_id=first, n=n)]
-        assert np.array_equal(got[3], want[3])
-        for k in range(3):
-            assert_costs(got[k], want[k], f"{case} output {k}")
-        assert g.search(seed, n, first_id=first) == o.search(seed, n, first_id=first)
-    # the per-thread mapping gives the same bits on a larger sample (several grid rounds of the per-warp kernel)
-    m = 1 << 15
-    a = [t.clone() for t in g.eval_batch(z.seed, first_id=77, n=m)]
-    g.set_option(binding.LGX_OPT_CUT_WARP, 0)
-    assert g.query(21) == 0
-    b = g.eval_batch(z.seed, first_id=77, n=m)
-    assert all(torch.equal(x, y) for x, y in zip(a, b))
-    g.close()
-    # tight demand: most candidates fail eq. (2)
-    from dataclasses import replace
-    t = replace(z, bp_demand_t=z.bp_demand_t * 1.08)
-    ot, gt = lgo.Oracle(t), binding.Instance(t)
-    gt.set_option(binding.LGX_OPT_CUT_WARP, 1)
-    want = ot.eval_batch(3, first_id=0, n=512)
-    got = [x.cpu().numpy() for x in gt.eval_batch(3, first_id=0, n=512)]
-    assert np.array_equal(got[3], want[3]) and np.array_equal(got[0], want[0])
-    gt.close()
-
-
-def test_cut_per_warp_is_refused_where_it_cannot_work():
-    """8-bit field ids and zero-demand BPs keep the per-thread kernel: LGX_OPT_CUT_WARP = 1 is LGX_EINVAL there."""
-    for inst in (wl.make("medium"),):
-        g = binding.Instance(inst)
-        assert g.query(23) == 0
-        with pytest.raises(binding.LgxError):
-            g.set_option(binding.LGX_OPT_CUT_WARP, 1)
-        g.close()
-    z = wl.make("sweep"); z.bp_demand_t = z.bp_demand_t.copy(); z.bp_demand_t[2] = 0.0
-    g = binding.Instance(z)
-    assert g.query(23) == 0 and g.query(21) == 0
-    g.close()
 
 
 @pytest.mark.parametrize("name", ["small", "large", "sweep", "paper_scale"])
@@ -443,3 +386,17 @@ def test_walk_lockstep_does_not_change_results(ctxs, name):
     assert all(torch.equal(a, b) for a, b in zip(outs[0][:4], outs[1][:4])) and outs[0][4:] == outs[1][4:]
     want = o.eval_batch(inst.seed, first_id=9, n=512)
     assert np.array_equal(outs[1][0][:512].cpu().numpy(), want[0]) and np.array_equal(outs[1][3][:512].cpu().numpy(), want[3])
+
+
+def test_pipe_microbenchmarks_report_plausible_rates():
+    """lgx_selftest what = 1..5 (include/lgx.h): sustained warp-instructions per clock per SM of five pipes.  No pipe
+    can beat the four schedulers of an SM, and each of these is known to be a fraction of that; the bounds are wide
+    (they guard the counting and the clock arithmetic, not a particular GPU)."""
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    for what, lo, hi in ((1, 0.4, 2.1), (2, 0.9, 4.01), (3, 0.4, 2.1), (4, 0.02, 2.1), (5, 0.1, 1.1)):
+        n_inst, cycles = binding.selftest(what, 1 << 13)
+        assert n_inst == 2 * sms * 32 * (1 << 13) * 4 * 8 * (2 if what in (2, 3) else 1) and cycles > 0
+        rate = n_inst / cycles / sms
+        assert lo <= rate <= hi, (what, rate)
+    with pytest.raises(binding.LgxError):
+        binding.selftest(6, 1 << 10)
