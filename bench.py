@@ -99,10 +99,10 @@ SM_MAX_MHZ_FALLBACK = 1965.0
 # (everything lives in shared memory and the L2-resident queue); these numbers show the real traffic is negligible.
 TRAFFIC = {
     # name: (capture, candidates the captured kernel pair covered, bytes of lgx_decode_cut, bytes of lgx_walk_finish)
-    "medium":      ("profiles/r02_medium_ncu_full.md", 16777216, 4.409e8, 4.995e8),
-    "large":       ("profiles/r02_large_ncu_full.md", 932068, 1.784e8, 2.390e8),
-    "sweep":       ("profiles/r02_sweep_ncu_full.md", 1973790, 2.088e9, 2.252e9),
-    "paper_scale": ("profiles/r02_paper_scale_ncu_full.md", 860370, 2.086e9, 4.059e9),
+    "medium":      ("profiles/r03_medium_ncu_full.md", 16777216, 4.412e+08, 5.019e+08),
+    "large":       ("profiles/r03_large_ncu_full.md", 932068, 1.765e+08, 2.399e+08),
+    "sweep":       ("profiles/r03_sweep_ncu_full.md", 123362, 3.452e+07, 9.736e+07),
+    "paper_scale": ("profiles/r03_paper_scale_ncu_full.md", 188206, 3.838e+08, 8.302e+08),
 }
 
 
